@@ -1,0 +1,157 @@
+/*
+ * lsp.h -- C ABI of the B200-native batched Lomb-Scargle periodogram library (liblsp_b200.so).
+ *
+ * What the library computes (arXiv 2105.04006, section 2):
+ *   - time series (t_j, X_j), j = 1..N_t, unevenly sampled, assumed zero-mean
+ *   - omega = 2*pi*f; Scargle offset  tan 2 omega tau = sum sin 2 omega t_j / sum cos 2 omega t_j   Eq. 1
+ *   - P_LS(f) = 1/2 ( [sum X_j cos omega(t_j-tau)]^2 / sum cos^2 omega(t_j-tau)
+ *                   + [sum X_j sin omega(t_j-tau)]^2 / sum sin^2 omega(t_j-tau) )      Eq. 2
+ *   - evenly spaced grid on [f_min, f_max): df = (f_max - f_min)/N_f, f_k = f_min + k df, k = 0..N_f-1
+ *   - one grid shared by every object of a batch
+ *   - FP32 or FP64 selectable
+ *   - returning the periodogram is optional; best period = argmax_k P(f_k)
+ *   - periodograms returned to the host go through several CUDA streams and pinned memory, overlapped
+ *     with the computation of later objects
+ *
+ * Conventions:
+ *   - f is CYCLIC (cycles per unit of t), omega = 2 pi f is formed inside; period = 1/f          (a1)
+ *   - f_max itself is not sampled                                                                (a2)
+ *   - output is Eq. 2 exactly as printed ("non-normalised"); normalize=1 divides by 1/2 sum y^2   (a3)
+ *   - y is used as given; center=1 subtracts the per-object mean first                           (a4)
+ *   - argmax: lowest index wins exact ties, NaN never wins                                       (a7)
+ *   - the LS period 1/f_k* is returned, never doubled                                            (a8)
+ *
+ * All entry points are plain C: pointers are labelled HOST or DEVICE, sizes are int64_t, no C++ or
+ * torch types cross this boundary.  No entry point throws or aborts; every failure is a status code,
+ * with a message available from lsp_last_error().  There is no CPU fallback anywhere: without a CUDA
+ * device lsp_plan_create fails with LSP_ERR_CUDA.
+ */
+#ifndef LSP_B200_H
+#define LSP_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lsp_plan lsp_plan; /* opaque; created by lsp_plan_create, freed by lsp_destroy */
+
+typedef enum { LSP_F32 = 0, LSP_F64 = 1 } lsp_dtype;
+
+typedef enum {
+    LSP_OK = 0,
+    LSP_ERR_INVALID_ARG = 1,
+    LSP_ERR_CUDA = 2,
+    LSP_ERR_OOM = 3,
+    LSP_ERR_UNSUPPORTED = 4
+} lsp_status;
+
+/* Which periodogram kernel family runs steps 2-5 of the hot path. */
+typedef enum {
+    LSP_KERNEL_AUTO = 0,     /* library picks (factored unless the problem is too small to fill it)     */
+    LSP_KERNEL_DIRECT = 1,   /* one sincos per (t,f) pair, thread = frequency (the paper's Listing 1 shape,
+                                PAPER.md:L137-216, with smem staging L121-125 and range-reduced phase)     */
+    LSP_KERNEL_FACTORED = 2  /* angle-addition outer product: no sincos in the O(N_t N_f) loop, 4 FMA/pair */
+} lsp_kernel;
+
+typedef struct lsp_config {
+    double  f_min;          /* cycles per unit of t; 0 < f_min < f_max                                     */
+    double  f_max;          /* NOT sampled: last frequency is f_max - df */
+    int64_t n_freq;         /* N_f >= 1 (<= 2^31 - 1)                                                      */
+    int32_t dtype;          /* lsp_dtype: element type of t, y, power, best_period, best_power             */
+    int32_t fast_math;      /* FP32 only: 1 = MUFU.SIN/COS (__sincosf class), 0 = accurate   */
+    int32_t normalize;      /* 0 = Eq. 2 as printed; 1 = divide by (1/2) sum_j y_j^2 per object            */
+    int32_t center;         /* 0 = y as given (paper: caller centres); 1 = subtract mean */
+    int32_t device;         /* CUDA device ordinal                                                         */
+    int32_t n_copy_streams; /* D2H streams for host output (paper: 3); 0 = default (3)      */
+    int64_t chunk_bytes;    /* device staging chunk for host output (paper: 8 MiB); 0 = library default    */
+    int64_t max_objects;    /* scratch sizing hints; 0 = size on first use (scratch grows when needed)     */
+    int64_t max_total_obs;
+    int32_t kernel;         /* lsp_kernel                                                                  */
+    int32_t reserved;       /* must be 0                                                                   */
+} lsp_config;
+
+/*
+ * Create a plan: validates cfg, selects the device, creates the D2H copy streams and events and
+ * allocates scratch (argmax partials, split-N_t partial sums, the device chunk ring for host output).
+ * The plan owns all of that; the caller owns every buffer passed to the calls below.
+ * Errors: LSP_ERR_INVALID_ARG (f_min <= 0, f_max <= f_min, n_freq < 1, fast_math with FP64, unknown
+ * enum, reserved != 0), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
+ * failure.  A plan is not thread-safe; distinct plans are independent.
+ */
+lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan /* HOST */);
+
+/*
+ * Full periodogram of a CSR batch (hot-path steps 1-6, and 7 when the output is on the host;
+ * PAPER.md:L85, L103, L109, L113, L117).
+ *   n_obj        objects in the batch (>= 0; 1 = the paper's single-object mode)
+ *   d_offsets    DEVICE, int64[n_obj+1], offsets[0] = 0, non-decreasing; object o owns [offsets[o], offsets[o+1])
+ *   h_offsets    HOST copy of the same array, or NULL (the library then reads offsets back itself:
+ *                one small synchronous D2H on the call's stream)
+ *   d_t, d_y     DEVICE, offsets[n_obj] elements of cfg.dtype: times and magnitudes, concatenated
+ *   out_power    n_obj * n_freq elements of cfg.dtype, row-major by object:
+ *                a DEVICE pointer when out_is_host == 0, else a HOST pointer (pinned for overlap; pageable
+ *                memory works but serialises) filled through the plan's chunk ring and copy streams
+ *   d_best_*     DEVICE, optional (all three NULL or all three non-NULL): per object best period
+ *                (cfg.dtype), its power (cfg.dtype) and grid index (int64; -1 and NaN period when N_t = 0)
+ *   cuda_stream  cudaStream_t as void* (NULL = default stream).  Device-output calls are asynchronous
+ *                on it; host-output calls return after the last chunk has landed in out_power.
+ * Errors: LSP_ERR_INVALID_ARG (NULL where required, n_obj < 0, bad offsets when h_offsets is given),
+ * LSP_ERR_CUDA, LSP_ERR_OOM.  Outputs are unspecified after an error.
+ */
+lsp_status lsp_periodogram_batched(lsp_plan* plan, int64_t n_obj,
+                                   const int64_t* d_offsets, const int64_t* h_offsets,
+                                   const void* d_t, const void* d_y,
+                                   void* out_power, int32_t out_is_host,
+                                   void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                                   void* cuda_stream);
+
+/*
+ * Best period per object with the argmax fused into the periodogram kernels: the N_obj x N_f array
+ * is never written to memory (space O(N_t + N_o)).  Arguments as above; all three
+ * outputs are required.  Asynchronous on cuda_stream.
+ */
+lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj,
+                           const int64_t* d_offsets, const int64_t* h_offsets,
+                           const void* d_t, const void* d_y,
+                           void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                           void* cuda_stream);
+
+/* Frees the plan and everything it owns (synchronises its streams first).  NULL is a no-op. */
+void lsp_destroy(lsp_plan* plan);
+
+/* Message of the last failure on this plan (plan-owned, valid until the next call on the plan); with
+ * plan == NULL, the message of the last failed lsp_plan_create on this thread.  Never NULL. */
+const char* lsp_last_error(const lsp_plan* plan);
+
+/* Bookkeeping of the LAST call on the plan, for benchmarks: how many of the library's kernels it launched,
+ * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), and --
+ * host-output calls only -- chunks copied.  Any pointer may be NULL. */
+void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used,
+                        int32_t* n_split, int64_t* n_chunks);
+
+/*
+ * Device time of the periodogram kernel(s) of the LAST call, in milliseconds, measured with CUDA events
+ * recorded on the launching stream around the dominant kernel (bench.py's roofline.achieved).  Enabled by
+ * lsp_set_timing(plan, 1); the query synchronises on the stop event.  Returns < 0 if timing was off.
+ */
+void  lsp_set_timing(lsp_plan* plan, int32_t on);
+float lsp_last_kernel_ms(lsp_plan* plan);
+
+/*
+ * Pipe-peak microbenchmark used for the roofline denominators: runs a register-only
+ * loop of one instruction class on every SM and returns the measured thread-level operations per second.
+ *   which: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2, counted as 2 FMA per lane), 2 = DFMA, 3 = MUFU.SIN+MUFU.COS (counted
+ *          as 2 ops), 4 = FFMA2 with one LDS.128 per 8 (the factored kernel's inner-loop mix)
+ * Returns LSP_OK and writes *ops_per_s (HOST) and *sm_mhz_est (HOST, may be NULL): ops / (SMs * lanes) is left to the caller.
+ */
+lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, double* elapsed_ms);
+
+/* Library version / build string (static). */
+const char* lsp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LSP_B200_H */

@@ -1,0 +1,18 @@
+"""B200-native batched Lomb-Scargle periodogram (arXiv 2105.04006 hot path).
+
+The product is the C-ABI CUDA library `liblsp_b200.so` (include/lsp.h, sources under csrc/); this package is
+its thin Python binding.  There is no CPU fallback: the calls fail loudly without the library or a GPU.
+"""
+from .binding import (  # noqa: F401
+    EXPORTS,
+    LspConfig,
+    LspError,
+    Plan,
+    load_library,
+    lsp_best_period,
+    lsp_destroy,
+    lsp_periodogram_batched,
+    lsp_pipe_peak,
+    lsp_plan_create,
+    lsp_version,
+)

@@ -1,0 +1,228 @@
+"""Thin ctypes binding of liblsp_b200.so (include/lsp.h).  Argument marshalling only: every step of the
+Lomb-Scargle hot path runs inside the CUDA library; torch is used for device memory and streams.
+
+The module-level functions carry the C ABI's names (lsp_plan_create, lsp_periodogram_batched, lsp_best_period,
+lsp_destroy); `Plan` is a small convenience wrapper around them.  If the shared library is missing and cannot
+be built, importing this module raises: there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+from . import build as _build
+
+LSP_F32, LSP_F64 = 0, 1
+LSP_KERNEL_AUTO, LSP_KERNEL_DIRECT, LSP_KERNEL_FACTORED = 0, 1, 2
+LSP_OK, LSP_ERR_INVALID_ARG, LSP_ERR_CUDA, LSP_ERR_OOM, LSP_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
+_STATUS = {0: "LSP_OK", 1: "LSP_ERR_INVALID_ARG", 2: "LSP_ERR_CUDA", 3: "LSP_ERR_OOM", 4: "LSP_ERR_UNSUPPORTED"}
+_KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LSP_KERNEL_FACTORED}
+_KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
+
+EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_destroy", "lsp_last_error",
+           "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_pipe_peak", "lsp_version")
+
+
+class LspConfig(ctypes.Structure):
+    """struct lsp_config of include/lsp.h (field order and widths must match)."""
+    _fields_ = [
+        ("f_min", ctypes.c_double), ("f_max", ctypes.c_double), ("n_freq", ctypes.c_int64),
+        ("dtype", ctypes.c_int32), ("fast_math", ctypes.c_int32), ("normalize", ctypes.c_int32),
+        ("center", ctypes.c_int32), ("device", ctypes.c_int32), ("n_copy_streams", ctypes.c_int32),
+        ("chunk_bytes", ctypes.c_int64), ("max_objects", ctypes.c_int64), ("max_total_obs", ctypes.c_int64),
+        ("kernel", ctypes.c_int32), ("reserved", ctypes.c_int32),
+    ]
+
+
+class LspError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"{_STATUS.get(status, status)}: {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None) -> ctypes.CDLL:
+    """dlopen the in-tree liblsp_b200.so (building it with nvcc first if it is missing or stale)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    lib = ctypes.CDLL(path or _build.build())
+    vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+    lib.lsp_plan_create.argtypes = [ctypes.POINTER(LspConfig), ctypes.POINTER(vp)]
+    lib.lsp_plan_create.restype = ctypes.c_int
+    lib.lsp_periodogram_batched.argtypes = [vp, i64, vp, vp, vp, vp, vp, i32, vp, vp, vp, vp]
+    lib.lsp_periodogram_batched.restype = ctypes.c_int
+    lib.lsp_best_period.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.lsp_best_period.restype = ctypes.c_int
+    lib.lsp_destroy.argtypes = [vp]
+    lib.lsp_destroy.restype = None
+    lib.lsp_last_error.argtypes = [vp]
+    lib.lsp_last_error.restype = ctypes.c_char_p
+    lib.lsp_last_call_info.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i32),
+                                       ctypes.POINTER(i32), ctypes.POINTER(i64)]
+    lib.lsp_last_call_info.restype = None
+    lib.lsp_set_timing.argtypes = [vp, i32]
+    lib.lsp_set_timing.restype = None
+    lib.lsp_last_kernel_ms.argtypes = [vp]
+    lib.lsp_last_kernel_ms.restype = ctypes.c_float
+    lib.lsp_pipe_peak.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    lib.lsp_pipe_peak.restype = ctypes.c_int
+    lib.lsp_version.argtypes = []
+    lib.lsp_version.restype = ctypes.c_char_p
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _check(status: int, plan=None):
+    if status != LSP_OK:
+        msg = load_library().lsp_last_error(plan).decode(errors="replace")
+        raise LspError(status, msg)
+
+
+def _dptr(x: Optional[torch.Tensor]):
+    return None if x is None else ctypes.c_void_p(x.data_ptr())
+
+
+def _stream_ptr(stream) -> ctypes.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+# ---- the C ABI's four calls, same names ---------------------------------------------------------------------
+def lsp_plan_create(cfg: LspConfig) -> ctypes.c_void_p:
+    plan = ctypes.c_void_p()
+    _check(load_library().lsp_plan_create(ctypes.byref(cfg), ctypes.byref(plan)))
+    return plan
+
+
+def lsp_periodogram_batched(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y, out_power, out_is_host: bool,
+                            d_best_period=None, d_best_power=None, d_best_index=None, stream=None) -> None:
+    h_ptr = None if h_offsets is None else ctypes.c_void_p(h_offsets.data_ptr())
+    _check(load_library().lsp_periodogram_batched(plan, int(n_obj), _dptr(d_offsets), h_ptr, _dptr(d_t), _dptr(d_y),
+                                                  _dptr(out_power), int(bool(out_is_host)), _dptr(d_best_period),
+                                                  _dptr(d_best_power), _dptr(d_best_index), _stream_ptr(stream)), plan)
+
+
+def lsp_best_period(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y, d_best_period, d_best_power, d_best_index,
+                    stream=None) -> None:
+    h_ptr = None if h_offsets is None else ctypes.c_void_p(h_offsets.data_ptr())
+    _check(load_library().lsp_best_period(plan, int(n_obj), _dptr(d_offsets), h_ptr, _dptr(d_t), _dptr(d_y),
+                                          _dptr(d_best_period), _dptr(d_best_power), _dptr(d_best_index),
+                                          _stream_ptr(stream)), plan)
+
+
+def lsp_destroy(plan) -> None:
+    load_library().lsp_destroy(plan)
+
+
+def lsp_pipe_peak(which: int, device: int = 0):
+    """(ops_per_s, elapsed_ms) of the pipe microbenchmark `which` (see include/lsp.h)."""
+    ops, ms = ctypes.c_double(), ctypes.c_double()
+    _check(load_library().lsp_pipe_peak(int(device), int(which), ctypes.byref(ops), ctypes.byref(ms)))
+    return ops.value, ms.value
+
+
+def lsp_version() -> str:
+    return load_library().lsp_version().decode()
+
+
+# ---- convenience wrapper ---------------------------------------------------------------------------------------
+class Plan:
+    """One frequency grid + precision + output conventions (lsp_plan).  Buffers are torch tensors."""
+
+    def __init__(self, f_min: float, f_max: float, n_freq: int, dtype: str = "f32", *, fast_math: bool = False,
+                 normalize: bool = False, center: bool = False, device: int = 0, n_copy_streams: int = 0,
+                 chunk_bytes: int = 0, kernel: str = "auto", max_objects: int = 0, max_total_obs: int = 0):
+        if dtype not in ("f32", "f64"):
+            raise ValueError("dtype must be 'f32' or 'f64'")
+        self.cfg = LspConfig(float(f_min), float(f_max), int(n_freq), LSP_F32 if dtype == "f32" else LSP_F64,
+                             int(fast_math), int(normalize), int(center), int(device), int(n_copy_streams),
+                             int(chunk_bytes), int(max_objects), int(max_total_obs), _KERNELS[kernel], 0)
+        self.dtype = dtype
+        self.torch_dtype = torch.float32 if dtype == "f32" else torch.float64
+        self.n_freq = int(n_freq)
+        self.device = torch.device("cuda", device)
+        self._plan = lsp_plan_create(self.cfg)
+
+    # -- life cycle
+    def destroy(self):
+        if getattr(self, "_plan", None) is not None:
+            lsp_destroy(self._plan)
+            self._plan = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    # -- helpers
+    def _check_inputs(self, offsets, t, y):
+        if offsets.dtype != torch.int64 or not offsets.is_cuda:
+            raise TypeError("offsets must be a CUDA int64 tensor")
+        for x in (t, y):
+            if x.dtype != self.torch_dtype or not x.is_cuda or not x.is_contiguous():
+                raise TypeError(f"t and y must be contiguous CUDA tensors of {self.torch_dtype}")
+        return int(offsets.numel() - 1)
+
+    def set_timing(self, on: bool):
+        load_library().lsp_set_timing(self._plan, int(on))
+
+    def last_kernel_ms(self) -> float:
+        return float(load_library().lsp_last_kernel_ms(self._plan))
+
+    def last_call_info(self) -> dict:
+        nl, npairs, nch = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        ku, ns = ctypes.c_int32(), ctypes.c_int32()
+        load_library().lsp_last_call_info(self._plan, ctypes.byref(nl), ctypes.byref(npairs), ctypes.byref(ku),
+                                          ctypes.byref(ns), ctypes.byref(nch))
+        return {"launches": nl.value, "pairs": npairs.value, "kernel": _KERNEL_NAMES.get(ku.value, ku.value),
+                "n_split": ns.value, "chunks": nch.value}
+
+    # -- the two calls
+    def periodogram_batched(self, offsets, t, y, *, out=None, host_out=None, best: bool = False, h_offsets=None,
+                            stream=None):
+        """Full periodogram.  Returns (power, best) where power is `out` (device), `host_out` (host) or a new
+        device tensor [n_obj, n_freq], and best is None or (period, power, index) device tensors."""
+        n_obj = self._check_inputs(offsets, t, y)
+        if host_out is not None:
+            if host_out.is_cuda or host_out.dtype != self.torch_dtype or host_out.numel() != n_obj * self.n_freq \
+                    or not host_out.is_contiguous():
+                raise TypeError("host_out must be a contiguous host tensor [n_obj, n_freq] of the plan dtype")
+            power, is_host = host_out, True
+        else:
+            power = out if out is not None else torch.empty((n_obj, self.n_freq), dtype=self.torch_dtype, device=self.device)
+            if not power.is_cuda or power.dtype != self.torch_dtype or power.numel() != n_obj * self.n_freq \
+                    or not power.is_contiguous():
+                raise TypeError("out must be a contiguous CUDA tensor [n_obj, n_freq] of the plan dtype")
+            is_host = False
+        bp = bw = bi = None
+        if best:
+            bp = torch.empty(n_obj, dtype=self.torch_dtype, device=self.device)
+            bw = torch.empty(n_obj, dtype=self.torch_dtype, device=self.device)
+            bi = torch.empty(n_obj, dtype=torch.int64, device=self.device)
+        lsp_periodogram_batched(self._plan, n_obj, offsets, h_offsets, t, y, power, is_host, bp, bw, bi, stream)
+        return power, ((bp, bw, bi) if best else None)
+
+    def best_period(self, offsets, t, y, *, out=None, h_offsets=None, stream=None):
+        """Fused best period: (period, power, index) device tensors; the periodogram is never materialised."""
+        n_obj = self._check_inputs(offsets, t, y)
+        if out is None:
+            out = (torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),
+                   torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),
+                   torch.empty(n_obj, dtype=torch.int64, device=self.device))
+        lsp_best_period(self._plan, n_obj, offsets, h_offsets, t, y, out[0], out[1], out[2], stream)
+        return out

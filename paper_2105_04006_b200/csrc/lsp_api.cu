@@ -1,0 +1,587 @@
+// lsp_api.cu -- the C ABI of include/lsp.h: plan object, argument validation, scheduling (hot-path step 1),
+// kernel launches (steps 2-6') and the pinned-host multi-stream D2H pipeline (step 7).
+// There is no CPU fallback in this file or anywhere in the library.
+#include "../../include/lsp.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "lsp_factored_ws.cuh"
+#include "lsp_peak.cuh"
+
+using namespace lsp;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct DeviceBuffer {
+    void*  ptr = nullptr;
+    size_t bytes = 0;
+};
+
+}  // namespace
+
+struct lsp_plan {
+    lsp_config cfg{};
+    int sm_count = 0;
+    std::string error;
+
+    std::vector<cudaStream_t> copy_streams;
+    std::vector<cudaEvent_t> slot_ready, slot_free;
+    std::vector<char> slot_used;
+    DeviceBuffer ring;            // n_slots * slot_bytes
+    DeviceBuffer partials;        // Best[n_obj * n_parts]
+    DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
+    DeviceBuffer stats;           // ObjStats[n_obj]
+    DeviceBuffer counter;         // work counter of the persistent kernel
+    bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
+    int64_t* h_offsets_pinned = nullptr;
+    size_t   h_offsets_cap = 0;
+
+    // last-call bookkeeping
+    int64_t n_launches = 0, n_pairs = 0, n_chunks = 0;
+    int32_t kernel_used = 0, n_split = 1;
+    bool timing = false;
+    std::vector<cudaEvent_t> t_start, t_stop;
+    size_t t_used = 0;
+};
+
+namespace {
+
+lsp_status fail(lsp_plan* p, lsp_status st, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (p) p->error = buf; else g_create_error = buf;
+    return st;
+}
+
+#define LSP_CUDA(p, call)                                                                              \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail((p), e_ == cudaErrorMemoryAllocation ? LSP_ERR_OOM : LSP_ERR_CUDA, "%s: %s",  \
+                        #call, cudaGetErrorString(e_));                                                \
+    } while (0)
+
+lsp_status ensure(lsp_plan* p, DeviceBuffer& b, size_t bytes)
+{
+    if (bytes <= b.bytes) return LSP_OK;
+    if (b.ptr) {
+        LSP_CUDA(p, cudaFree(b.ptr));
+        b.ptr = nullptr;
+        b.bytes = 0;
+    }
+    LSP_CUDA(p, cudaMalloc(&b.ptr, bytes));
+    b.bytes = bytes;
+    return LSP_OK;
+}
+
+size_t elem_size(const lsp_config& c) { return c.dtype == LSP_F32 ? 4 : 8; }
+
+// ---- step 1: scheduling ------------------------------------------------------------------------------------
+struct Schedule {
+    int kernel;      // LSP_KERNEL_DIRECT / LSP_KERNEL_FACTORED
+    int direct_r;    // frequencies per thread of the direct kernel (1 or 4)
+    int tile;        // frequencies per CTA
+    int n_tiles;
+    int n_split;
+};
+
+Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
+{
+    const lsp_config& c = p->cfg;
+    Schedule s{};
+    int k = c.kernel;
+    if (k == LSP_KERNEL_AUTO) k = (c.n_freq >= 1024) ? LSP_KERNEL_FACTORED : LSP_KERNEL_DIRECT;
+    s.kernel = k;
+    int64_t slots;                                                // resident CTAs on the whole GPU
+    if (k == LSP_KERNEL_FACTORED) {
+        s.tile = c.dtype == LSP_F32 ? fac_tile<float>() : fac_tile<double>();
+        s.direct_r = 0;
+        slots = p->use_ws ? (int64_t)p->sm_count                  // one persistent CTA per SM
+                          : (int64_t)p->sm_count * 2;             // __launch_bounds__(256, 2)
+    } else {
+        const int64_t tiles4 = (c.n_freq + 4 * kDirectThreads - 1) / (4 * kDirectThreads);
+        s.direct_r = (n_obj * tiles4 >= (int64_t)p->sm_count * 8) ? 4 : 1;
+        s.tile = s.direct_r * kDirectThreads;
+        slots = (int64_t)p->sm_count * (s.direct_r == 4 ? (c.dtype == LSP_F32 ? 4 : 3) : 8);
+    }
+    s.n_tiles = (int)((c.n_freq + s.tile - 1) / s.tile);
+    // Split the observations of every object when (object, tile) items alone cannot fill the GPU for a few
+    // waves (large-N_t / small-N_f problems; PAPER.md:L373, L396 describe the under-filled GPU).  Among the
+    // admissible split counts pick the one whose last wave is fullest (wave quantisation), then the smallest.
+    const int64_t items = std::max<int64_t>(1, n_obj * s.n_tiles);
+    int64_t split = 1;
+    if (items < 8 * slots && n_obj > 0) {
+        const int64_t avg_nt = total_obs / std::max<int64_t>(1, n_obj);
+        const int64_t min_obs = (k == LSP_KERNEL_FACTORED) ? 128 : 64;      // per split, to amortise prologue/epilogue
+        const int64_t s_max = std::max<int64_t>(1, std::min<int64_t>(64, avg_nt / min_obs));
+        double best_score = -1.0;
+        for (int64_t cand = 1; cand <= s_max; ++cand) {
+            const double waves = (double)(items * cand) / (double)slots;
+            const double eff = waves / std::ceil(waves);               // occupancy of the average wave
+            const double score = eff - 0.004 * (double)(cand - 1);     // each split adds a partial-sum pass
+            if (score > best_score + 1e-9) { best_score = score; split = cand; }
+            if (waves >= 8.0) break;
+        }
+    }
+    s.n_split = (int)split;
+    return s;
+}
+
+template <typename T, bool FAST>
+cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, int64_t n_obj_launch, const int64_t* d_off,
+                        const void* d_t, const void* d_y, const ObjStats* stats, void* out, Best* partials,
+                        void* sums, cudaStream_t st)
+{
+    using V4 = typename Vec4<T>::type;
+    const int64_t grid = n_obj_launch * s.n_tiles * s.n_split;
+    if (grid <= 0) return cudaSuccess;
+    if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws) {
+        auto kern = lsp_factored_ws_kernel<T, FAST>;
+        static bool attr_done = false;     // per instantiation
+        if (!attr_done) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ws_smem_bytes<T>());
+            if (e != cudaSuccess) return e;
+            attr_done = true;
+        }
+        cudaError_t e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
+        if (e != cudaSuccess) return e;
+        const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
+        kern<<<ctas, kWsThreads, ws_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
+                                                          (V4*)sums, n_obj_launch, (long long)grid,
+                                                          (unsigned long long*)p->counter.ptr);
+    } else if (s.kernel == LSP_KERNEL_FACTORED) {
+        auto kern = lsp_factored_kernel<T, FAST>;
+        static bool attr_done = false;     // per instantiation
+        if (!attr_done) {
+            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fac_smem_bytes<T>());
+            if (e != cudaSuccess) return e;
+            attr_done = true;
+        }
+        kern<<<(unsigned)grid, kFacThreads, fac_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats,
+                                                                     (T*)out, partials, (V4*)sums, n_obj_launch);
+    } else if (s.direct_r == 4) {
+        lsp_direct_kernel<T, FAST, 4><<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y,
+                                                                                 stats, (T*)out, partials, (V4*)sums, n_obj_launch);
+    } else {
+        lsp_direct_kernel<T, FAST, 1><<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y,
+                                                                                 stats, (T*)out, partials, (V4*)sums, n_obj_launch);
+    }
+    return cudaGetLastError();
+}
+
+// Launches steps 2-6' for objects [obj_base, obj_base + n_obj_launch) on `st`.
+// `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed globally.
+lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n_obj_launch, const int64_t* d_off,
+                     const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out, cudaStream_t st)
+{
+    const lsp_config& c = p->cfg;
+    GridParams gp;
+    gp.f_min = c.f_min;
+    gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gp.n_freq = (int)c.n_freq;
+    gp.n_tiles = s.n_tiles;
+    gp.n_split = s.n_split;
+    gp.obj_base = (int)obj_base;
+    const ObjStats* stats = (c.center || c.normalize) ? (const ObjStats*)p->stats.ptr : nullptr;
+    void* sums = nullptr;
+    const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
+    if (s.n_split > 1) {
+        const size_t need = (size_t)s.n_split * n_obj_launch * c.n_freq * 4 * elem_size(c);
+        lsp_status e = ensure(p, p->sums, need);
+        if (e != LSP_OK) return e;
+        sums = p->sums.ptr;
+    }
+    *n_parts_out = (s.n_split > 1) ? n_cparts : s.n_tiles;
+    if (want_best) {     // partials are indexed by the launch-local object: each launch's finalize follows it in-stream
+        lsp_status e = ensure(p, p->partials, (size_t)n_obj_launch * (size_t)*n_parts_out * sizeof(Best));
+        if (e != LSP_OK) return e;
+    }
+
+    Best* partials = want_best ? (Best*)p->partials.ptr : nullptr;
+
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    if (p->timing) {
+        if (p->t_used == p->t_start.size()) {
+            cudaEvent_t a, b;
+            LSP_CUDA(p, cudaEventCreate(&a));
+            LSP_CUDA(p, cudaEventCreate(&b));
+            p->t_start.push_back(a);
+            p->t_stop.push_back(b);
+        }
+        ev0 = p->t_start[p->t_used];
+        ev1 = p->t_stop[p->t_used];
+        ++p->t_used;
+        LSP_CUDA(p, cudaEventRecord(ev0, st));
+    }
+    cudaError_t e;
+    void* main_out = (s.n_split > 1) ? nullptr : out;
+    Best* main_partials = (s.n_split > 1) ? nullptr : partials;
+    if (c.dtype == LSP_F32) {
+        e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st)
+                        : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st);
+    } else {
+        e = launch_main<double, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st);
+    }
+    if (e != cudaSuccess) return fail(p, LSP_ERR_CUDA, "periodogram kernel launch: %s", cudaGetErrorString(e));
+    ++p->n_launches;
+    if (ev1) LSP_CUDA(p, cudaEventRecord(ev1, st));
+
+    if (s.n_split > 1) {
+        const int64_t grid = n_obj_launch * n_cparts;
+        if (c.dtype == LSP_F32)
+            lsp_combine_kernel<float><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, d_off, stats, (const float4*)sums, (float*)out,
+                                                                                  partials, n_cparts, n_obj_launch);
+        else
+            lsp_combine_kernel<double><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, d_off, stats, (const double4*)sums, (double*)out,
+                                                                                   partials, n_cparts, n_obj_launch);
+        LSP_CUDA(p, cudaGetLastError());
+        ++p->n_launches;
+    }
+    return LSP_OK;
+}
+
+lsp_status run_finalize(lsp_plan* p, int64_t obj_base, int64_t n_obj_launch, int n_parts, const int64_t* d_off,
+                        void* d_best_period, void* d_best_power, int64_t* d_best_index, cudaStream_t st)
+{
+    const lsp_config& c = p->cfg;
+    GridParams gp;
+    gp.f_min = c.f_min;
+    gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gp.n_freq = (int)c.n_freq;
+    gp.n_tiles = n_parts;
+    gp.n_split = 1;
+    gp.obj_base = (int)obj_base;
+    const int wpb = 4;
+    const unsigned grid = (unsigned)((n_obj_launch + wpb - 1) / wpb);
+    if (c.dtype == LSP_F32)
+        lsp_finalize_best_kernel<float><<<grid, wpb * 32, 0, st>>>(gp, d_off, (const Best*)p->partials.ptr, n_parts, n_obj_launch,
+                                                                   (float*)d_best_period, (float*)d_best_power, d_best_index);
+    else
+        lsp_finalize_best_kernel<double><<<grid, wpb * 32, 0, st>>>(gp, d_off, (const Best*)p->partials.ptr, n_parts, n_obj_launch,
+                                                                    (double*)d_best_period, (double*)d_best_power, d_best_index);
+    LSP_CUDA(p, cudaGetLastError());
+    ++p->n_launches;
+    return LSP_OK;
+}
+
+lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int64_t* h_off, const void* d_t,
+                    const void* d_y, void* out_power, int out_is_host, void* d_best_period, void* d_best_power,
+                    int64_t* d_best_index, void* cuda_stream)
+{
+    if (!p) return LSP_ERR_INVALID_ARG;
+    const lsp_config& c = p->cfg;
+    p->n_launches = p->n_pairs = p->n_chunks = 0;
+    p->t_used = 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
+    const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
+    if (n_best != 0 && n_best != 3) return fail(p, LSP_ERR_INVALID_ARG, "best_period/best_power/best_index: give all three or none");
+    const bool want_best = n_best == 3;
+    if (!out_power && !want_best) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
+    if (n_obj == 0) return LSP_OK;
+    if (!d_off) return fail(p, LSP_ERR_INVALID_ARG, "d_offsets is NULL");
+    if (n_obj > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "n_obj too large");
+    LSP_CUDA(p, cudaSetDevice(c.device));
+
+    int64_t total_obs;
+    if (h_off) {
+        if (h_off[0] != 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[0] != 0");
+        for (int64_t o = 0; o < n_obj; ++o)
+            if (h_off[o + 1] < h_off[o]) return fail(p, LSP_ERR_INVALID_ARG, "offsets decrease at object %lld", (long long)o);
+        total_obs = h_off[n_obj];
+    } else {
+        if (!p->h_offsets_pinned) LSP_CUDA(p, cudaMallocHost((void**)&p->h_offsets_pinned, sizeof(int64_t)));
+        LSP_CUDA(p, cudaMemcpyAsync(p->h_offsets_pinned, d_off + n_obj, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaStreamSynchronize(st));
+        total_obs = p->h_offsets_pinned[0];
+        if (total_obs < 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[n_obj] < 0");
+    }
+    if (total_obs > 0 && (!d_t || !d_y)) return fail(p, LSP_ERR_INVALID_ARG, "d_t / d_y is NULL");
+
+    const Schedule s = make_schedule(p, n_obj, total_obs);
+    p->kernel_used = s.kernel;
+    p->n_split = s.n_split;
+    p->n_pairs = total_obs * c.n_freq;
+
+    if (c.center || c.normalize) {
+        lsp_status e = ensure(p, p->stats, (size_t)n_obj * sizeof(ObjStats));
+        if (e != LSP_OK) return e;
+        if (c.dtype == LSP_F32)
+            lsp_object_stats_kernel<float><<<(unsigned)n_obj, 128, 0, st>>>(d_off, (const float*)d_y, (ObjStats*)p->stats.ptr, c.center, c.normalize);
+        else
+            lsp_object_stats_kernel<double><<<(unsigned)n_obj, 128, 0, st>>>(d_off, (const double*)d_y, (ObjStats*)p->stats.ptr, c.center, c.normalize);
+        LSP_CUDA(p, cudaGetLastError());
+        ++p->n_launches;
+    }
+
+    int n_parts = 0;
+    if (!out_power || !out_is_host) {
+        // steps 2-6': one launch over the whole batch, asynchronous on the caller's stream
+        lsp_status e = run_range(p, s, 0, n_obj, d_off, d_t, d_y, out_power, want_best, &n_parts, st);
+        if (e != LSP_OK) return e;
+        if (want_best) return run_finalize(p, 0, n_obj, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
+        return LSP_OK;
+    }
+
+    // ---- step 7: chunked compute -> event -> copy streams -> (pinned) host -------------------
+    const size_t es = elem_size(c);
+    const size_t row_bytes = (size_t)c.n_freq * es;
+    const size_t chunk_bytes = c.chunk_bytes > 0 ? (size_t)c.chunk_bytes : ((size_t)64 << 20);
+    const int64_t objs_per_chunk = std::max<int64_t>(1, (int64_t)(chunk_bytes / row_bytes));
+    const size_t slot_bytes = (size_t)objs_per_chunk * row_bytes;
+    const int n_slots = (int)p->slot_ready.size();
+    {
+        lsp_status e = ensure(p, p->ring, slot_bytes * n_slots);
+        if (e != LSP_OK) return e;
+    }
+    std::fill(p->slot_used.begin(), p->slot_used.end(), 0);
+    // a chunk's schedule is made for the chunk's own object count, so small chunks still split observations
+    int64_t chunk = 0;
+    for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_chunk, ++chunk) {
+        const int64_t no = std::min(objs_per_chunk, n_obj - o0);
+        const int slot = (int)(chunk % n_slots);
+        char* dslot = (char*)p->ring.ptr + (size_t)slot * slot_bytes;
+        if (p->slot_used[slot]) LSP_CUDA(p, cudaStreamWaitEvent(st, p->slot_free[slot], 0));
+        const int64_t obs_est = total_obs / n_obj * no;
+        Schedule sc = make_schedule(p, no, obs_est);
+        sc.kernel = s.kernel;
+        lsp_status e = run_range(p, sc, o0, no, d_off, d_t, d_y, dslot, want_best, &n_parts, st);
+        if (e != LSP_OK) return e;
+        if (want_best) {
+            e = run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
+            if (e != LSP_OK) return e;
+        }
+        LSP_CUDA(p, cudaEventRecord(p->slot_ready[slot], st));
+        cudaStream_t cs = p->copy_streams[chunk % p->copy_streams.size()];
+        LSP_CUDA(p, cudaStreamWaitEvent(cs, p->slot_ready[slot], 0));
+        LSP_CUDA(p, cudaMemcpyAsync((char*)out_power + (size_t)o0 * row_bytes, dslot, (size_t)no * row_bytes,
+                                    cudaMemcpyDeviceToHost, cs));
+        LSP_CUDA(p, cudaEventRecord(p->slot_free[slot], cs));
+        p->slot_used[slot] = 1;
+    }
+    p->n_chunks = chunk;
+    for (cudaStream_t cs : p->copy_streams) LSP_CUDA(p, cudaStreamSynchronize(cs));
+    return LSP_OK;
+}
+
+}  // namespace
+
+// =============================================================================================================
+extern "C" {
+
+lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
+{
+    if (out_plan) *out_plan = nullptr;
+    if (!cfg || !out_plan) return fail(nullptr, LSP_ERR_INVALID_ARG, "cfg / out_plan is NULL");
+    if (!(cfg->f_min > 0.0) || !(cfg->f_max > cfg->f_min) || !std::isfinite(cfg->f_max))
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "need 0 < f_min < f_max (got %g, %g)", cfg->f_min, cfg->f_max);
+    if (cfg->n_freq < 1 || cfg->n_freq > 0x7fffffffLL) return fail(nullptr, LSP_ERR_INVALID_ARG, "n_freq out of range");
+    if (cfg->dtype != LSP_F32 && cfg->dtype != LSP_F64) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown dtype");
+    if (cfg->fast_math != 0 && cfg->fast_math != 1) return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math must be 0 or 1");
+    if (cfg->fast_math && cfg->dtype == LSP_F64)
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math (MUFU sincos) is FP32-only");
+    if (cfg->kernel < LSP_KERNEL_AUTO || cfg->kernel > LSP_KERNEL_FACTORED) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown kernel");
+    if (cfg->reserved != 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "reserved must be 0");
+    if (cfg->n_copy_streams < 0 || cfg->n_copy_streams > 16 || cfg->chunk_bytes < 0 || cfg->max_objects < 0 || cfg->max_total_obs < 0)
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "negative / oversized sizing field");
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0) {
+        cudaGetLastError();
+        return fail(nullptr, LSP_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    if (cfg->device < 0 || cfg->device >= n_dev) return fail(nullptr, LSP_ERR_INVALID_ARG, "device ordinal out of range");
+    lsp_plan* p = new (std::nothrow) lsp_plan;
+    if (!p) return fail(nullptr, LSP_ERR_OOM, "host allocation failed");
+    p->cfg = *cfg;
+    if (p->cfg.n_copy_streams == 0) p->cfg.n_copy_streams = 3;
+    auto bail = [&](lsp_status st) {
+        g_create_error = p->error;
+        lsp_destroy(p);
+        return st;
+    };
+#define LSP_CREATE_CUDA(call)                                                                   \
+    do {                                                                                        \
+        cudaError_t e_ = (call);                                                                \
+        if (e_ != cudaSuccess) {                                                                \
+            p->error = std::string(#call) + ": " + cudaGetErrorString(e_);                      \
+            return bail(e_ == cudaErrorMemoryAllocation ? LSP_ERR_OOM : LSP_ERR_CUDA);          \
+        }                                                                                       \
+    } while (0)
+    LSP_CREATE_CUDA(cudaSetDevice(cfg->device));
+    cudaDeviceProp prop;
+    LSP_CREATE_CUDA(cudaGetDeviceProperties(&prop, cfg->device));
+    if (prop.major < 10) {
+        p->error = "device is not sm_100 class (this library is built for sm_100a only)";
+        return bail(LSP_ERR_UNSUPPORTED);
+    }
+    p->sm_count = prop.multiProcessorCount;
+    const int n_slots = p->cfg.n_copy_streams + 1;
+    for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
+        cudaStream_t s;
+        LSP_CREATE_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+        p->copy_streams.push_back(s);
+    }
+    for (int i = 0; i < n_slots; ++i) {
+        cudaEvent_t a, b;
+        LSP_CREATE_CUDA(cudaEventCreateWithFlags(&a, cudaEventDisableTiming));
+        p->slot_ready.push_back(a);
+        LSP_CREATE_CUDA(cudaEventCreateWithFlags(&b, cudaEventDisableTiming));
+        p->slot_free.push_back(b);
+    }
+    p->slot_used.assign(n_slots, 0);
+    if (ensure(p, p->counter, 64) != LSP_OK) return bail(LSP_ERR_OOM);
+    if (const char* impl = getenv("LSP_FACTORED_IMPL")) p->use_ws = strcmp(impl, "classic") != 0;
+    if (cfg->max_objects > 0) {
+        const int tile = cfg->dtype == LSP_F32 ? fac_tile<float>() : fac_tile<double>();
+        const size_t parts = (size_t)std::max<int64_t>((cfg->n_freq + tile - 1) / tile,
+                                                       (cfg->n_freq + kDirectThreads - 1) / kDirectThreads);
+        if (ensure(p, p->partials, (size_t)cfg->max_objects * parts * sizeof(Best)) != LSP_OK) return bail(LSP_ERR_OOM);
+        if (ensure(p, p->stats, (size_t)cfg->max_objects * sizeof(ObjStats)) != LSP_OK) return bail(LSP_ERR_OOM);
+    }
+#undef LSP_CREATE_CUDA
+    *out_plan = p;
+    return LSP_OK;
+}
+
+lsp_status lsp_periodogram_batched(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
+                                   const void* d_t, const void* d_y, void* out_power, int32_t out_is_host,
+                                   void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
+{
+    if (!plan) return LSP_ERR_INVALID_ARG;
+    if (!out_power) return fail(plan, LSP_ERR_INVALID_ARG, "out_power is NULL (use lsp_best_period for best-only output)");
+    return run_call(plan, n_obj, d_offsets, h_offsets, d_t, d_y, out_power, out_is_host, d_best_period, d_best_power,
+                    d_best_index, cuda_stream);
+}
+
+lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
+                           const void* d_t, const void* d_y, void* d_best_period, void* d_best_power,
+                           int64_t* d_best_index, void* cuda_stream)
+{
+    if (!plan) return LSP_ERR_INVALID_ARG;
+    if (!d_best_period || !d_best_power || !d_best_index)
+        return fail(plan, LSP_ERR_INVALID_ARG, "best_period, best_power and best_index are all required");
+    return run_call(plan, n_obj, d_offsets, h_offsets, d_t, d_y, nullptr, 0, d_best_period, d_best_power, d_best_index,
+                    cuda_stream);
+}
+
+void lsp_destroy(lsp_plan* p)
+{
+    if (!p) return;
+    cudaSetDevice(p->cfg.device);
+    for (cudaStream_t s : p->copy_streams) {
+        cudaStreamSynchronize(s);
+        cudaStreamDestroy(s);
+    }
+    for (cudaEvent_t e : p->slot_ready) cudaEventDestroy(e);
+    for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
+    for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
+    for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter})
+        if (b->ptr) cudaFree(b->ptr);
+    if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
+    cudaGetLastError();
+    delete p;
+}
+
+const char* lsp_last_error(const lsp_plan* plan)
+{
+    return plan ? plan->error.c_str() : g_create_error.c_str();
+}
+
+void lsp_last_call_info(const lsp_plan* p, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used, int32_t* n_split,
+                        int64_t* n_chunks)
+{
+    if (!p) return;
+    if (n_launches) *n_launches = p->n_launches;
+    if (n_pairs) *n_pairs = p->n_pairs;
+    if (kernel_used) *kernel_used = p->kernel_used;
+    if (n_split) *n_split = p->n_split;
+    if (n_chunks) *n_chunks = p->n_chunks;
+}
+
+void lsp_set_timing(lsp_plan* p, int32_t on)
+{
+    if (p) p->timing = on != 0;
+}
+
+float lsp_last_kernel_ms(lsp_plan* p)
+{
+    if (!p || !p->timing || p->t_used == 0) return -1.f;
+    float total = 0.f;
+    for (size_t i = 0; i < p->t_used; ++i) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(p->t_stop[i]) != cudaSuccess) return -1.f;
+        if (cudaEventElapsedTime(&ms, p->t_start[i], p->t_stop[i]) != cudaSuccess) return -1.f;
+        total += ms;
+    }
+    return total;
+}
+
+lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, double* elapsed_ms)
+{
+    if (!ops_per_s || which < 0 || which > 4) return fail(nullptr, LSP_ERR_INVALID_ARG, "lsp_pipe_peak: bad argument");
+    lsp_plan* p = nullptr;
+    LSP_CUDA(p, cudaSetDevice(device));
+    cudaDeviceProp prop;
+    LSP_CUDA(p, cudaGetDeviceProperties(&prop, device));
+    void* out = nullptr;
+    LSP_CUDA(p, cudaMalloc(&out, 64));
+    cudaEvent_t e0, e1;
+    LSP_CUDA(p, cudaEventCreate(&e0));
+    LSP_CUDA(p, cudaEventCreate(&e1));
+    const int ctas_per_sm = (which == 4) ? 2 : 4;
+    const unsigned grid = (unsigned)(prop.multiProcessorCount * ctas_per_sm * 4);    // 4 full waves
+    double ops_per_thread = 0.0;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {                      // rep 0 is the warm-up
+        LSP_CUDA(p, cudaEventRecord(e0, 0));
+        switch (which) {
+            case 0: peak_ffma_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
+                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
+            case 1: peak_ffma2_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
+                    ops_per_thread = 2.0 * kPeakIters * kPeakIlp; break;
+            case 2: peak_dfma_kernel<<<grid, kPeakThreads>>>((double*)out, 1.0000001, 1e-9);
+                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
+            case 3: peak_mufu_kernel<<<grid, kPeakThreads>>>((float*)out, 0.001f);
+                    ops_per_thread = 2.0 * (kPeakIters / 4) * kPeakIlp; break;
+            default: peak_mix_kernel<<<grid, kPeakThreads>>>((float*)out, 0.5f);
+                    ops_per_thread = 2.0 * 32.0 * 16.0 * (kPeakIters / 16); break;
+        }
+        LSP_CUDA(p, cudaGetLastError());
+        LSP_CUDA(p, cudaEventRecord(e1, 0));
+        LSP_CUDA(p, cudaEventSynchronize(e1));
+        float ms = 0.f;
+        LSP_CUDA(p, cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0) best_ms = std::min(best_ms, ms);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    *ops_per_s = ops_per_thread * (double)grid * kPeakThreads / (best_ms * 1e-3);
+    if (elapsed_ms) *elapsed_ms = best_ms;
+    return LSP_OK;
+}
+
+const char* lsp_version(void)
+{
+    return "lsp-b200 0.1 (sm_100a; kernels: direct, factored-ffma2, factored-dfma)";
+}
+
+}  // extern "C"

@@ -1,0 +1,149 @@
+// lsp_common.cuh -- shared device helpers of the CUDA path: phase reduction, the per-(object, frequency)
+// epilogue (hot-path step 5), and the (power, index) argmax reduction (step 6').
+// Nothing here is shared with oracle/ (the CPU oracle is a separate C file with its own arithmetic).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+
+namespace lsp {
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+// Per-call constants every kernel needs; passed by value (fits the 4 KB parameter space easily).
+struct GridParams {
+    double f_min;       // cycles per unit of t
+    double df;          // (f_max - f_min) / n_freq
+    int    n_freq;      // N_f
+    int    n_tiles;     // frequency tiles per object
+    int    n_split;     // observation splits per (object, tile); 1 = epilogue fused in the main kernel
+    int    obj_base;    // first object of this launch (host-output chunks)
+};
+
+// Per-object pre-pass results (step 1): mean to subtract (0 unless center=1) and the output scale
+// (1, or 1/(0.5*sum y^2) when normalize=1).
+struct ObjStats {
+    double mean;
+    double scale;
+};
+
+// A (power, index) candidate of the fused argmax.  Lowest index wins exact ties; NaN never wins
+// (reading a7): NaN powers are mapped to -1 before they get here (P >= 0 otherwise).
+struct Best {
+    double  p;
+    int64_t k;
+};
+
+__device__ __forceinline__ Best best_of(Best a, Best b)
+{
+    return (b.p > a.p || (b.p == a.p && b.k < a.k)) ? b : a;
+}
+
+__device__ __forceinline__ Best warp_best(Best v)
+{
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) {
+        Best o;
+        o.p = __shfl_xor_sync(0xffffffffu, v.p, s);
+        o.k = __shfl_xor_sync(0xffffffffu, v.k, s);
+        v = best_of(v, o);
+    }
+    return v;
+}
+
+// CTA-wide argmax; result valid in thread 0.  `scratch` holds >= blockDim.x/32 entries.
+__device__ __forceinline__ Best block_best(Best v, Best* scratch)
+{
+    v = warp_best(v);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0) scratch[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        Best w;
+        w.p = -2.0;
+        w.k = INT64_MAX;
+        if (lane < nw) w = scratch[lane];
+        v = warp_best(w);
+    }
+    return v;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Step 5: power from the four un-rotated sums of one (object, frequency):
+//   xc = sum y cos(wt), xs = sum y sin(wt), c2 = sum cos(2wt), s2 = sum sin(2wt), n = N_t.
+// Eq. 1's tau diagonalises M = [[CC, CS], [CS, SS]] with CC = (n + c2)/2, SS = (n - c2)/2, CS = s2/2, and
+// Eq. 2 is 1/2 b^T M^-1 b with b = (xc, xs) (the paper's own single-scan epilogue,
+// Listing 1, evaluates the same quantity through atan2 + a second sincos).  Written out:
+//   P = [ n (xc^2 + xs^2) - c2 (xc^2 - xs^2) - 2 s2 xc xs ] / (n^2 - c2^2 - s2^2)
+// One division, no atan2/sincos.  When the smaller eigenvalue (n - |w|)/2 of M vanishes (all 2wt_j equal
+// mod 2pi: N_t = 1, exact aliasing) its term is dropped, as the oracle does (reading a6):
+//   P -> (xc^2 + xs^2) / (n + |w|).
+// Every product and sum below is an explicit round-to-nearest intrinsic, so the compiler cannot contract them
+// differently in different kernels or code paths: the same sums give the same bits everywhere.
+__device__ __forceinline__ float  mul_rn(float a, float b)   { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float  add_rn(float a, float b)   { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float  div_rn(float a, float b)   { return __fdividef(a, b); }   // MUFU.RCP + FMUL, <= 2 ulp: the
+                                                                                          // FP32 tolerance is 1e-3 max P
+__device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
+
+template <typename T>
+__device__ __forceinline__ T power_from_sums(T xc, T xs, T c2, T s2, T n, T scale)
+{
+    const T eps = sizeof(T) == 4 ? T(2e-6) : T(4e-12);
+    const T a = mul_rn(xc, xc), b = mul_rn(xs, xs);
+    const T w2 = fma(c2, c2, mul_rn(s2, s2));
+    const T nn = mul_rn(n, n);
+    const T den = add_rn(nn, -w2);
+    T p;
+    if (den > mul_rn(eps, nn)) {
+        // n (a + b) - c2 (a - b) - 2 s2 xc xs
+        const T num = fma(-mul_rn(T(2), s2), mul_rn(xc, xs), fma(-c2, add_rn(a, -b), mul_rn(n, add_rn(a, b))));
+        p = div_rn(num, den);
+    } else if (n > T(0)) {
+        p = div_rn(add_rn(a, b), add_rn(n, sqrt(w2)));
+    } else {
+        p = T(0);
+    }
+    return mul_rn(p, scale);
+}
+
+// frac(x) to (-1/2, 1/2] by the round-to-nearest magic constant (x >= 0 and < 2^51 here): two DADDs on the
+// FP64 pipe instead of FRND.F64.
+__device__ __forceinline__ double frac_cycles(double p)
+{
+    const double magic = 6755399441055744.0;   // 1.5 * 2^52
+    const double r = (p + magic) - magic;
+    return p - r;
+}
+
+// Exact-product phase: f*t = p + e exactly (fma), reduced to cycles in (-1/2, 1/2].
+__device__ __forceinline__ double phase_cycles_exact(double f, double t)
+{
+    const double p = f * t;
+    const double e = fma(f, t, -p);
+    return frac_cycles(p) + e;
+}
+
+// sin/cos of 2*pi*r for r in about [-1, 1] cycles.
+//   FAST (FP32): MUFU.SIN / MUFU.COS through __sinf/__cosf (the paper's "__sincosf").
+//   accurate FP32: CUDA's sincospif (polynomial on the FMA pipe, <= 2 ulp).
+template <bool FAST>
+__device__ __forceinline__ void sincos_cycles(float r, float* s, float* c)
+{
+    if (FAST) {
+        const float a = r * 6.283185307179586f;
+        *s = __sinf(a);
+        *c = __cosf(a);
+    } else {
+        sincospif(2.0f * r, s, c);
+    }
+}
+template <bool FAST>
+__device__ __forceinline__ void sincos_cycles(double r, double* s, double* c)
+{
+    sincospi(2.0 * r, s, c);   // FAST has no FP64 meaning (rejected at plan creation)
+}
+
+}  // namespace lsp

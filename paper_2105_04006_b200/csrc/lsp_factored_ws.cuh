@@ -1,0 +1,375 @@
+// lsp_factored_ws.cuh -- persistent, warp-specialised version of the factored kernel (see lsp_factored.cuh for
+// the mathematics: angle addition + conjugate symmetry, 4 FMA per (t, f) pair, no sincos in the O(N_t N_f) loop).
+//
+// One CTA per SM, 12 warps:
+//   warps 0-3   consumers, contract Z(k) = sum y e^{i theta}        } 32 FFMA2 + 4 LDS.128 (FP32) or
+//   warps 4-7   consumers, contract W(k) = sum e^{2 i theta}        } 32 DFMA  + 6 LDS.128 (FP64) per observation
+//   warps 8-11  producers: stage (t_j, y_j), form the range-reduced phases in FP64, evaluate sincos (MUFU or
+//               accurate) and write the operands a = y e^{i alpha}, a2, b = e^{i beta}, b2 of one observation
+//               chunk into a shared-memory ring (hot-path steps 2-3)
+// Producers and consumers meet only through mbarriers (full[s] / empty[s] per ring stage), so the FMA pipe is
+// fed by warps that never wait on a sincos dependency chain or a CTA-wide barrier, while the XU / FP64 pipes
+// work for the producers.  The CTA is persistent: it pulls (object, frequency tile, observation split) work
+// items from a global counter (step 1: dynamic scheduling absorbs the 10x spread of N_t across objects), and the
+// producers run ahead into the next item while the consumers finish the epilogue of the previous one.
+//
+// Epilogue (step 5, 6, 6'): Z and W warps exchange half of their sums through shared memory so that all eight
+// consumer warps evaluate powers; powers are staged and stored coalesced; the per-CTA argmax partial is fused.
+#pragma once
+#include "lsp_factored.cuh"
+
+namespace lsp {
+
+constexpr int kWsConsumers = 256;
+constexpr int kWsProducers = 128;
+constexpr int kWsThreads = kWsConsumers + kWsProducers;
+
+template <typename T> struct WsCfg;
+template <> struct WsCfg<float> {
+    static constexpr int JC = 8;         // observations per ring stage
+    static constexpr int STAGES = 6;
+    static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<float>::NL);   // complex elements per stage
+};
+template <> struct WsCfg<double> {
+    static constexpr int JC = 4;
+    static constexpr int STAGES = 6;
+    static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<double>::NL);
+};
+
+struct WsMeta {          // one per ring stage, written by producer thread 0
+    long long item;      // work item id, -1 = no more work
+    int last;            // 1 = last chunk of the item: consumers run the epilogue after it
+    int pad;
+};
+
+template <typename T> constexpr size_t ws_smem_bytes()
+{
+    return (size_t)WsCfg<T>::STAGES * WsCfg<T>::STAGE_ELEMS * 2 * sizeof(T)      // operand ring
+           + (size_t)FactoredCfg<T>::TILE * 3 * sizeof(T)              // epilogue exchange + staged powers
+           + WsCfg<T>::STAGES * (2 * sizeof(unsigned long long) + sizeof(WsMeta)) + 64;
+}
+
+// ---- mbarrier helpers (CTA scope) ---------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    unsigned done;
+    do {       // try_wait suspends the thread in hardware for a bounded time; loop until the phase completes
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void named_bar_sync(int id, int n_threads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
+}
+
+struct WsItem {
+    int64_t obj_local, obj, lo, n_t, j0, j1, K0;
+    int tile, split;
+};
+template <int TILE>
+__device__ __forceinline__ WsItem ws_decode(const GridParams& gp, long long item, const int64_t* __restrict__ offsets)
+{
+    WsItem w;
+    w.split = (int)(item % gp.n_split);
+    const long long r = item / gp.n_split;
+    w.tile = (int)(r % gp.n_tiles);
+    w.obj_local = r / gp.n_tiles;
+    w.obj = w.obj_local + gp.obj_base;
+    w.lo = offsets[w.obj];
+    w.n_t = offsets[w.obj + 1] - w.lo;
+    w.j0 = (w.n_t * w.split) / gp.n_split;
+    w.j1 = (w.n_t * (w.split + 1)) / gp.n_split;
+    w.K0 = (int64_t)w.tile * TILE;
+    return w;
+}
+
+template <typename T, bool FAST>
+__global__ void __launch_bounds__(kWsThreads, 1)
+lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
+                       const T* __restrict__ y, const ObjStats* __restrict__ stats,
+                       T* __restrict__ out_power, Best* __restrict__ partials,
+                       typename Vec4<T>::type* __restrict__ sums, int64_t n_obj_launch,
+                       long long total_items, unsigned long long* __restrict__ work_counter)
+{
+    using C = FactoredCfg<T>;
+    using V2 = typename C::V2;
+    constexpr int G = kFacGroups, TH = C::TH, TM = C::TM, NL = C::NL, L = 2 * NL, TILE = C::TILE, EPC = C::EPC;
+    constexpr int JC = WsCfg<T>::JC, S = WsCfg<T>::STAGES;
+    constexpr int NGI = G / TH, NMI = NL / TM;
+    constexpr int STAGE = WsCfg<T>::STAGE_ELEMS;             // V2 elements per stage: [JC][G] a, [JC][G] a2, [JC][NL] b, [JC][NL] b2
+    static_assert(NGI * NMI == kWsConsumers / 2, "Z and W halves each cover the G x NL tile once");
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    V2* ring = reinterpret_cast<V2*>(smem_raw);
+    V2* sX = ring + (size_t)S * STAGE;                         // [TILE] exchanged sums
+    T* sP = reinterpret_cast<T*>(sX + TILE);                   // [TILE] staged powers
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(sP + TILE);
+    unsigned long long* empty = full + S;
+    WsMeta* meta = reinterpret_cast<WsMeta*>(empty + S);
+    __shared__ Best sbest[kWsConsumers / 32];
+    __shared__ long long s_next_item;
+
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        for (int s = 0; s < S; ++s) {
+            mbar_init(&full[s], kWsProducers);
+            mbar_init(&empty[s], kWsConsumers / 32);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (tid >= kWsConsumers) {
+        // =========================================== producers ===============================================
+        const int ptid = tid - kWsConsumers;
+        const int gen_g = ptid & (G - 1);
+        const int gen_m = ptid & (NL - 1);
+        const int gen_pos_a = operand_pos<TH, NGI, EPC>(gen_g);
+        const int gen_pos_b = operand_pos<TM, NMI, EPC>(gen_m);
+        const double f_beta = ((double)gen_m + 0.5) * gp.df;                       // (m + 1/2) df
+        constexpr int NA = (G * JC) / kWsProducers;                                // a-elements per thread per chunk
+        constexpr int NB = (NL * JC + kWsProducers - 1) / kWsProducers;            // b-elements per thread per chunk
+        long long item = blockIdx.x;      // first item is static; the rest come from the global counter
+        unsigned c = 0;
+        while (true) {
+            if (item >= total_items) {
+                const int s = c % S;
+                mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
+                if (ptid == 0) { meta[s].item = -1; meta[s].last = 1; }
+                mbar_arrive(&full[s]);
+                break;
+            }
+            const WsItem w = ws_decode<TILE>(gp, item, offsets);
+            const T mean = stats ? (T)stats[w.obj].mean : T(0);
+            const double f_centre = gp.f_min + ((double)(w.K0 + (int64_t)gen_g * L + NL) - 0.5) * gp.df;   // f(c_g)
+            if (ptid == 0) s_next_item = (long long)gridDim.x + (long long)atomicAdd(work_counter, 1ULL);
+            int64_t jb = w.j0;
+            do {      // at least one chunk per item, so empty objects still reach the epilogue
+                // loads first, so their latency overlaps the wait for a free stage
+                T ta[NA], ya[NA], tb[NB];
+#pragma unroll
+                for (int it = 0; it < NA; ++it) {
+                    const int64_t j = jb + (ptid + it * kWsProducers) / G;
+                    ta[it] = (j < w.j1) ? t[w.lo + j] : T(0);
+                    ya[it] = (j < w.j1) ? y[w.lo + j] - mean : T(0);
+                }
+#pragma unroll
+                for (int it = 0; it < NB; ++it) {
+                    const int64_t j = jb + (ptid + it * kWsProducers) / NL;
+                    tb[it] = (j < w.j1) ? t[w.lo + j] : T(0);
+                }
+                const int s = c % S;
+                mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
+                V2* sA1 = ring + (size_t)s * STAGE;
+                V2* sA2 = sA1 + JC * G;
+                V2* sB1 = sA2 + JC * G;
+                V2* sB2 = sB1 + JC * NL;
+#pragma unroll
+                for (int it = 0; it < NA; ++it) {
+                    const int jj = (ptid + it * kWsProducers) / G;
+                    T sn, cs;
+                    sincos_cycles<FAST>(phase_for<T>(f_centre, ta[it]), &sn, &cs);
+                    V2 a1, a2;
+                    a1.x = ya[it] * cs;              // a  = y e^{i alpha}   (y = 0 beyond the item's range)
+                    a1.y = ya[it] * sn;
+                    const bool live = (jb + jj) < w.j1;
+                    a2.x = live ? fma(cs, cs, -sn * sn) : T(0);      // a2 = e^{2 i alpha}
+                    a2.y = live ? T(2) * cs * sn : T(0);
+                    sA1[jj * G + gen_pos_a] = a1;
+                    sA2[jj * G + gen_pos_a] = a2;
+                }
+#pragma unroll
+                for (int it = 0; it < NB; ++it) {
+                    const int e = ptid + it * kWsProducers;
+                    if ((NL * JC) % kWsProducers != 0 && e >= NL * JC) break;
+                    const int jj = e / NL;
+                    T sn, cs;
+                    sincos_cycles<FAST>(phase_for<T>(f_beta, tb[it]), &sn, &cs);
+                    V2 b1, b2;
+                    b1.x = cs;                        // b  = e^{i beta}
+                    b1.y = sn;
+                    b2.x = fma(cs, cs, -sn * sn);     // b2 = e^{2 i beta}
+                    b2.y = T(2) * cs * sn;
+                    sB1[jj * NL + gen_pos_b] = b1;
+                    sB2[jj * NL + gen_pos_b] = b2;
+                }
+                jb += JC;
+                if (ptid == 0) { meta[s].item = item; meta[s].last = (jb >= w.j1) ? 1 : 0; }
+                mbar_arrive(&full[s]);      // release: the stores above are visible to the waiting consumers
+                ++c;
+            } while (jb < w.j1);
+            named_bar_sync(1, kWsProducers);         // s_next_item written (and everyone done with this item's decode)
+            item = s_next_item;
+            named_bar_sync(1, kWsProducers);         // everyone has read it before thread 0 overwrites it
+        }
+    } else {
+        // =========================================== consumers ===============================================
+        const int lane = tid & 31, wq = (tid >> 5) & 3;
+        const bool is_w = tid >= kWsConsumers / 2;             // warps 4-7 contract W (doubled angles)
+        int gi, mi;
+        if (NMI == 8) {      // FP32: mi = (b1, b3, b4), gi = (b0, b2, warp)
+            mi = ((lane >> 1) & 1) | (((lane >> 3) & 3) << 1);
+            gi = (lane & 1) | (((lane >> 2) & 1) << 1) | (wq << 2);
+        } else {             // FP64: mi = (b1, b3), gi = (b0, b2, b4, warp)
+            mi = ((lane >> 1) & 1) | (((lane >> 3) & 1) << 1);
+            gi = (lane & 1) | (((lane >> 2) & 1) << 1) | (((lane >> 4) & 1) << 2) | (wq << 3);
+        }
+        const int offA = is_w ? JC * G : 0;
+        const int offB = 2 * JC * G + (is_w ? JC * NL : 0);
+
+        V2 acc_r[TH][TM], acc_i[TH][TM];        // (Srr, Sri) and (Sir, Sii) of this thread's (group, m) pairs
+#pragma unroll
+        for (int a = 0; a < TH; ++a)
+#pragma unroll
+            for (int cc = 0; cc < TM; ++cc) {
+                acc_r[a][cc].x = acc_r[a][cc].y = T(0);
+                acc_i[a][cc].x = acc_i[a][cc].y = T(0);
+            }
+        unsigned c = 0;
+        while (true) {
+            const int s = c % S;
+            mbar_wait(&full[s], (c / S) & 1);
+            const long long item = meta[s].item;
+            const int last = meta[s].last;
+            if (item < 0) break;
+            const V2* A = ring + (size_t)s * STAGE + offA;
+            const V2* B = ring + (size_t)s * STAGE + offB;
+#pragma unroll
+            for (int jj = 0; jj < JC; ++jj) {                  // step 4
+                V2 av[TH], bv[TM];
+                if constexpr (EPC == 2) {           // one LDS.128 = two complex operands
+#pragma unroll
+                    for (int q = 0; q < TH / 2; ++q) {
+                        const float4 ch = reinterpret_cast<const float4*>(A + jj * G)[q * NGI + gi];
+                        av[2 * q].x = ch.x; av[2 * q].y = ch.y; av[2 * q + 1].x = ch.z; av[2 * q + 1].y = ch.w;
+                    }
+#pragma unroll
+                    for (int q = 0; q < TM / 2; ++q) {
+                        const float4 ch = reinterpret_cast<const float4*>(B + jj * NL)[q * NMI + mi];
+                        bv[2 * q].x = ch.x; bv[2 * q].y = ch.y; bv[2 * q + 1].x = ch.z; bv[2 * q + 1].y = ch.w;
+                    }
+                } else {                            // one LDS.128 = one complex operand
+#pragma unroll
+                    for (int a = 0; a < TH; ++a) av[a] = A[jj * G + a * NGI + gi];
+#pragma unroll
+                    for (int cc = 0; cc < TM; ++cc) bv[cc] = B[jj * NL + cc * NMI + mi];
+                }
+#pragma unroll
+                for (int a = 0; a < TH; ++a)
+#pragma unroll
+                    for (int cc = 0; cc < TM; ++cc) cmac(acc_r[a][cc], acc_i[a][cc], av[a].x, av[a].y, bv[cc]);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+            ++c;
+            if (!last) continue;
+
+            // ---- epilogue of `item` (steps 5, 6, 6') -------------------------------------------------------------
+            const WsItem w = ws_decode<TILE>(gp, item, offsets);
+            const T scale = stats ? (T)stats[w.obj].scale : T(1);
+            // Each thread keeps the sums of its "own" half of its (group, m) pairs and publishes the other half:
+            // Z threads own cc < TM/2, W threads own cc >= TM/2.
+            // (register arrays are indexed with compile-time constants only; the role picks by select)
+            constexpr int HM = TM / 2;
+#pragma unroll
+            for (int a = 0; a < TH; ++a)
+#pragma unroll
+                for (int h = 0; h < HM; ++h) {
+                    const V2 pr = is_w ? acc_r[a][h] : acc_r[a][HM + h];
+                    const V2 pi = is_w ? acc_i[a][h] : acc_i[a][HM + h];
+                    const int kg = (gi * TH + a) * L, m = mi * TM + (is_w ? h : HM + h);
+                    V2 up, dn;
+                    up.x = pr.x - pi.y;    // Srr - Sii
+                    up.y = pr.y + pi.x;    // Sri + Sir
+                    dn.x = pr.x + pi.y;    // Srr + Sii
+                    dn.y = pi.x - pr.y;    // Sir - Sri
+                    sX[kg + NL + m] = up;
+                    sX[kg + NL - 1 - m] = dn;
+                }
+            named_bar_sync(2, kWsConsumers);
+            Best mine;
+            mine.p = -1.0;
+            mine.k = INT64_MAX;
+            const bool stage_out = (gp.n_split == 1) && (out_power != nullptr);
+#pragma unroll
+            for (int a = 0; a < TH; ++a)
+#pragma unroll
+                for (int h = 0; h < HM; ++h) {
+                    const V2 orr = is_w ? acc_r[a][HM + h] : acc_r[a][h];
+                    const V2 oi = is_w ? acc_i[a][HM + h] : acc_i[a][h];
+                    const int kg = (gi * TH + a) * L, m = mi * TM + (is_w ? HM + h : h);
+#pragma unroll
+                    for (int up = 0; up < 2; ++up) {
+                        const int kl = up ? (kg + NL + m) : (kg + NL - 1 - m);
+                        const int64_t k = w.K0 + kl;
+                        const V2 other = sX[kl];
+                        V2 me;
+                        if (up) {
+                            me.x = orr.x - oi.y;
+                            me.y = orr.y + oi.x;
+                        } else {
+                            me.x = orr.x + oi.y;
+                            me.y = oi.x - orr.y;
+                        }
+                        const V2 z = is_w ? other : me;      // (xc, xs)
+                        const V2 ww = is_w ? me : other;     // (c2, s2)
+                        if (gp.n_split > 1) {
+                            if (k < gp.n_freq)
+                                sums[((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + k] = make_vec4<T>(z.x, z.y, ww.x, ww.y);
+                        } else {
+                            const T p = power_from_sums<T>(z.x, z.y, ww.x, ww.y, (T)w.n_t, scale);
+                            if (stage_out) sP[kl] = p;
+                            if (k < gp.n_freq) {
+                                Best b;
+                                b.p = (p == p) ? (double)p : -1.0;
+                                b.k = k;
+                                mine = best_of(mine, b);
+                            }
+                        }
+                    }
+                }
+            if (stage_out) {
+                named_bar_sync(2, kWsConsumers);
+                T* dst = out_power + w.obj_local * gp.n_freq + w.K0;
+                const int n_valid = (int)min((int64_t)TILE, (int64_t)gp.n_freq - w.K0);
+                for (int i = tid; i < n_valid; i += kWsConsumers) dst[i] = sP[i];
+            }
+            if (partials && gp.n_split == 1) {
+                mine = warp_best(mine);
+                if (lane == 0) sbest[tid >> 5] = mine;
+                named_bar_sync(2, kWsConsumers);
+                if (tid < 32) {
+                    Best v;
+                    v.p = -2.0;
+                    v.k = INT64_MAX;
+                    if (lane < kWsConsumers / 32) v = sbest[lane];
+                    v = warp_best(v);
+                    if (lane == 0) partials[w.obj_local * gp.n_tiles + w.tile] = v;
+                }
+            }
+            named_bar_sync(2, kWsConsumers);      // sX / sP / sbest are free again before the next item's epilogue
+#pragma unroll
+            for (int a = 0; a < TH; ++a)
+#pragma unroll
+                for (int cc = 0; cc < TM; ++cc) {
+                    acc_r[a][cc].x = acc_r[a][cc].y = T(0);
+                    acc_i[a][cc].x = acc_i[a][cc].y = T(0);
+                }
+        }
+    }
+}
+
+}  // namespace lsp
