@@ -1,0 +1,409 @@
+#!/usr/bin/env python
+"""bench.py -- (t,f) pair-evaluations/s of the batched Lomb-Scargle hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4] [--dtype f32|f64] [--fast-math]
+    python bench.py --impl reference ...          # the CPU oracle, as it stands, on the box's host cores
+
+A "step" is one pass of the whole hot path (SURVEY.md section 8(a) steps 1-6/6', and 7 for host output) over one
+batch of seeded synthetic input.  Default workload: BASELINE.json configs[1] (single object, N_t = 10,000,
+N_f = 1,000,000, full periodogram), in FP32 (primary line) and FP64 (the "fp64" object of the same line).
+  value       device-resident: inputs and output in HBM, CUDA events around each step on the launching stream
+  e2e         the same pass through lsp_periodogram_batched_host: pinned HOST inputs, H2D + kernels + D2H inside
+              the timed region
+  roofline    the dominant kernel against the FMA-pipe (FP32) / FP64-pipe peak: "bound": "alu"
+  cpu_baseline  the oracle timed on a bounded sample of the same workload (rank 0, N = 1 only)
+Multi-GPU (torchrun, one rank per GPU): every rank runs its own object of the same shape (seed + rank), no data-path
+collective ("scaling": "weak"); times are device times, max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "lsp_pair_evals_per_s"
+UNIT = "pairs/s"
+
+# ALU roofline denominators: 148 SMs x lanes/clk/SM x 2 flop x clocks.max.sm (1965 MHz, B200_PROFILING.md)
+N_SM = 148
+SM_MAX_HZ = 1965e6
+FP32_LANES = 128      # FP32 FMA lanes per SM per clock
+FP64_LANES = 64       # FP64 FMA lanes per SM per clock
+FLOP_PER_PAIR = 8.0   # factored formulation: 4 FMA per (t,f) pair ("4 FMA = 8 flop/pair")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4"])
+    ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="precision of the primary line")
+    ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the other-precision leg")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
+    return ap.parse_args()
+
+
+def workload_for(name: str, dtype: str, rank: int):
+    from workloads import make_config
+    from workloads.configs import config_seed  # noqa: F401  (seed recipe: DESIGN.md "Input recipe")
+    cfg = {"c2": 2, "c3": 3, "c4": 4}[name]
+    # weak scaling: rank r draws its own object(s) from the same generator with sweep-point index r
+    return make_config(cfg, dtype=dtype, point=rank)
+
+
+# ---- clocks --------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "hw_power_brake": 0x80}
+    NOTE = {"sw_power_cap": 0x4}
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reasons = [], set()
+        self.period, self.stop_flag, self.thread, self.ok = period_s, threading.Event(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                try:
+                    phys = int(vis.split(",")[index])
+                except ValueError:
+                    phys = index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as exc:  # no NVML: clocks are reported as unavailable, never invented
+            self.err = repr(exc)
+
+    def _run(self):
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in {**self.BAD, **self.NOTE}.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self.thread = threading.Thread(target=self._run, daemon=True)
+            self.thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        if self.thread:
+            self.stop_flag.set()
+            self.thread.join()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml_unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": float(s[len(s) // 2]), "sm_max_mhz": float(self.max_mhz), "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+# ---- the CPU oracle leg (cpu_baseline and --impl reference) ---------------------------------------------------
+def oracle_sample_runner(w, seconds_per_step: float):
+    """Returns (run, pairs_per_step, cores, description): `run()` evaluates the oracle, as it stands, on a bounded
+    sample of workload `w`: whole objects for batches, a strided subset of the grid for a single object."""
+    import numpy as np
+    import oracle
+    oracle.build()
+    probe_k = np.linspace(0, w.n_freq - 1, 512).astype(np.int64)
+    one = w.take_objects([0]) if w.n_obj > 1 else w
+    t0 = time.perf_counter()
+    _, cores = oracle.periodogram(one.offsets, one.t, one.y, w.f_min, w.f_max, w.n_freq, k_list=probe_k, return_threads=True)
+    dt = max(time.perf_counter() - t0, 1e-4)
+    rate = one.n_obs * probe_k.size / dt                 # pairs/s seen by the probe
+    pairs_target = rate * seconds_per_step
+    if w.n_obj == 1:
+        n_k = int(min(w.n_freq, max(cores * 8, pairs_target / max(1, w.n_obs))))
+        ks = np.unique(np.linspace(0, w.n_freq - 1, n_k).astype(np.int64))
+        sub, desc = w, f"{ks.size} of {w.n_freq} grid frequencies (strided) x all {w.n_obs} observations"
+    else:
+        ks = np.unique(np.linspace(0, w.n_freq - 1, min(w.n_freq, 2000)).astype(np.int64))
+        mean_nt = w.n_obs / w.n_obj
+        n_o = int(min(w.n_obj, max(2 * cores, pairs_target / (mean_nt * ks.size))))
+        sub = w.take_objects(np.arange(n_o))
+        desc = f"first {n_o} of {w.n_obj} objects x {ks.size} of {w.n_freq} grid frequencies (strided)"
+
+    def run():
+        oracle.periodogram(sub.offsets, sub.t, sub.y, w.f_min, w.f_max, w.n_freq, k_list=ks)
+
+    return run, int(sub.n_obs) * int(ks.size), int(cores), desc
+
+
+def cpu_baseline(w, seconds: float):
+    run, pairs, cores, desc = oracle_sample_runner(w, seconds)
+    t0 = time.perf_counter()
+    run()
+    dt = time.perf_counter() - t0
+    return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+            "seconds": round(dt, 3)}
+
+
+def run_reference(args, rank: int, world: int):
+    if rank != 0:
+        return
+    w = workload_for(args.workload, args.dtype, 0)
+    n_steps = args.steps + args.warmup
+    per_step = max(0.05, min(3.0, 90.0 / max(1, n_steps)))
+    run, pairs, cores, desc = oracle_sample_runner(w, per_step)
+    for _ in range(args.warmup):
+        run()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        run()
+    dt = time.perf_counter() - t0
+    value = pairs * args.steps / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": describe_workload(args.workload, w), "sample_per_step": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def describe_workload(name: str, w) -> str:
+    if name == "c2":
+        return (f"BASELINE.json configs[1]: single object, N_t={w.n_obs}, N_f={w.n_freq}, f in [{w.f_min},{w.f_max}) c/d, "
+                f"full periodogram")
+    if name == "c3":
+        return (f"BASELINE.json configs[2]: {w.n_obj} objects, N_t in [50,500] (sum {w.n_obs}), N_f={w.n_freq}, "
+                f"best period only")
+    return (f"BASELINE.json configs[3]: {w.n_obj} objects (sum N_t {w.n_obs}), N_f={w.n_freq}, full periodogram to "
+            f"pinned host over copy streams")
+
+
+# ---- the B200 leg -----------------------------------------------------------------------------------------------
+class Leg:
+    """One precision of one workload on this rank's GPU: device-resident steps and end-to-end (host buffer) steps."""
+
+    def __init__(self, pkg, torch, w, name: str, dtype: str, fast_math: bool, kernel: str, device: int):
+        self.torch, self.w, self.name, self.dtype = torch, w, name, dtype
+        self.tdt = torch.float32 if dtype == "f32" else torch.float64
+        self.plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, dtype, fast_math=fast_math and dtype == "f32", kernel=kernel,
+                             device=device)
+        self.plan.set_timing(True)
+        self.h_off = torch.from_numpy(w.offsets)
+        self.h_t = torch.from_numpy(w.t).pin_memory()
+        self.h_y = torch.from_numpy(w.y).pin_memory()
+        dev = torch.device("cuda", device)
+        self.d_off, self.d_t, self.d_y = self.h_off.to(dev), self.h_t.to(dev), self.h_y.to(dev)
+        self.best_only = name == "c3"
+        self.host_mode = name == "c4"          # the workload itself ends on the host
+        n = w.n_obj
+        self.d_best = (torch.empty(n, dtype=self.tdt, device=dev), torch.empty(n, dtype=self.tdt, device=dev),
+                       torch.empty(n, dtype=torch.int64, device=dev))
+        self.h_best = (torch.empty(n, dtype=self.tdt).pin_memory(), torch.empty(n, dtype=self.tdt).pin_memory(),
+                       torch.empty(n, dtype=torch.int64).pin_memory())
+        self.d_out = self.h_out = None
+        if not self.best_only:
+            if self.host_mode:
+                self.h_out = torch.empty((n, w.n_freq), dtype=self.tdt).pin_memory()
+            else:
+                self.d_out = torch.empty((n, w.n_freq), dtype=self.tdt, device=dev)
+                self.h_out = torch.empty((n, w.n_freq), dtype=self.tdt).pin_memory()
+        self.launches = 0
+        self.kernel_ms = []
+
+    def step_device(self):
+        """Inputs resident in HBM.  c2: full periodogram to HBM; c3: fused best period; c4: periodograms to pinned host."""
+        if self.best_only:
+            self.plan.best_period(self.d_off, self.d_t, self.d_y, out=self.d_best, h_offsets=self.h_off)
+        elif self.host_mode:
+            self.plan.periodogram_batched(self.d_off, self.d_t, self.d_y, host_out=self.h_out, h_offsets=self.h_off)
+        else:
+            self.plan.periodogram_batched(self.d_off, self.d_t, self.d_y, out=self.d_out, h_offsets=self.h_off)
+
+    def step_e2e(self):
+        if self.best_only:
+            self.plan.periodogram_batched_host(self.h_off, self.h_t, self.h_y, best_out=self.h_best)
+        else:
+            self.plan.periodogram_batched_host(self.h_off, self.h_t, self.h_y, host_out=self.h_out)
+
+    def e2e_bytes(self):
+        h2d = self.h_off.numel() * 8 + self.h_t.numel() * self.h_t.element_size() * 2
+        if self.best_only:
+            d2h = sum(x.numel() * x.element_size() for x in self.h_best)
+        else:
+            d2h = self.h_out.numel() * self.h_out.element_size()
+        return int(h2d), int(d2h)
+
+    def note_call(self, timed: bool):
+        info = self.plan.last_call_info()
+        if timed:
+            self.launches += info["launches"]
+            self.kernel_ms.append(self.plan.last_kernel_ms())
+        return info
+
+
+def timed_loop(torch, dist, world, leg, step, steps: int, warmup: int, flush):
+    """W warm-up steps, then K steps, each bracketed by CUDA events on the launching (current) stream; the L2 flush runs
+    between steps, outside the event pairs.  Returns (total_ms over K steps: max over ranks, info of the last call)."""
+    for _ in range(warmup):
+        flush()
+        step()
+        leg.note_call(False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+        torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    info = None
+    for a, b in ev:
+        flush()
+        a.record()
+        step()
+        b.record()
+        info = leg.note_call(True)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+        torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    if world > 1:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    return total_ms, info
+
+
+def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_clocks: bool):
+    w = workload_for(args.workload, dtype, rank)
+    leg = Leg(pkg, torch, w, args.workload, dtype, args.fast_math, args.kernel, device)
+    pairs_step = w.pairs
+    pairs_all = pairs_step
+    if world > 1:
+        tt = torch.tensor([float(pairs_step)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.SUM)
+        pairs_all = float(tt.item())
+    sampler = ClockSampler(device) if with_clocks else None
+    if sampler:
+        sampler.__enter__()
+    total_ms, info = timed_loop(torch, dist, world, leg, leg.step_device, args.steps, args.warmup, flush)
+    if sampler:
+        sampler.__exit__()
+    dev_launches, kernel_ms = leg.launches, list(leg.kernel_ms)
+    leg.launches, leg.kernel_ms = 0, []
+    e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, args.steps, args.warmup, flush)
+    h2d, d2h = leg.e2e_bytes()
+    ms_step = total_ms / args.steps
+    k_ms = sum(kernel_ms) / len(kernel_ms)
+    lanes = FP32_LANES if dtype == "f32" else FP64_LANES
+    peak_tflops = N_SM * lanes * 2 * SM_MAX_HZ / 1e12
+    factored = info["kernel"] == "factored"
+    flop_pair = FLOP_PER_PAIR if factored else None
+    achieved = (pairs_step * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12) if factored else None
+    # measured pipe peak with the same clocks the kernels see (register-only FFMA2 / DFMA loops, lsp_pipe_peak)
+    pipe_ops, _ = pkg.lsp_pipe_peak(1 if dtype == "f32" else 2, device)
+    out = {
+        "dtype": dtype,
+        "value": pairs_all * args.steps / (total_ms * 1e-3),
+        "ms_per_step": ms_step,
+        "kernel": info["kernel"], "n_split": info["n_split"],
+        "kernel_ms_per_step": k_ms,
+        "gpu_launches": dev_launches,
+        "e2e": {"value": pairs_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
+        "roofline": {
+            "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+            "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
+            "kernel": ("lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double")) if factored else "lsp_direct_kernel",
+            "flop_per_pair": flop_pair,
+            "peak_is": "derived: 148 SMs x %d %s FMA lanes/clk/SM x 2 flop x 1965 MHz (clocks.max.sm)" % (lanes, "FP32" if dtype == "f32" else "FP64"),
+            "pipe_peak_measured": pipe_ops * 2 / 1e12,
+            "frac_of_measured_pipe": (achieved / (pipe_ops * 2 / 1e12)) if achieved else None,
+        },
+    }
+    if sampler:
+        out["clocks"] = sampler.summary()
+    leg.plan.destroy()
+    return out, w
+
+
+def run_b200(args, rank: int, world: int, local_rank: int):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device visible; the library has no CPU fallback (use --impl reference for the oracle)")
+    import paper_2105_04006_b200 as pkg
+    pkg.load_library()
+    dist = None
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")     # > 126 MB L2
+
+    def flush():
+        flush_buf.fill_(1)
+
+    primary, w = run_leg(args, pkg, torch, dist, rank, world, local_rank, args.dtype, flush, True)
+    other = None
+    if not args.no_secondary and args.workload == "c2":
+        other_dtype = "f64" if args.dtype == "f32" else "f32"
+        other, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, other_dtype, flush, False)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = cpu_baseline(w, args.cpu_seconds)
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": primary["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": primary["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": primary["dtype"], "data": "synthetic",
+            "config": {"workload": describe_workload(args.workload, w), "kernel": primary["kernel"],
+                       "fast_math": bool(args.fast_math and args.dtype == "f32"), "n_split": primary["n_split"],
+                       "l2": "flushed between steps (256 MiB fill, outside the event pairs)",
+                       "parallelism": f"replicas x{world} (one object set per rank, no collective)"},
+            "e2e": primary["e2e"], "gpu_launches": primary["gpu_launches"],
+            "kernel_ms_per_step": primary["kernel_ms_per_step"],
+            "roofline": primary["roofline"], "clocks": primary.get("clocks"),
+        }
+        if other is not None:
+            line[other["dtype"] == "f64" and "fp64" or "fp32"] = {k: other[k] for k in
+                                                                 ("value", "ms_per_step", "kernel_ms_per_step", "e2e", "roofline",
+                                                                  "gpu_launches", "kernel")}
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_b200(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

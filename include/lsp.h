@@ -118,6 +118,27 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj,
                            void* d_best_period, void* d_best_power, int64_t* d_best_index,
                            void* cuda_stream);
 
+/*
+ * End-to-end form of the two calls above for callers whose data lives on the HOST (the paper's own call
+ * shape: H2D of the concatenated (t, y) arrays, kernel, D2H of periodograms and/or periods,
+ * PAPER.md:L85-91, L103-117).  Every pointer is a HOST pointer (pinned memory lets the copies overlap;
+ * pageable memory works but serialises):
+ *   h_offsets    int64[n_obj+1]   (validated: offsets[0] = 0, non-decreasing)
+ *   h_t, h_y     offsets[n_obj] elements of cfg.dtype
+ *   h_out_power  n_obj * n_freq elements of cfg.dtype, or NULL for best-period-only output (the
+ *                N_obj x N_f array is then never written anywhere)
+ *   h_best_*     optional (all three NULL or all three non-NULL; required when h_out_power is NULL)
+ * The inputs are copied to plan-owned device buffers on cuda_stream, the same kernels run, full
+ * periodograms come back through the chunk ring and copy streams (step 7) and the best-period arrays by
+ * one small D2H each.  The call returns after everything has landed on the host.
+ * Errors as for lsp_periodogram_batched.
+ */
+lsp_status lsp_periodogram_batched_host(lsp_plan* plan, int64_t n_obj,
+                                        const int64_t* h_offsets, const void* h_t, const void* h_y,
+                                        void* h_out_power,
+                                        void* h_best_period, void* h_best_power, int64_t* h_best_index,
+                                        void* cuda_stream);
+
 /* Frees the plan and everything it owns (synchronises its streams first).  NULL is a no-op. */
 void lsp_destroy(lsp_plan* plan);
 

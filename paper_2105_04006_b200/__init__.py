@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     lsp_best_period,
     lsp_destroy,
     lsp_periodogram_batched,
+    lsp_periodogram_batched_host,
     lsp_pipe_peak,
     lsp_plan_create,
     lsp_version,

@@ -22,7 +22,8 @@ _STATUS = {0: "LSP_OK", 1: "LSP_ERR_INVALID_ARG", 2: "LSP_ERR_CUDA", 3: "LSP_ERR
 _KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LSP_KERNEL_FACTORED}
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
-EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_destroy", "lsp_last_error",
+EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host", "lsp_destroy",
+           "lsp_last_error",
            "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_pipe_peak", "lsp_version")
 
 
@@ -59,6 +60,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_periodogram_batched.restype = ctypes.c_int
     lib.lsp_best_period.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsp_best_period.restype = ctypes.c_int
+    lib.lsp_periodogram_batched_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.lsp_periodogram_batched_host.restype = ctypes.c_int
     lib.lsp_destroy.argtypes = [vp]
     lib.lsp_destroy.restype = None
     lib.lsp_last_error.argtypes = [vp]
@@ -116,6 +119,14 @@ def lsp_best_period(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y, d_best_per
     _check(load_library().lsp_best_period(plan, int(n_obj), _dptr(d_offsets), h_ptr, _dptr(d_t), _dptr(d_y),
                                           _dptr(d_best_period), _dptr(d_best_power), _dptr(d_best_index),
                                           _stream_ptr(stream)), plan)
+
+
+def lsp_periodogram_batched_host(plan, n_obj: int, h_offsets, h_t, h_y, h_out_power=None, h_best_period=None,
+                                 h_best_power=None, h_best_index=None, stream=None) -> None:
+    """All-HOST form (include/lsp.h): every tensor is a host tensor; H2D, kernels and D2H run inside the call."""
+    _check(load_library().lsp_periodogram_batched_host(plan, int(n_obj), _dptr(h_offsets), _dptr(h_t), _dptr(h_y),
+                                                       _dptr(h_out_power), _dptr(h_best_period), _dptr(h_best_power),
+                                                       _dptr(h_best_index), _stream_ptr(stream)), plan)
 
 
 def lsp_destroy(plan) -> None:
@@ -216,6 +227,28 @@ class Plan:
             bi = torch.empty(n_obj, dtype=torch.int64, device=self.device)
         lsp_periodogram_batched(self._plan, n_obj, offsets, h_offsets, t, y, power, is_host, bp, bw, bi, stream)
         return power, ((bp, bw, bi) if best else None)
+
+    def periodogram_batched_host(self, h_offsets, h_t, h_y, *, host_out=None, best_out=None, stream=None):
+        """End-to-end call on HOST tensors (pinned for overlap): fills `host_out` [n_obj, n_freq] (or skips the
+        periodogram when None) and `best_out` = (period, power, index) host tensors (optional unless host_out
+        is None).  Returns after all results are on the host."""
+        if h_offsets.is_cuda or h_offsets.dtype != torch.int64:
+            raise TypeError("h_offsets must be a host int64 tensor")
+        n_obj = int(h_offsets.numel() - 1)
+        for x in (h_t, h_y):
+            if x.is_cuda or x.dtype != self.torch_dtype or not x.is_contiguous():
+                raise TypeError(f"h_t and h_y must be contiguous host tensors of {self.torch_dtype}")
+        if host_out is not None and (host_out.is_cuda or host_out.dtype != self.torch_dtype or not host_out.is_contiguous()
+                                     or host_out.numel() != n_obj * self.n_freq):
+            raise TypeError("host_out must be a contiguous host tensor [n_obj, n_freq] of the plan dtype")
+        bp = bw = bi = None
+        if best_out is not None:
+            bp, bw, bi = best_out
+            if bp.is_cuda or bw.is_cuda or bi.is_cuda or bp.dtype != self.torch_dtype or bw.dtype != self.torch_dtype \
+                    or bi.dtype != torch.int64 or min(bp.numel(), bw.numel(), bi.numel()) < n_obj:
+                raise TypeError("best_out must be host tensors (period, power, index[int64]) of n_obj elements")
+        lsp_periodogram_batched_host(self._plan, n_obj, h_offsets, h_t, h_y, host_out, bp, bw, bi, stream)
+        return host_out, best_out
 
     def best_period(self, offsets, t, y, *, out=None, h_offsets=None, stream=None):
         """Fused best period: (period, power, index) device tensors; the periodogram is never materialised."""

@@ -44,6 +44,7 @@ struct lsp_plan {
     DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
     DeviceBuffer stats;           // ObjStats[n_obj]
     DeviceBuffer counter;         // work counter of the persistent kernel
+    DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t* h_offsets_pinned = nullptr;
     size_t   h_offsets_cap = 0;
@@ -294,8 +295,8 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
     if (n_best != 0 && n_best != 3) return fail(p, LSP_ERR_INVALID_ARG, "best_period/best_power/best_index: give all three or none");
     const bool want_best = n_best == 3;
-    if (!out_power && !want_best) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
     if (n_obj == 0) return LSP_OK;
+    if (!out_power && !want_best) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
     if (!d_off) return fail(p, LSP_ERR_INVALID_ARG, "d_offsets is NULL");
     if (n_obj > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "n_obj too large");
     LSP_CUDA(p, cudaSetDevice(c.device));
@@ -465,7 +466,8 @@ lsp_status lsp_periodogram_batched(lsp_plan* plan, int64_t n_obj, const int64_t*
                                    void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
 {
     if (!plan) return LSP_ERR_INVALID_ARG;
-    if (!out_power) return fail(plan, LSP_ERR_INVALID_ARG, "out_power is NULL (use lsp_best_period for best-only output)");
+    if (!out_power && n_obj != 0)
+        return fail(plan, LSP_ERR_INVALID_ARG, "out_power is NULL (use lsp_best_period for best-only output)");
     return run_call(plan, n_obj, d_offsets, h_offsets, d_t, d_y, out_power, out_is_host, d_best_period, d_best_power,
                     d_best_index, cuda_stream);
 }
@@ -481,6 +483,58 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj, const int64_t* d_offse
                     cuda_stream);
 }
 
+lsp_status lsp_periodogram_batched_host(lsp_plan* plan, int64_t n_obj, const int64_t* h_offsets, const void* h_t,
+                                        const void* h_y, void* h_out_power, void* h_best_period, void* h_best_power,
+                                        int64_t* h_best_index, void* cuda_stream)
+{
+    lsp_plan* p = plan;
+    if (!p) return LSP_ERR_INVALID_ARG;
+    const lsp_config& c = p->cfg;
+    if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
+    const int n_best = (h_best_period != nullptr) + (h_best_power != nullptr) + (h_best_index != nullptr);
+    if (n_best != 0 && n_best != 3) return fail(p, LSP_ERR_INVALID_ARG, "best_period/best_power/best_index: give all three or none");
+    if (!h_out_power && n_best == 0) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
+    p->n_launches = p->n_pairs = p->n_chunks = 0;
+    if (n_obj == 0) return LSP_OK;
+    if (!h_offsets) return fail(p, LSP_ERR_INVALID_ARG, "h_offsets is NULL");
+    if (h_offsets[0] != 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[0] != 0");
+    for (int64_t o = 0; o < n_obj; ++o)
+        if (h_offsets[o + 1] < h_offsets[o]) return fail(p, LSP_ERR_INVALID_ARG, "offsets decrease at object %lld", (long long)o);
+    const int64_t total_obs = h_offsets[n_obj];
+    if (total_obs > 0 && (!h_t || !h_y)) return fail(p, LSP_ERR_INVALID_ARG, "h_t / h_y is NULL");
+    LSP_CUDA(p, cudaSetDevice(c.device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t es = elem_size(c);
+    lsp_status e;
+    if ((e = ensure(p, p->in_off, (size_t)(n_obj + 1) * sizeof(int64_t))) != LSP_OK) return e;
+    if ((e = ensure(p, p->in_t, std::max<size_t>(16, (size_t)total_obs * es))) != LSP_OK) return e;
+    if ((e = ensure(p, p->in_y, std::max<size_t>(16, (size_t)total_obs * es))) != LSP_OK) return e;
+    LSP_CUDA(p, cudaMemcpyAsync(p->in_off.ptr, h_offsets, (size_t)(n_obj + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    if (total_obs > 0) {
+        LSP_CUDA(p, cudaMemcpyAsync(p->in_t.ptr, h_t, (size_t)total_obs * es, cudaMemcpyHostToDevice, st));
+        LSP_CUDA(p, cudaMemcpyAsync(p->in_y.ptr, h_y, (size_t)total_obs * es, cudaMemcpyHostToDevice, st));
+    }
+    char* d_bper = nullptr;
+    char* d_bpow = nullptr;
+    int64_t* d_bidx = nullptr;
+    if (n_best) {
+        if ((e = ensure(p, p->out_best, (size_t)n_obj * (2 * es + sizeof(int64_t)))) != LSP_OK) return e;
+        d_bidx = (int64_t*)p->out_best.ptr;                       // int64 first: keeps every array aligned
+        d_bper = (char*)p->out_best.ptr + (size_t)n_obj * sizeof(int64_t);
+        d_bpow = d_bper + (size_t)n_obj * es;
+    }
+    e = run_call(p, n_obj, (const int64_t*)p->in_off.ptr, h_offsets, p->in_t.ptr, p->in_y.ptr, h_out_power,
+                 h_out_power ? 1 : 0, d_bper, d_bpow, d_bidx, cuda_stream);
+    if (e != LSP_OK) return e;
+    if (n_best) {
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_index, d_bidx, (size_t)n_obj * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_period, d_bper, (size_t)n_obj * es, cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_power, d_bpow, (size_t)n_obj * es, cudaMemcpyDeviceToHost, st));
+    }
+    LSP_CUDA(p, cudaStreamSynchronize(st));
+    return LSP_OK;
+}
+
 void lsp_destroy(lsp_plan* p)
 {
     if (!p) return;
@@ -493,7 +547,7 @@ void lsp_destroy(lsp_plan* p)
     for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
-    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter})
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
     cudaGetLastError();
