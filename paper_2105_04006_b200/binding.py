@@ -52,7 +52,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     global _lib
     if _lib is not None and path is None:
         return _lib
-    lib = ctypes.CDLL(path or _build.build())
+    # LSP_B200_LIB names a prebuilt library to use instead of the in-tree build (kernel A/B experiments)
+    lib = ctypes.CDLL(path or os.environ.get("LSP_B200_LIB") or _build.build())
     vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
     lib.lsp_plan_create.argtypes = [ctypes.POINTER(LspConfig), ctypes.POINTER(vp)]
     lib.lsp_plan_create.restype = ctypes.c_int

@@ -24,15 +24,27 @@ constexpr int kWsConsumers = 256;
 constexpr int kWsProducers = 128;
 constexpr int kWsThreads = kWsConsumers + kWsProducers;
 
+#ifndef LSP_WS_JC_F32
+#define LSP_WS_JC_F32 16
+#endif
+#ifndef LSP_WS_JC_F64
+#define LSP_WS_JC_F64 16
+#endif
+#ifndef LSP_WS_STAGES_F32
+#define LSP_WS_STAGES_F32 4
+#endif
+#ifndef LSP_WS_STAGES_F64
+#define LSP_WS_STAGES_F64 4
+#endif
 template <typename T> struct WsCfg;
 template <> struct WsCfg<float> {
-    static constexpr int JC = 8;         // observations per ring stage
-    static constexpr int STAGES = 6;
+    static constexpr int JC = LSP_WS_JC_F32;         // observations per ring stage
+    static constexpr int STAGES = LSP_WS_STAGES_F32;
     static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<float>::NL);   // complex elements per stage
 };
 template <> struct WsCfg<double> {
-    static constexpr int JC = 4;
-    static constexpr int STAGES = 6;
+    static constexpr int JC = LSP_WS_JC_F64;
+    static constexpr int STAGES = LSP_WS_STAGES_F64;
     static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<double>::NL);
 };
 
