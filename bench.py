@@ -48,7 +48,7 @@ def parse_args():
     ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4"])
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="precision of the primary line")
     ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored", "tensor"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="skip the other-precision leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")

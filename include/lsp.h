@@ -49,10 +49,13 @@ typedef enum {
 
 /* Which periodogram kernel family runs steps 2-5 of the hot path. */
 typedef enum {
-    LSP_KERNEL_AUTO = 0,     /* library picks (factored unless the problem is too small to fill it)     */
+    LSP_KERNEL_AUTO = 0,     /* library picks: tensor (FP32) / factored (FP64), direct for grids under 1024 points */
     LSP_KERNEL_DIRECT = 1,   /* one sincos per (t,f) pair, thread = frequency (the paper's Listing 1 shape,
                                 PAPER.md:L137-216, with smem staging L121-125 and range-reduced phase)     */
-    LSP_KERNEL_FACTORED = 2  /* angle-addition outer product: no sincos in the O(N_t N_f) loop, 4 FMA/pair */
+    LSP_KERNEL_FACTORED = 2, /* angle-addition outer product: no sincos in the O(N_t N_f) loop, 4 FMA/pair */
+    LSP_KERNEL_TENSOR = 3    /* FP32 mode only: the same contraction on the tensor cores (tcgen05.mma kind::f16, FP32
+                                accumulators in TMEM).  Operands are FP16 hi+lo pairs, three MMAs per product
+                                (fast_math = 1: hi only, one MMA, MUFU sincos); phases stay FP64-reduced.          */
 } lsp_kernel;
 
 typedef struct lsp_config {

@@ -16,10 +16,11 @@ import torch
 from . import build as _build
 
 LSP_F32, LSP_F64 = 0, 1
-LSP_KERNEL_AUTO, LSP_KERNEL_DIRECT, LSP_KERNEL_FACTORED = 0, 1, 2
+LSP_KERNEL_AUTO, LSP_KERNEL_DIRECT, LSP_KERNEL_FACTORED, LSP_KERNEL_TENSOR = 0, 1, 2, 3
 LSP_OK, LSP_ERR_INVALID_ARG, LSP_ERR_CUDA, LSP_ERR_OOM, LSP_ERR_UNSUPPORTED = 0, 1, 2, 3, 4
 _STATUS = {0: "LSP_OK", 1: "LSP_ERR_INVALID_ARG", 2: "LSP_ERR_CUDA", 3: "LSP_ERR_OOM", 4: "LSP_ERR_UNSUPPORTED"}
-_KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LSP_KERNEL_FACTORED}
+_KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LSP_KERNEL_FACTORED,
+            "tensor": LSP_KERNEL_TENSOR}
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
 EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host", "lsp_destroy",

@@ -13,9 +13,11 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "lsp_factored_ws.cuh"
+#include "lsp_tensor.cuh"
 #include "lsp_peak.cuh"
 
 using namespace lsp;
@@ -34,6 +36,7 @@ struct DeviceBuffer {
 struct lsp_plan {
     lsp_config cfg{};
     int sm_count = 0;
+    int smem_optin = 0;           // max dynamic shared memory per CTA
     std::string error;
 
     std::vector<cudaStream_t> copy_streams;
@@ -44,6 +47,9 @@ struct lsp_plan {
     DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
     DeviceBuffer stats;           // ObjStats[n_obj]
     DeviceBuffer counter;         // work counter of the persistent kernel
+    DeviceBuffer tc_objs;         // TensorObj[n_obj_launch]   (tensor path pre-pass)
+    DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
+    size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t* h_offsets_pinned = nullptr;
@@ -100,6 +106,7 @@ struct Schedule {
     int tile;        // frequencies per CTA
     int n_tiles;
     int n_split;
+    TensorParams tp;   // tensor path only
 };
 
 Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
@@ -107,10 +114,26 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
     const lsp_config& c = p->cfg;
     Schedule s{};
     int k = c.kernel;
-    if (k == LSP_KERNEL_AUTO) k = (c.n_freq >= 1024) ? LSP_KERNEL_FACTORED : LSP_KERNEL_DIRECT;
+    if (k == LSP_KERNEL_AUTO)
+        k = (c.n_freq < 1024) ? LSP_KERNEL_DIRECT : (c.dtype == LSP_F32 ? LSP_KERNEL_TENSOR : LSP_KERNEL_FACTORED);
     s.kernel = k;
     int64_t slots;                                                // resident CTAs on the whole GPU
-    if (k == LSP_KERNEL_FACTORED) {
+    if (k == LSP_KERNEL_TENSOR) {
+        // tiles of 64 groups x 2 NL frequencies, NL the smallest multiple of 8 that covers N_f with the fewest tiles
+        const int64_t max_tile = (int64_t)kTcGroups * 2 * kTcMaxNL;
+        const int64_t nt = (c.n_freq + max_tile - 1) / max_tile;
+        int64_t nl = (c.n_freq + nt * 2 * kTcGroups - 1) / (nt * 2 * kTcGroups);
+        nl = std::min<int64_t>(kTcMaxNL, std::max<int64_t>(8, (nl + 7) / 8 * 8));
+        s.tp.nl = (int)nl;
+        s.tp.tile = (int)(kTcGroups * 2 * nl);
+        s.tp.n_ops = c.fast_math ? 2 : 4;
+        s.tp.a_stage_bytes = s.tp.n_ops * 128 * kTcKB * 2;
+        s.tp.b_stage_bytes = s.tp.n_ops * 2 * (int)nl * kTcKB * 2;
+        s.tp.stages = (int)std::min<int64_t>(8, (int64_t)(p->smem_optin - 2048) / (s.tp.a_stage_bytes + s.tp.b_stage_bytes));
+        s.tile = s.tp.tile;
+        s.direct_r = 0;
+        slots = p->sm_count;
+    } else if (k == LSP_KERNEL_FACTORED) {
         s.tile = c.dtype == LSP_F32 ? fac_tile<float>() : fac_tile<double>();
         s.direct_r = 0;
         slots = p->use_ws ? (int64_t)p->sm_count                  // one persistent CTA per SM
@@ -129,7 +152,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
     int64_t split = 1;
     if (items < 8 * slots && n_obj > 0) {
         const int64_t avg_nt = total_obs / std::max<int64_t>(1, n_obj);
-        const int64_t min_obs = (k == LSP_KERNEL_FACTORED) ? 128 : 64;      // per split, to amortise prologue/epilogue
+        const int64_t min_obs = (k == LSP_KERNEL_TENSOR) ? 256 : (k == LSP_KERNEL_FACTORED) ? 128 : 64;   // per split, to amortise prologue/epilogue
         const int64_t s_max = std::max<int64_t>(1, std::min<int64_t>(64, avg_nt / min_obs));
         double best_score = -1.0;
         for (int64_t cand = 1; cand <= s_max; ++cand) {
@@ -153,7 +176,24 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
     const int64_t grid = n_obj_launch * s.n_tiles * s.n_split;
     if (grid <= 0) return cudaSuccess;
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws) {
+    if (s.kernel == LSP_KERNEL_TENSOR) {
+        if constexpr (std::is_same<T, float>::value) {
+            auto kern = lsp_tensor_kernel<float, FAST>;
+            const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
+            static size_t attr_smem = 0;       // per instantiation
+            if (smem > attr_smem) {
+                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                if (e != cudaSuccess) return e;
+                attr_smem = smem;
+            }
+            const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
+            kern<<<ctas, kTcThreads, smem, st>>>(gp, s.tp, d_off, (const float*)d_t, (const float*)d_y,
+                                                 (const TensorObj*)p->tc_objs.ptr, (const __half*)p->tc_table.ptr, (float*)out,
+                                                 partials, (float4*)sums, n_obj_launch, (long long)grid);
+        } else {
+            return cudaErrorInvalidValue;      // rejected at plan creation
+        }
+    } else if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws) {
         auto kern = lsp_factored_ws_kernel<T, FAST>;
         static bool attr_done = false;     // per instantiation
         if (!attr_done) {
@@ -189,10 +229,37 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 
 // Launches steps 2-6' for objects [obj_base, obj_base + n_obj_launch) on `st`.
 // `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed globally.
-lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n_obj_launch, const int64_t* d_off,
-                     const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out, cudaStream_t st)
+lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
+                     const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
+                     cudaStream_t st)
 {
     const lsp_config& c = p->cfg;
+    if (s.kernel == LSP_KERNEL_TENSOR) {
+        // pre-pass of the tensor path: per-object statistics, table offsets, then the B-operand table (once per object,
+        // shared by all of its frequency tiles and observation splits)
+        const int64_t kb_bound = obs_bound / kTcKB + n_obj_launch;
+        lsp_status e = ensure(p, p->tc_objs, (size_t)(n_obj_launch + 1) * sizeof(TensorObj));
+        if (e != LSP_OK) return e;
+        if ((e = ensure(p, p->tc_table, std::max<size_t>(256, (size_t)kb_bound * (size_t)s.tp.b_stage_bytes))) != LSP_OK) return e;
+        GridParams gq{};
+        gq.f_min = c.f_min;
+        gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
+        gq.n_freq = (int)c.n_freq;
+        gq.obj_base = (int)obj_base;
+        lsp_tensor_stats_kernel<float><<<(unsigned)n_obj_launch, 128, 0, st>>>(d_off, (const float*)d_y, (TensorObj*)p->tc_objs.ptr,
+                                                                            (int)obj_base, c.center, c.normalize);
+        lsp_tensor_scan_kernel<<<1, 1024, 0, st>>>(d_off, (TensorObj*)p->tc_objs.ptr, (int)obj_base, (int)n_obj_launch);
+        if (kb_bound > 0) {
+            if (c.fast_math)
+                lsp_tensor_table_kernel<float, true><<<(unsigned)kb_bound, kTcMaxNL, 0, st>>>(gq, s.tp, d_off, (const float*)d_t,
+                                                                                          (const TensorObj*)p->tc_objs.ptr, (int)n_obj_launch, (__half*)p->tc_table.ptr);
+            else
+                lsp_tensor_table_kernel<float, false><<<(unsigned)kb_bound, kTcMaxNL, 0, st>>>(gq, s.tp, d_off, (const float*)d_t,
+                                                                                           (const TensorObj*)p->tc_objs.ptr, (int)n_obj_launch, (__half*)p->tc_table.ptr);
+        }
+        LSP_CUDA(p, cudaGetLastError());
+        p->n_launches += 3;
+    }
     GridParams gp;
     gp.f_min = c.f_min;
     gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
@@ -333,17 +400,56 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     }
 
     int n_parts = 0;
+    const size_t es = elem_size(c);
+    const size_t row_bytes = (size_t)c.n_freq * es;
+    // Host copy of the offsets, fetched only when an object range has to be cut by observation count.
+    std::vector<int64_t> off_cache;
+    auto host_offsets = [&]() -> const int64_t* {
+        if (h_off) return h_off;
+        if (off_cache.empty()) {
+            off_cache.resize((size_t)n_obj + 1);
+            if (cudaMemcpyAsync(off_cache.data(), d_off, off_cache.size() * sizeof(int64_t), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaStreamSynchronize(st) != cudaSuccess) {
+                off_cache.clear();
+                return nullptr;
+            }
+        }
+        return off_cache.data();
+    };
     if (!out_power || !out_is_host) {
-        // steps 2-6': one launch over the whole batch, asynchronous on the caller's stream
-        lsp_status e = run_range(p, s, 0, n_obj, d_off, d_t, d_y, out_power, want_best, &n_parts, st);
-        if (e != LSP_OK) return e;
-        if (want_best) return run_finalize(p, 0, n_obj, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
+        // steps 2-6': asynchronous on the caller's stream.  One launch over the whole batch, except on the tensor path
+        // when the B-operand table of the whole batch would exceed its memory budget: then objects go in ranges.
+        const bool cut = s.kernel == LSP_KERNEL_TENSOR &&
+                         (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget;
+        if (!cut) {
+            lsp_status e = run_range(p, s, 0, n_obj, total_obs, d_off, d_t, d_y, out_power, want_best, &n_parts, st);
+            if (e != LSP_OK) return e;
+            if (want_best) return run_finalize(p, 0, n_obj, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
+            return LSP_OK;
+        }
+        const int64_t* ho = host_offsets();
+        if (!ho) return fail(p, LSP_ERR_CUDA, "reading offsets back failed");
+        const int64_t kb_cap = (int64_t)(p->tc_table_budget / (size_t)s.tp.b_stage_bytes);
+        for (int64_t o0 = 0; o0 < n_obj;) {
+            int64_t no = 0, kbs = 0;
+            while (o0 + no < n_obj) {
+                const int64_t k = tc_n_kb(ho[o0 + no + 1] - ho[o0 + no]);
+                if (no > 0 && kbs + k > kb_cap) break;
+                kbs += k;
+                ++no;
+            }
+            Schedule sc = make_schedule(p, no, ho[o0 + no] - ho[o0]);
+            sc.kernel = s.kernel;
+            lsp_status e = run_range(p, sc, o0, no, ho[o0 + no] - ho[o0], d_off, d_t, d_y,
+                                     out_power ? (char*)out_power + (size_t)o0 * row_bytes : nullptr, want_best, &n_parts, st);
+            if (e != LSP_OK) return e;
+            if (want_best && (e = run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+            o0 += no;
+        }
         return LSP_OK;
     }
 
     // ---- step 7: chunked compute -> event -> copy streams -> (pinned) host -------------------
-    const size_t es = elem_size(c);
-    const size_t row_bytes = (size_t)c.n_freq * es;
     const size_t chunk_bytes = c.chunk_bytes > 0 ? (size_t)c.chunk_bytes : ((size_t)64 << 20);
     const int64_t objs_per_chunk = std::max<int64_t>(1, (int64_t)(chunk_bytes / row_bytes));
     const size_t slot_bytes = (size_t)objs_per_chunk * row_bytes;
@@ -360,10 +466,10 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         const int slot = (int)(chunk % n_slots);
         char* dslot = (char*)p->ring.ptr + (size_t)slot * slot_bytes;
         if (p->slot_used[slot]) LSP_CUDA(p, cudaStreamWaitEvent(st, p->slot_free[slot], 0));
-        const int64_t obs_est = total_obs / n_obj * no;
+        const int64_t obs_est = h_off ? (h_off[o0 + no] - h_off[o0]) : total_obs / n_obj * no;
         Schedule sc = make_schedule(p, no, obs_est);
         sc.kernel = s.kernel;
-        lsp_status e = run_range(p, sc, o0, no, d_off, d_t, d_y, dslot, want_best, &n_parts, st);
+        lsp_status e = run_range(p, sc, o0, no, h_off ? obs_est : total_obs, d_off, d_t, d_y, dslot, want_best, &n_parts, st);
         if (e != LSP_OK) return e;
         if (want_best) {
             e = run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
@@ -398,7 +504,9 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     if (cfg->fast_math != 0 && cfg->fast_math != 1) return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math must be 0 or 1");
     if (cfg->fast_math && cfg->dtype == LSP_F64)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math (MUFU sincos) is FP32-only");
-    if (cfg->kernel < LSP_KERNEL_AUTO || cfg->kernel > LSP_KERNEL_FACTORED) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown kernel");
+    if (cfg->kernel < LSP_KERNEL_AUTO || cfg->kernel > LSP_KERNEL_TENSOR) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown kernel");
+    if (cfg->kernel == LSP_KERNEL_TENSOR && cfg->dtype != LSP_F32)
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "the tensor-core kernel is FP32-mode only (FP16-split operands, FP32 accumulation)");
     if (cfg->reserved != 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "reserved must be 0");
     if (cfg->n_copy_streams < 0 || cfg->n_copy_streams > 16 || cfg->chunk_bytes < 0 || cfg->max_objects < 0 || cfg->max_total_obs < 0)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "negative / oversized sizing field");
@@ -433,6 +541,8 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
         return bail(LSP_ERR_UNSUPPORTED);
     }
     p->sm_count = prop.multiProcessorCount;
+    p->smem_optin = (int)prop.sharedMemPerBlockOptin;
+    if (const char* b = getenv("LSP_TABLE_BUDGET_MB")) p->tc_table_budget = (size_t)std::max(1L, atol(b)) << 20;
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
         cudaStream_t s;
@@ -547,7 +657,7 @@ void lsp_destroy(lsp_plan* p)
     for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
-    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
     cudaGetLastError();
@@ -635,7 +745,7 @@ lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, doubl
 
 const char* lsp_version(void)
 {
-    return "lsp-b200 0.1 (sm_100a; kernels: direct, factored-ffma2, factored-dfma)";
+    return "lsp-b200 0.2 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05)";
 }
 
 }  // extern "C"

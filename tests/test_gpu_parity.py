@@ -92,8 +92,10 @@ def test_config1_full_and_best_f64(lsp, oracle, kernel):
 
 # ---- config 2 shape: one long object, large f*t, all precisions and kernels -------------------------------
 @pytest.mark.parametrize("dtype,fast", [("f64", False), ("f32", False), ("f32", True)])
-@pytest.mark.parametrize("kernel", ["direct", "factored"])
+@pytest.mark.parametrize("kernel", ["direct", "factored", "tensor"])
 def test_config2_shape_small(lsp, oracle, dtype, fast, kernel):
+    if kernel == "tensor" and dtype == "f64":
+        pytest.skip("the tensor-core kernel is FP32-mode only")
     # N_t = 1500 spans several observation chunks with a ragged tail; N_f = 9001 spans several tiles with a ragged tail
     w = make_config(2, dtype=dtype, n_t=1500, n_freq=9001)
     P_ref = oracle_full(oracle, w)
@@ -108,7 +110,7 @@ def test_config2_full_size_sampled(lsp, oracle, dtype, fast):
     checks a seeded sample of frequencies plus a window around the peak, and the bounds hold everywhere."""
     w = make_config(2, dtype=dtype)
     P, best, info = gpu_full(lsp, w, fast_math=fast)
-    assert info["kernel"] == "factored"
+    assert info["kernel"] == ("tensor" if dtype == "f32" else "factored")
     rng = np.random.default_rng(22)
     ks = np.unique(np.concatenate([rng.integers(0, w.n_freq, 600), np.arange(0, 64), np.arange(w.n_freq - 64, w.n_freq),
                                    np.clip(np.arange(-100, 101) + int(best[2][0]), 0, w.n_freq - 1)])).astype(np.int64)
@@ -125,7 +127,8 @@ def test_config2_full_size_sampled(lsp, oracle, dtype, fast):
 
 
 # ---- config 3 shape: batch of short night-clustered objects, best period fused ----------------------------
-@pytest.mark.parametrize("kernel,fast", [("factored", False), ("factored", True), ("direct", True)])
+@pytest.mark.parametrize("kernel,fast", [("factored", False), ("factored", True), ("direct", True),
+                                         ("tensor", False), ("tensor", True)])
 def test_config3_shape_best_only(lsp, oracle, kernel, fast):
     w = make_config(3, n_obj=24, n_freq=20_011)
     P_ref = oracle_full(oracle, w)
@@ -143,7 +146,7 @@ def test_config3_full_size_sampled_objects(lsp, oracle):
     a seeded sample of whole objects (so best-period parity is testable)."""
     w = make_config(3)
     best, info = gpu_best(lsp, w, fast_math=True)
-    assert info["kernel"] == "factored" and info["n_split"] == 1
+    assert info["kernel"] == "tensor" and info["n_split"] == 1
     rng = np.random.default_rng(33)
     pick = np.sort(rng.choice(w.n_obj, 12, replace=False))
     sub = w.take_objects(pick)
@@ -187,8 +190,10 @@ def test_config4_shape_host_output_streams(lsp, oracle):
 
 # ---- config 5 shape: large N_t / small N_f -> observation split path ----------------------------------------
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("kernel", ["factored", "direct"])
+@pytest.mark.parametrize("kernel", ["factored", "direct", "tensor"])
 def test_config5_split_path(lsp, oracle, dtype, kernel):
+    if kernel == "tensor" and dtype == "f64":
+        pytest.skip("the tensor-core kernel is FP32-mode only")
     w = make_config(5, dtype=dtype, n_t=16384, n_freq=6000, point=7)
     rng = np.random.default_rng(55)
     P, best, info = gpu_full(lsp, w, kernel=kernel, fast_math=(dtype == "f32"))
@@ -203,8 +208,10 @@ def test_config5_split_path(lsp, oracle, dtype, kernel):
 
 # ---- edge cases ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-@pytest.mark.parametrize("kernel", ["direct", "factored"])
+@pytest.mark.parametrize("kernel", ["direct", "factored", "tensor"])
 def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, kernel):
+    if kernel == "tensor" and dtype == "f64":
+        pytest.skip("the tensor-core kernel is FP32-mode only")
     rng = np.random.default_rng(9)
     lens = [0, 1, 2, 3, 17, 0, 130]
     off = np.zeros(len(lens) + 1, dtype=np.int64)
@@ -234,7 +241,7 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, kernel):
 def test_edge_ragged_grid_sizes(lsp, oracle, n_freq):
     w = make_config(1, n_freq=n_freq, dtype="f32")
     P_ref = oracle_full(oracle, w)
-    for kernel in ("direct", "factored"):
+    for kernel in ("direct", "factored", "tensor"):
         P, best, _ = gpu_full(lsp, w, kernel=kernel)
         assert_power_parity(P, P_ref, "f32", f"nf={n_freq}/{kernel}")
         assert_best_parity(best, P_ref, w, "f32", oracle)
