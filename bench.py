@@ -37,6 +37,44 @@ SM_MAX_HZ = 1965e6
 FP32_LANES = 128      # FP32 FMA lanes per SM per clock
 FP64_LANES = 64       # FP64 FMA lanes per SM per clock
 FLOP_PER_PAIR = 8.0   # factored formulation: 4 FMA per (t,f) pair ("4 FMA = 8 flop/pair")
+# Tensor path: the same 4 MAC per pair as one FP16 GEMM; the accurate mode issues three products per MAC
+# (a_hi b_hi + a_hi b_lo + a_lo b_hi), fast_math one.
+TENSOR_PRODUCTS = {False: 3, True: 1}
+TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 burst; fp16 : bf16 nominal ratio is 1)
+
+
+def measured_tensor_peak():
+    """(TFLOP/s, provenance) -- the driver-written cuBLAS bf16 burst figure; FP16 runs at the same nominal rate."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["bf16_tflops"]), "of measured (MEASURED_PEAKS.json bf16_tflops, burst; fp16:bf16 = 1)"
+    except Exception:
+        return TENSOR_PEAK_FALLBACK, "of fallback (B200_PROFILING.md 1.59 PFLOP/s bf16 burst; fp16:bf16 = 1)"
+
+
+def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float):
+    """Roofline object of the dominant kernel: achieved = algorithmic flop per launch
+    (8 flop per (t,f) pair x pairs) / mean launch duration measured with CUDA events on the launching stream."""
+    achieved = pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
+    if kernel == "tensor":
+        peak, prov = measured_tensor_peak()
+        prod = TENSOR_PRODUCTS[bool(fast)]
+        return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
+                "peak_is": prov,
+                "executed_flop_per_pair": FLOP_PER_PAIR * prod,
+                "executed_tflops": achieved * prod, "frac_executed": achieved * prod / peak,
+                "note": "FP16 hi+lo split operands: %d tcgen05 products per algorithmic MAC" % prod}
+    lanes = FP32_LANES if dtype == "f32" else FP64_LANES
+    peak = N_SM * lanes * 2 * SM_MAX_HZ / 1e12
+    if kernel != "factored":       # direct kernel (tiny grids): XU/issue bound, no flop roofline claimed
+        return {"bound": "alu", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
+                "kernel": "lsp_direct_kernel", "flop_per_pair": None}
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+            "kernel": "lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double"),
+            "flop_per_pair": FLOP_PER_PAIR,
+            "peak_is": "derived: 148 SMs x %d %s FMA lanes/clk/SM x 2 flop x 1965 MHz (clocks.max.sm)" % (lanes, "FP32" if dtype == "f32" else "FP64"),
+            "pipe_peak_measured": pipe_ops * 2 / 1e12, "frac_of_measured_pipe": achieved / (pipe_ops * 2 / 1e12)}
 
 
 def parse_args():
@@ -69,7 +107,7 @@ class ClockSampler:
     BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "hw_power_brake": 0x80}
     NOTE = {"sw_power_cap": 0x4}
 
-    def __init__(self, index: int, period_s: float = 0.02):
+    def __init__(self, index: int, period_s: float = 0.002):
         self.samples, self.reasons = [], set()
         self.period, self.stop_flag, self.thread, self.ok = period_s, threading.Event(), None, False
         try:
@@ -292,9 +330,12 @@ def timed_loop(torch, dist, world, leg, step, steps: int, warmup: int, flush):
     return total_ms, info
 
 
-def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_clocks: bool):
+def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_clocks: bool, kernel=None, fast=None,
+            with_e2e: bool = True):
     w = workload_for(args.workload, dtype, rank)
-    leg = Leg(pkg, torch, w, args.workload, dtype, args.fast_math, args.kernel, device)
+    kernel = args.kernel if kernel is None else kernel
+    fast = bool(args.fast_math if fast is None else fast) and dtype == "f32"
+    leg = Leg(pkg, torch, w, args.workload, dtype, fast, kernel, device)
     pairs_step = w.pairs
     pairs_all = pairs_step
     if world > 1:
@@ -305,40 +346,28 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     if sampler:
         sampler.__enter__()
     total_ms, info = timed_loop(torch, dist, world, leg, leg.step_device, args.steps, args.warmup, flush)
-    if sampler:
-        sampler.__exit__()
     dev_launches, kernel_ms = leg.launches, list(leg.kernel_ms)
     leg.launches, leg.kernel_ms = 0, []
-    e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, args.steps, args.warmup, flush)
-    h2d, d2h = leg.e2e_bytes()
     ms_step = total_ms / args.steps
     k_ms = sum(kernel_ms) / len(kernel_ms)
-    lanes = FP32_LANES if dtype == "f32" else FP64_LANES
-    peak_tflops = N_SM * lanes * 2 * SM_MAX_HZ / 1e12
-    factored = info["kernel"] == "factored"
-    flop_pair = FLOP_PER_PAIR if factored else None
-    achieved = (pairs_step * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12) if factored else None
     # measured pipe peak with the same clocks the kernels see (register-only FFMA2 / DFMA loops, lsp_pipe_peak)
     pipe_ops, _ = pkg.lsp_pipe_peak(1 if dtype == "f32" else 2, device)
     out = {
         "dtype": dtype,
         "value": pairs_all * args.steps / (total_ms * 1e-3),
         "ms_per_step": ms_step,
-        "kernel": info["kernel"], "n_split": info["n_split"],
+        "kernel": info["kernel"], "n_split": info["n_split"], "fast_math": fast,
         "kernel_ms_per_step": k_ms,
         "gpu_launches": dev_launches,
-        "e2e": {"value": pairs_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps},
-        "roofline": {
-            "bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-            "frac": (achieved / peak_tflops) if achieved else None, "traffic": None,
-            "kernel": ("lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double")) if factored else "lsp_direct_kernel",
-            "flop_per_pair": flop_pair,
-            "peak_is": "derived: 148 SMs x %d %s FMA lanes/clk/SM x 2 flop x 1965 MHz (clocks.max.sm)" % (lanes, "FP32" if dtype == "f32" else "FP64"),
-            "pipe_peak_measured": pipe_ops * 2 / 1e12,
-            "frac_of_measured_pipe": (achieved / (pipe_ops * 2 / 1e12)) if achieved else None,
-        },
+        "roofline": roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops),
     }
+    if with_e2e:
+        e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, args.steps, args.warmup, flush)
+        h2d, d2h = leg.e2e_bytes()
+        out["e2e"] = {"value": pairs_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                      "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps}
+    if sampler:
+        sampler.__exit__()
     if sampler:
         out["clocks"] = sampler.summary()
     leg.plan.destroy()
@@ -363,9 +392,17 @@ def run_b200(args, rank: int, world: int, local_rank: int):
 
     primary, w = run_leg(args, pkg, torch, dist, rank, world, local_rank, args.dtype, flush, True)
     other = None
+    variants = {}
     if not args.no_secondary and args.workload == "c2":
         other_dtype = "f64" if args.dtype == "f32" else "f32"
         other, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, other_dtype, flush, False)
+        if args.kernel == "auto" and not args.fast_math:
+            # the other FP32 formulations on the same workload (device-resident only): the FFMA2 contraction on the
+            # FMA pipe (north_star's "FP32 issue-bound roofline") and the fast_math tensor mode
+            variants["fp32_fma_pipe"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
+                                                   kernel="factored", fast=False, with_e2e=False)
+            variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
+                                                    kernel="auto", fast=True, with_e2e=False)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w, args.cpu_seconds)
@@ -386,6 +423,8 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             line[other["dtype"] == "f64" and "fp64" or "fp32"] = {k: other[k] for k in
                                                                  ("value", "ms_per_step", "kernel_ms_per_step", "e2e", "roofline",
                                                                   "gpu_launches", "kernel")}
+        for name, v in variants.items():
+            line[name] = {k: v[k] for k in ("value", "ms_per_step", "kernel_ms_per_step", "roofline", "gpu_launches", "kernel")}
         if cpu is not None:
             line["cpu_baseline"] = cpu
         print(json.dumps(line), flush=True)
