@@ -24,8 +24,9 @@
 //   B operands  e^{i beta}, e^{2 i beta} depend on (object, observation, m) only -- not on the tile -- so a pre-pass
 //               (lsp_tensor_table_kernel) writes them once per object into a table already laid out as shared-memory
 //               stages; warp 0 streams the stages in with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx).
-//   A operands  depend on the tile: warps 12-19 generate them (FP64 phase -> sincos -> scale by y -> FP16 hi/lo) straight
-//               into the stage ring (st.shared + fence.proxy.async).
+//   A operands  depend on the tile: warps 12-19 generate them straight into the stage ring (st.shared +
+//               fence.proxy.async): one sincos per thread per stage (two-float FP32 phase), then the 64 x 16 operands as
+//               phasor products e^{i alpha_g} = u_{g mod 8} v_{g div 8} on the FMA pipe, scaled by y, split into FP16 hi/lo.
 //   warp 1      one thread issues the MMAs of a stage when its mbarrier completes, and tcgen05.commit releases the
 //               stage / publishes the finished accumulators.
 //   warps 4-11  epilogue: tcgen05.ld the accumulators, combine rows with a shuffle, closed-form power (step 5),
@@ -40,10 +41,13 @@ namespace lsp {
 constexpr int kTcGroups = 64;                  // frequency groups per tile (128 MMA rows)
 constexpr int kTcKB = 16;                      // observations per MMA / ring stage (kind::f16: K = 16)
 constexpr int kTcMaxNL = 128;                  // N = 2 NL <= 256
-constexpr int kTcGenWarps = 8, kTcEpiWarps = 8;
-constexpr int kTcThreads = (4 + kTcEpiWarps + kTcGenWarps) * 32;      // 640
-constexpr int kTcGenThreads = kTcGenWarps * 32;
+constexpr int kTcGenWarps = 16, kTcEpiWarps = 8;                      // generators: two groups of 8 warps
+constexpr int kTcThreads = (4 + kTcEpiWarps + kTcGenWarps) * 32;      // 896: 72 registers per thread at launch
+constexpr int kTcGenGroupThreads = 256;                               // threads that build one ring stage
+// register split (setmaxnreg, per 4-warp group): 128 x 40 + 256 x 120 + 512 x 56 = 64512 = 896 x 72
+constexpr int kTcCtrlRegs = 40, kTcEpiRegs = 120, kTcGenRegs = 56;
 constexpr int kTcEpiThreads = kTcEpiWarps * 32;
+constexpr int kTcScratchQuad = 16 * 4 + 2;   // float2 per observation quad of the generator scratch (+16 B: conflict-free LDS.128)
 constexpr float kTcUnitScale = 256.0f;         // scale of the unit-modulus A_W operands (keeps the FP16 low part normal)
 
 struct TensorParams {
@@ -243,6 +247,12 @@ __device__ __forceinline__ void tc_commit(unsigned long long* bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ bool elect_one()
+{
+    unsigned pred;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_ld16(unsigned taddr, float* v)
@@ -315,11 +325,14 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
     __shared__ Best sbest[kTcEpiWarps];
+    __shared__ __align__(16) float2 s_uv[2][2][4 * kTcScratchQuad];  // generator scratch: [group][buffer][j/4][phasor q][j%4], padded
+    __shared__ __align__(16) float s_yv[2][2][kTcKB];                // scaled, centred y of the stage
 
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // broadcast: the compiler may treat the role as warp-uniform
     if (tid == 0) {
         for (int s = 0; s < S; ++s) {
-            mbar_init(&full[s], kTcGenThreads + 1);
+            mbar_init(&full[s], kTcGenGroupThreads + 1);
             mbar_init(&empty[s], 1);
         }
         mbar_init(tmem_full, 1);
@@ -335,64 +348,88 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     tc_fence_after();
     const unsigned tmem = tmem_base_s;
 
+    if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcCtrlRegs));
     if (warp == 0) {
         // =============================== TMA producer: B stages from the per-object table ========================
         if (lane == 0) {
-            unsigned c = 0;
+            int st = 0;
+            unsigned ph = 1;                                      // parity of the "empty" phase to wait for
+            const unsigned b_bytes = (unsigned)tp.b_stage_bytes;
+            unsigned char* dst0 = smem + tp.a_stage_bytes;
             for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
                 const TcItem w = tc_decode(gp, tp, item, offsets);
-                const __half* src = table + (size_t)(objs[w.obj_local].kb_off + w.kb0) * (size_t)(tp.b_stage_bytes / 2);
-                for (int kb = w.kb0; kb < w.kb1; ++kb, ++c) {
-                    const int s = c % S;
-                    mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
-                    mbar_arrive_expect_tx(&full[s], (unsigned)tp.b_stage_bytes);
-                    tma_bulk_g2s(smem + (size_t)s * stage_bytes + tp.a_stage_bytes, src, (unsigned)tp.b_stage_bytes, &full[s]);
-                    src += tp.b_stage_bytes / 2;
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(table) +
+                                           (size_t)(objs[w.obj_local].kb_off + w.kb0) * (size_t)b_bytes;
+                for (int kb = w.kb0; kb < w.kb1; ++kb) {
+                    mbar_wait(&empty[st], ph);
+                    mbar_arrive_expect_tx(&full[st], b_bytes);
+                    tma_bulk_g2s(dst0 + (size_t)st * stage_bytes, src, b_bytes, &full[st]);
+                    src += b_bytes;
+                    if (++st == S) { st = 0; ph ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
         // =============================== MMA issuer ===============================================================
-        if (lane == 0) {
+        // The whole warp runs the loop with warp-uniform values (item ranges are broadcast from lane 0), so descriptors
+        // and barrier addresses live in uniform registers; one elected lane issues the MMAs and commits.
+        {
             const unsigned idesc = (1u << 4) | ((unsigned)((2 * tp.nl) >> 3) << 17) | ((unsigned)(128 >> 4) << 24);
             const unsigned a_lbo = 16 * 128, b_lbo = (unsigned)(2 * tp.nl / 8) * 128, sbo = 128;
-            unsigned c = 0, n_acc = 0;
+            // Descriptors of stage 0; stage s adds s * stage_bytes / 16 to the 14-bit start-address field (the whole ring
+            // lies below 256 KB, so the field never carries into the LBO bits).
+            const unsigned sa0 = smem_u32(smem), sb0 = sa0 + tp.a_stage_bytes;
+            const uint64_t a_zh0 = tc_smem_desc(sa0, a_lbo, sbo), a_wh0 = tc_smem_desc(sa0 + A_PLANE, a_lbo, sbo);
+            const uint64_t a_zl0 = tc_smem_desc(sa0 + 2 * A_PLANE, a_lbo, sbo), a_wl0 = tc_smem_desc(sa0 + 3 * A_PLANE, a_lbo, sbo);
+            const uint64_t b_zh0 = tc_smem_desc(sb0, b_lbo, sbo), b_wh0 = tc_smem_desc(sb0 + b_plane, b_lbo, sbo);
+            const uint64_t b_zl0 = tc_smem_desc(sb0 + 2 * b_plane, b_lbo, sbo), b_wl0 = tc_smem_desc(sb0 + 3 * b_plane, b_lbo, sbo);
+            const uint64_t stage_inc = (uint64_t)(stage_bytes >> 4);
+            int st = 0;
+            unsigned ph = 0, n_acc = 0;
+            uint64_t so = 0;                                      // st * stage_inc
             for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
                 const TcItem w = tc_decode(gp, tp, item, offsets);
-                if (w.kb1 <= w.kb0) continue;
+                const int kb0 = __shfl_sync(0xffffffffu, w.kb0, 0), kb1 = __shfl_sync(0xffffffffu, w.kb1, 0);
+                if (kb1 <= kb0) continue;
                 mbar_wait(tmem_empty, (n_acc & 1) ^ 1);          // the epilogue has drained the previous accumulators
                 tc_fence_after();
-                for (int kb = w.kb0; kb < w.kb1; ++kb, ++c) {
-                    const int s = c % S;
-                    mbar_wait(&full[s], (c / S) & 1);
+                unsigned acc = 0;
+                for (int kb = kb0; kb < kb1; ++kb) {
+                    mbar_wait(&full[st], ph);
                     tc_fence_after();
-                    const unsigned sa = smem_u32(smem + (size_t)s * stage_bytes);
-                    const unsigned sb = sa + tp.a_stage_bytes;
-                    const unsigned acc = kb > w.kb0;
-                    // planes: 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
-                    const uint64_t a_zh = tc_smem_desc(sa, a_lbo, sbo), a_wh = tc_smem_desc(sa + A_PLANE, a_lbo, sbo);
-                    const uint64_t b_zh = tc_smem_desc(sb, b_lbo, sbo), b_wh = tc_smem_desc(sb + b_plane, b_lbo, sbo);
-                    if (!FAST) {
-                        const uint64_t a_zl = tc_smem_desc(sa + 2 * A_PLANE, a_lbo, sbo), a_wl = tc_smem_desc(sa + 3 * A_PLANE, a_lbo, sbo);
-                        const uint64_t b_zl = tc_smem_desc(sb + 2 * b_plane, b_lbo, sbo), b_wl = tc_smem_desc(sb + 3 * b_plane, b_lbo, sbo);
-                        tc_mma_f16(tmem, a_zl, b_zh, idesc, acc);
-                        tc_mma_f16(tmem, a_zh, b_zl, idesc, 1u);
-                        tc_mma_f16(tmem, a_zh, b_zh, idesc, 1u);
-                        tc_mma_f16(tmem + 256, a_wl, b_wh, idesc, acc);
-                        tc_mma_f16(tmem + 256, a_wh, b_wl, idesc, 1u);
-                        tc_mma_f16(tmem + 256, a_wh, b_wh, idesc, 1u);
-                    } else {
-                        tc_mma_f16(tmem, a_zh, b_zh, idesc, acc);
-                        tc_mma_f16(tmem + 256, a_wh, b_wh, idesc, acc);
+                    if (elect_one()) {
+                        // planes: 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
+                        if (!FAST) {
+                            tc_mma_f16(tmem, a_zl0 + so, b_zh0 + so, idesc, acc);
+                            tc_mma_f16(tmem, a_zh0 + so, b_zl0 + so, idesc, 1u);
+                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + so, idesc, 1u);
+                            tc_mma_f16(tmem + 256, a_wl0 + so, b_wh0 + so, idesc, acc);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wl0 + so, idesc, 1u);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + so, idesc, 1u);
+                        } else {
+                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + so, idesc, acc);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + so, idesc, acc);
+                        }
+                        tc_commit(&empty[st]);                   // stage st is free once these MMAs have read it
                     }
-                    tc_commit(&empty[s]);                        // stage s is free once these MMAs have read it
+                    __syncwarp();
+                    acc = 1u;
+                    so += stage_inc;
+                    if (++st == S) { st = 0; ph ^= 1; so = 0; }
                 }
-                tc_commit(tmem_full);                            // accumulators complete
+                if (elect_one()) tc_commit(tmem_full);           // accumulators complete
+                __syncwarp();
                 ++n_acc;
             }
         }
     } else if (warp >= 4 && warp < 4 + kTcEpiWarps) {
         // =============================== epilogue (steps 5, 6, 6') ================================================
+        // Lane l of quadrant q holds row 32 q + l: lanes 0-15 the "Re a" rows (Srr, Sri) of groups 16 q + l, lanes 16-31
+        // the "Im a" rows (Sir, Sii) of the same groups.  One shuffle per accumulator pairs them; the Re lane then owns
+        // the frequency above the group centre (k = c + m), the Im lane the one below (k = c - 1 - m), so all 32 lanes
+        // produce distinct powers.  Indices are tile-local 32-bit integers; the argmax runs in FP32 + int and is widened
+        // once per item; bounds are only checked on the grid's ragged last tile.
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTcEpiRegs));
         const int ew = warp - 4;
         const int q = warp & 3;                                   // TMEM lane quadrant this warp may access
         const int half_sel = ew >> 2;                             // which half of the m range
@@ -400,9 +437,10 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         const bool is_im = lane >= 16;
         const int g = 16 * q + (lane & 15);
         const int NL = tp.nl, L = 2 * NL;
-        const int n_chunks = NL / 16 + ((NL % 16) ? 1 : 0);       // 16-column chunks over m (NL is a multiple of 8)
+        const int n_chunks = (NL + 15) >> 4;                      // 16-column chunks over m (NL is a multiple of 8)
         const int ch0 = (n_chunks * half_sel) / 2, ch1 = (n_chunks * (half_sel + 1)) / 2;
         const bool vec_ok = (gp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(out_power) & 15) == 0);
+        const int kc = g * L + NL;                                // tile-local index of the first frequency above the centre
         unsigned n_acc = 0;
         for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
             const TcItem w = tc_decode(gp, tp, item, offsets);
@@ -412,87 +450,103 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 mbar_wait(tmem_full, n_acc & 1);
                 tc_fence_after();
             }
-            Best mine;
-            mine.p = -1.0;
-            mine.k = INT64_MAX;
+            float bp = -1.0f;                                     // running maximum (P >= 0; NaN never compares greater)
+            int bk = 0x7fffffff;
             const float n_hat = kTcUnitScale * (float)w.n_t;
-            T* orow = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq : nullptr;
+            const int n_valid = (int)min((int64_t)tp.tile, (int64_t)gp.n_freq - w.K0);     // frequencies of this tile on the grid
+            const bool ragged = n_valid < tp.tile;
+            T* otile = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq + w.K0 : nullptr;
+            float4* stile = (gp.n_split > 1) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
+            const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
+            bool released = false;
             for (int ch = ch0; ch < ch1; ++ch) {
                 const int m0 = ch * 16;
                 float zr[16], zi[16], wr[16], wi[16];
                 if (have) {
-                    const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
                     tc_ld16(ta + 256 + m0, wr);
                     tc_ld16(ta + 256 + NL + m0, wi);
                     tc_ld_wait();
+                    if (ch == ch1 - 1) {                          // last TMEM read of this warp: the MMA warp may overwrite
+                        tc_fence_before();
+                        mbar_arrive(tmem_empty);
+                        released = true;
+                    }
                 } else {
 #pragma unroll
                     for (int i = 0; i < 16; ++i) zr[i] = zi[i] = wr[i] = wi[i] = 0.f;
                 }
-                float pw[16];
-                const int m_lim = NL - m0;                               // valid i < m_lim (last chunk when NL % 16 == 8)
-                const int64_t kbase = w.K0 + (int64_t)g * L + NL;
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    // rows "Re a": (Srr, Sri); rows "Im a": (Sir, Sii); partner lane (xor 16) holds the other row
-                    const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
-                    const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
-                    const float dz = is_im ? (p0 + zi[i]) : (zr[i] - p1);      // down: Srr + Sii ; up: Srr - Sii
-                    const float ez = is_im ? (zr[i] - p1) : (zi[i] + p0);      // down: Sir - Sri ; up: Sri + Sir
-                    const float dw = is_im ? (q0 + wi[i]) : (wr[i] - q1);
-                    const float ew2 = is_im ? (wr[i] - q1) : (wi[i] + q0);
-                    // up lanes own k = c + m (ascending in i), down lanes k = c - 1 - m (descending in i)
-                    if (gp.n_split > 1) {       // split-N_t: un-scaled partial sums for lsp_combine_kernel
-                        const int64_t k = is_im ? (kbase - 1 - (m0 + i)) : (kbase + m0 + i);
-                        if (i < m_lim && k < gp.n_freq)
-                            sums[((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + k] =
-                                make_float4(dz * ob.zinv, ez * ob.zinv, dw * (1.0f / kTcUnitScale), ew2 * (1.0f / kTcUnitScale));
-                    } else {
-                        pw[i] = power_from_sums<float>(dz, ez, dw, ew2, n_hat, ob.pscale);
-                    }
-                }
-                if (gp.n_split > 1) continue;
+                const int i_lim = min(16, NL - m0);               // 16, or 8 in the last chunk when NL % 16 == 8
+                // tile-local index of element i: up lanes kc + m0 + i, down lanes kc - 1 - m0 - i
+                const int kl0 = is_im ? (kc - 1 - m0) : (kc + m0);
 #pragma unroll
                 for (int v4 = 0; v4 < 4; ++v4) {
-                    if (v4 * 4 >= m_lim) break;
-                    // element e of this vector: up -> i = 4 v4 + e ; down -> i = 4 v4 + 3 - e
-                    const int64_t k0 = is_im ? (kbase - 1 - (m0 + 4 * v4 + 3)) : (kbase + m0 + 4 * v4);
-                    {
-                        const float e0 = is_im ? pw[4 * v4 + 3] : pw[4 * v4], e1 = is_im ? pw[4 * v4 + 2] : pw[4 * v4 + 1];
-                        const float e2 = is_im ? pw[4 * v4 + 1] : pw[4 * v4 + 2], e3 = is_im ? pw[4 * v4] : pw[4 * v4 + 3];
-                        if (orow) {
-                            if (vec_ok && k0 + 3 < gp.n_freq) {
-                                *reinterpret_cast<float4*>(orow + k0) = make_float4(e0, e1, e2, e3);
+                    if (4 * v4 >= i_lim) break;
+                    float pw[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int i = 4 * v4 + e;
+                        // partner lane (xor 16) holds the other row of the same group
+                        const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
+                        const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
+                        // Re lane: (zr, zi) = (Srr, Sri), (p0, p1) = (Sir, Sii): up   Z = (Srr - Sii) + i (Sri + Sir)
+                        // Im lane: (zr, zi) = (Sir, Sii), (p0, p1) = (Srr, Sri): down Z = (Srr + Sii) + i (Sir - Sri)
+                        const float za = zr[i] - p1, zb = zi[i] + p0;
+                        const float wa = wr[i] - q1, wb = wi[i] + q0;
+                        const float xc = is_im ? zb : za, xs = is_im ? za : zb;
+                        const float c2 = is_im ? wb : wa, s2 = is_im ? wa : wb;
+                        if (stile) {                   // split-N_t: un-scaled partial sums for lsp_combine_kernel
+                            const int kl = is_im ? kl0 - i : kl0 + i;
+                            if (kl < n_valid)
+                                stile[kl] = make_float4(xc * ob.zinv, xs * ob.zinv, c2 * (1.0f / kTcUnitScale), s2 * (1.0f / kTcUnitScale));
+                        } else {
+                            pw[e] = power_from_sums<float>(xc, xs, c2, s2, n_hat, ob.pscale);
+                        }
+                    }
+                    if (stile) continue;
+                    // element e of the 4-vector in ascending frequency: up -> pw[e], down -> pw[3 - e]
+                    const int klv = is_im ? (kl0 - 4 * v4 - 3) : (kl0 + 4 * v4);
+                    const float e0 = is_im ? pw[3] : pw[0], e1 = is_im ? pw[2] : pw[1];
+                    const float e2 = is_im ? pw[1] : pw[2], e3 = is_im ? pw[0] : pw[3];
+                    if (!ragged) {
+                        if (otile) {
+                            if (vec_ok) {
+                                *reinterpret_cast<float4*>(otile + klv) = make_float4(e0, e1, e2, e3);
                             } else {
-                                if (k0 < gp.n_freq) orow[k0] = (T)e0;
-                                if (k0 + 1 < gp.n_freq) orow[k0 + 1] = (T)e1;
-                                if (k0 + 2 < gp.n_freq) orow[k0 + 2] = (T)e2;
-                                if (k0 + 3 < gp.n_freq) orow[k0 + 3] = (T)e3;
+                                otile[klv] = (T)e0; otile[klv + 1] = (T)e1; otile[klv + 2] = (T)e2; otile[klv + 3] = (T)e3;
                             }
                         }
                         if (partials) {
-                            const float ev[4] = {e0, e1, e2, e3};
+                            if (e0 > bp || (e0 == bp && klv < bk)) { bp = e0; bk = klv; }
+                            if (e1 > bp || (e1 == bp && klv + 1 < bk)) { bp = e1; bk = klv + 1; }
+                            if (e2 > bp || (e2 == bp && klv + 2 < bk)) { bp = e2; bk = klv + 2; }
+                            if (e3 > bp || (e3 == bp && klv + 3 < bk)) { bp = e3; bk = klv + 3; }
+                        }
+                    } else {
+                        const float ev[4] = {e0, e1, e2, e3};
 #pragma unroll
-                            for (int e = 0; e < 4; ++e) {
-                                if (k0 + e < gp.n_freq) {
-                                    Best b;
-                                    b.p = (ev[e] == ev[e]) ? (double)ev[e] : -1.0;
-                                    b.k = k0 + e;
-                                    mine = best_of(mine, b);
-                                }
+                        for (int e = 0; e < 4; ++e) {
+                            const int kl = klv + e;
+                            if (kl < n_valid) {
+                                if (otile) otile[kl] = (T)ev[e];
+                                if (partials && (ev[e] > bp || (ev[e] == bp && kl < bk))) { bp = ev[e]; bk = kl; }
                             }
                         }
                     }
                 }
             }
             if (have) {
-                tc_fence_before();
-                mbar_arrive(tmem_empty);                          // 256 arrivals: TMEM may be overwritten
+                if (!released) {                                  // a warp without chunks (NL <= 16) still signs off
+                    tc_fence_before();
+                    mbar_arrive(tmem_empty);
+                }
                 ++n_acc;
             }
             if (partials && gp.n_split == 1) {
+                Best mine;
+                mine.p = (double)bp;
+                mine.k = (bk == 0x7fffffff) ? INT64_MAX : w.K0 + (int64_t)bk;
                 mine = warp_best(mine);
                 if (lane == 0) sbest[ew] = mine;
                 named_bar_sync(3, kTcEpiThreads);
@@ -509,63 +563,147 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         }
     } else if (warp >= 4 + kTcEpiWarps) {
         // =============================== A-operand generators (steps 2-3) ==========================================
-        const int gw = warp - 4 - kTcEpiWarps;                    // 0..7
-        const int qb = gw & 3, c = gw >> 2;                       // row block (16 groups) and k chunk of this warp
+        // a_gj = y_j e^{i alpha_gj}, alpha_gj = 2 pi f(c_g) t_j, g = 8 g1 + g0.  Since f(c_g) = f(c_g0) + g1 (8 L df),
+        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}
+        // so a stage (16 observations) needs 16 x 16 sincos -- ONE per thread of a generator group (phase 1, into a
+        // small shared-memory scratch) -- instead of 64 x 16; phase 2 forms the 64 x 16 products on the FMA pipe, splits
+        // them into FP16 hi/lo and writes the UMMA operand planes.  Phases are FP32 two-float products (f = f_hi + f_lo,
+        // exact f_hi t through fma, reduced to (-1/2, 1/2] cycles before the low terms are added): no FP64 in the loop.
+        // Two groups of 8 warps take alternate ring stages, so one group's latencies (sincos chain, group barrier,
+        // LDS, mbarrier wait, proxy fence) are covered by the other group's instructions on the same schedulers.
+        // t / y of a group's NEXT stage (of this or a later work item) are loaded before its current stage is processed.
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcGenRegs));
+        const int gw = warp - (4 + kTcEpiWarps);                  // 0..15
+        const int grp = gw >> 3;                                  // generator group: stages with (stage number & 1) == grp
+        const int gw8 = gw & 7;
+        const int gtid = (tid - (4 + kTcEpiWarps) * 32) & (kTcGenGroupThreads - 1);      // 0..255 inside the group
+        // phase 1 role: phasor q (0-7: u_g0, 8-15: v_g1) of observation j1 of the stage
+        const int q1 = gtid >> 4, j1 = gtid & 15;
+        const int sc_w = (j1 >> 2) * kTcScratchQuad + q1 * 4 + (j1 & 3);
+        // phase 2 role: 16-group row block qb, k chunk c, group g, observations 4 hsel .. 4 hsel + 3 of the chunk
+        const int qb = gw8 & 3, c = gw8 >> 2;
         const int g = 16 * qb + (lane >> 1);
-        const int hsel = lane & 1;                                // observations 4 hsel .. 4 hsel + 3 of the chunk
+        const int hsel = lane & 1;
         const int row_re = 32 * qb + (lane >> 1), row_im = row_re + 16;
-        // byte offset of this thread's 8-byte slot inside an A plane: chunk c, row r, k%8 = 4 hsel
         const int off_re = c * (16 * 128) + (row_re >> 3) * 128 + (row_re & 7) * 16 + hsel * 8;
         const int off_im = c * (16 * 128) + (row_im >> 3) * 128 + (row_im & 7) * 16 + hsel * 8;
+        const int sc_u = (2 * c + hsel) * kTcScratchQuad + (g & 7) * 4;
+        const int sc_v = (2 * c + hsel) * kTcScratchQuad + (8 + (g >> 3)) * 4;
         const int NL = tp.nl, L = 2 * NL;
-        unsigned cnt = 0;
-        for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
-            const TcItem w = tc_decode(gp, tp, item, offsets);
-            const TensorObj ob = objs[w.obj_local];
-            const float mean = (float)ob.mean;
-            const double f_centre = gp.f_min + ((double)(w.K0 + (int64_t)g * L + NL) - 0.5) * gp.df;
-            for (int kb = w.kb0; kb < w.kb1; ++kb, ++cnt) {
-                const int64_t jb = (int64_t)kb * kTcKB + 8 * c + 4 * hsel;
-                float tj[4], yj[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const bool live = (jb + i) < w.n_t;
-                    tj[i] = live ? (float)t[w.lo + jb + i] : 0.f;
-                    yj[i] = live ? ((float)y[w.lo + jb + i] - mean) * ob.yscale : 0.f;
-                }
-                float ar[4], ai[4], a2r[4], a2i[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const bool live = (jb + i) < w.n_t;
-                    float sn, cs;
-                    sincos_cycles<FAST>((float)frac_cycles(f_centre * (double)tj[i]), &sn, &cs);
-                    ar[i] = yj[i] * cs;
-                    ai[i] = yj[i] * sn;
-                    const float u = live ? kTcUnitScale : 0.f;
-                    a2r[i] = u * fmaf(cs, cs, -sn * sn);
-                    a2i[i] = u * (2.f * cs * sn);
-                }
-                const int s = cnt % S;
-                mbar_wait(&empty[s], ((cnt / S) & 1) ^ 1);
-                unsigned char* sa = smem + (size_t)s * stage_bytes;
-                auto put = [&](int plane, int off, __half2 v0, __half2 v1) {
-                    uint2 u;
-                    u.x = *reinterpret_cast<unsigned*>(&v0);
-                    u.y = *reinterpret_cast<unsigned*>(&v1);
-                    *reinterpret_cast<uint2*>(sa + plane * A_PLANE + off) = u;
-                };
-                __half2 h0, h1, l0, l1;
-                split_half2(ar[0], ar[1], &h0, &l0);  split_half2(ar[2], ar[3], &h1, &l1);
-                put(0, off_re, h0, h1);  if (!FAST) put(2, off_re, l0, l1);
-                split_half2(ai[0], ai[1], &h0, &l0);  split_half2(ai[2], ai[3], &h1, &l1);
-                put(0, off_im, h0, h1);  if (!FAST) put(2, off_im, l0, l1);
-                split_half2(a2r[0], a2r[1], &h0, &l0);  split_half2(a2r[2], a2r[3], &h1, &l1);
-                put(1, off_re, h0, h1);  if (!FAST) put(NOPS - 1, off_re, l0, l1);
-                split_half2(a2i[0], a2i[1], &h0, &l0);  split_half2(a2i[2], a2i[3], &h1, &l1);
-                put(1, off_im, h0, h1);  if (!FAST) put(NOPS - 1, off_im, l0, l1);
-                fence_proxy_async();            // generic-proxy stores -> visible to the tensor core's async proxy
-                mbar_arrive(&full[s]);
+        const double fv = (q1 >= 8) ? (double)(8 * (q1 - 8)) * (double)L * gp.df : 0.0;      // v: the same for every item
+
+        // A cursor walks the CTA's stage sequence (items in round-robin order, 16-observation blocks inside an item).
+        struct Cursor {
+            long long item;
+            int64_t lo;           // first observation of the object
+            int n_t, kb, kb1;
+            float f_hi, f_lo, mean, yscale;
+        };
+        auto load_item = [&](Cursor& cu) {        // cu.item is set; fills the rest; returns false if the item has no stages
+            const TcItem w = tc_decode(gp, tp, cu.item, offsets);
+            cu.lo = w.lo;
+            cu.n_t = (int)w.n_t;
+            cu.kb = w.kb0;
+            cu.kb1 = w.kb1;
+            const double fd = (q1 < 8) ? gp.f_min + ((double)(w.K0 + (int64_t)q1 * L + NL) - 0.5) * gp.df : fv;
+            cu.f_hi = (float)fd;
+            cu.f_lo = (float)(fd - (double)cu.f_hi);
+            cu.mean = (float)objs[w.obj_local].mean;
+            cu.yscale = objs[w.obj_local].yscale;
+            return w.kb1 > w.kb0;
+        };
+        auto seek = [&](Cursor& cu) {             // first item at or after cu.item that has stages
+            while (cu.item < total_items && !load_item(cu)) cu.item += gridDim.x;
+        };
+        auto step = [&](Cursor& cu) {
+            if (++cu.kb >= cu.kb1) {
+                cu.item += gridDim.x;
+                seek(cu);
             }
+        };
+        Cursor cur;
+        cur.item = blockIdx.x;
+        seek(cur);
+        if (grp == 1 && cur.item < total_items) step(cur);
+        int st = grp;                                             // ring slot of this group's current stage
+        unsigned eph = 1;                                         // parity of the "empty" phase to wait for
+        if (st >= S) { st -= S; eph ^= 1; }
+        unsigned it = 0;
+        float t_cur = 0.f, y_cur = 0.f;
+        if (cur.item < total_items) {
+            const int j = cur.kb * kTcKB + j1;
+            if (j < cur.n_t) { t_cur = (float)t[cur.lo + j]; y_cur = (float)y[cur.lo + j]; }
+        }
+        float2* s_uvg = &s_uv[grp][0][0];
+        float* s_yvg = &s_yv[grp][0][0];
+        while (cur.item < total_items) {
+            // ---- the group's next stage (two ring stages ahead) and its (t, y)
+            Cursor nxt = cur;
+            step(nxt);
+            if (nxt.item < total_items) step(nxt);
+            float t_nxt = 0.f, y_nxt = 0.f;
+            if (nxt.item < total_items) {
+                const int jn = nxt.kb * kTcKB + j1;
+                if (jn < nxt.n_t) { t_nxt = (float)t[nxt.lo + jn]; y_nxt = (float)y[nxt.lo + jn]; }
+            }
+            // ---- phase 1: one phasor per thread
+            const int buf = it & 1;
+            float2* suv = s_uvg + buf * (4 * kTcScratchQuad);
+            float* syv = s_yvg + buf * kTcKB;
+            {
+                const bool live = (cur.kb * kTcKB + j1) < cur.n_t;
+                const float p = cur.f_hi * t_cur;
+                const float e = fmaf(cur.f_hi, t_cur, -p);
+                const float r = (p - rintf(p)) + fmaf(cur.f_lo, t_cur, e);
+                float sn, cs;
+                sincos_cycles<FAST>(r, &sn, &cs);
+                suv[sc_w] = live ? make_float2(cs, sn) : make_float2(0.f, 0.f);
+                if (q1 == 0) syv[j1] = live ? (y_cur - cur.mean) * cur.yscale : 0.f;
+            }
+            named_bar_sync(4 + grp, kTcGenGroupThreads);
+            // ---- phase 2: products, FP16 split, operand stores
+            const float4 u01 = *reinterpret_cast<const float4*>(&suv[sc_u]);
+            const float4 u23 = *reinterpret_cast<const float4*>(&suv[sc_u + 2]);
+            const float4 v01 = *reinterpret_cast<const float4*>(&suv[sc_v]);
+            const float4 v23 = *reinterpret_cast<const float4*>(&suv[sc_v + 2]);
+            const float4 yv = *reinterpret_cast<const float4*>(&syv[8 * c + 4 * hsel]);
+            const float uc[4] = {u01.x, u01.z, u23.x, u23.z}, us[4] = {u01.y, u01.w, u23.y, u23.w};
+            const float vc[4] = {v01.x, v01.z, v23.x, v23.z}, vs[4] = {v01.y, v01.w, v23.y, v23.w};
+            const float yj[4] = {yv.x, yv.y, yv.z, yv.w};
+            float ar[4], ai[4], a2r[4], a2i[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float ec = fmaf(uc[i], vc[i], -us[i] * vs[i]);
+                const float es = fmaf(uc[i], vs[i], us[i] * vc[i]);
+                ar[i] = yj[i] * ec;
+                ai[i] = yj[i] * es;
+                const float e256 = kTcUnitScale * ec;
+                a2r[i] = fmaf(e256, ec, -(kTcUnitScale * es) * es);
+                a2i[i] = (2.f * e256) * es;
+            }
+            mbar_wait(&empty[st], eph);
+            const unsigned sa = smem_u32(smem) + (unsigned)st * (unsigned)stage_bytes;
+            auto put = [&](int plane, int off, __half2 v0, __half2 v1) {
+                asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane * A_PLANE + off),
+                             "r"(*reinterpret_cast<unsigned*>(&v0)), "r"(*reinterpret_cast<unsigned*>(&v1)) : "memory");
+            };
+            __half2 h0, h1, l0, l1;
+            split_half2(ar[0], ar[1], &h0, &l0);  split_half2(ar[2], ar[3], &h1, &l1);
+            put(0, off_re, h0, h1);  if (!FAST) put(2, off_re, l0, l1);
+            split_half2(ai[0], ai[1], &h0, &l0);  split_half2(ai[2], ai[3], &h1, &l1);
+            put(0, off_im, h0, h1);  if (!FAST) put(2, off_im, l0, l1);
+            split_half2(a2r[0], a2r[1], &h0, &l0);  split_half2(a2r[2], a2r[3], &h1, &l1);
+            put(1, off_re, h0, h1);  if (!FAST) put(NOPS - 1, off_re, l0, l1);
+            split_half2(a2i[0], a2i[1], &h0, &l0);  split_half2(a2i[2], a2i[3], &h1, &l1);
+            put(1, off_im, h0, h1);  if (!FAST) put(NOPS - 1, off_im, l0, l1);
+            fence_proxy_async();            // generic-proxy stores -> visible to the tensor core's async proxy
+            mbar_arrive(&full[st]);
+            st += 2;
+            if (st >= S) { st -= S; eph ^= 1; }
+            ++it;
+            t_cur = t_nxt;
+            y_cur = y_nxt;
+            cur = nxt;
         }
     }
     // teardown: everyone is done with TMEM before it is freed
