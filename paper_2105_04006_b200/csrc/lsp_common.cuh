@@ -146,4 +146,73 @@ __device__ __forceinline__ void sincos_cycles(double r, double* s, double* c)
     sincospi(2.0 * r, s, c);   // FAST has no FP64 meaning (rejected at plan creation)
 }
 
+// sin/cos of 2*pi*r in FP64 for an ALREADY REDUCED r in about [-1/2 - 2^-20, 1/2 + 2^-20] cycles: 21 FP64-pipe instructions
+// and a handful of integer ones, against ~36 + ~75 for the library sincospi (which redoes the range reduction, handles
+// Inf/NaN and moves 64-bit halves around).  k = round(4 r) picks the octant pair, s = r - k/4 is exact (fma), and
+// sin 2 pi s, cos 2 pi s are Taylor series in z = s^2 on |2 pi s| <= pi/4 + 2^-17: truncation error <= (pi/4)^17/17! = 5e-17
+// (sin) and (pi/4)^18/18! = 2e-18 (cos), i.e. below one ulp of 1.  The quadrant is applied with selects and a sign flip.
+__device__ __forceinline__ void sincos_cycles_reduced(double r, double* sn, double* cs)
+{
+    const double magic = 6755399441055744.0;              // 1.5 * 2^52: the low word of (x + magic) is round(x)
+    const double tq = fma(r, 4.0, magic);
+    const int k = __double2loint(tq);
+    const double kf = tq - magic;
+    const double s = fma(kf, -0.25, r);
+    const double z = s * s;
+    double ps = -0.71812230177850051223;
+    ps = fma(ps, z, 3.8199525848482821277);
+    ps = fma(ps, z, -15.094642576822990392);
+    ps = fma(ps, z, 42.058693944897653145);
+    ps = fma(ps, z, -76.705859753061385842);
+    ps = fma(ps, z, 81.605249276075054203);
+    ps = fma(ps, z, -41.341702240399760234);
+    ps = fma(ps, z, 6.2831853071795864769);
+    const double S = ps * s;
+    double pc = 0.28200596845579121507;
+    pc = fma(pc, z, -1.7143907110886720654);
+    pc = fma(pc, z, 7.9035363713184688042);
+    pc = fma(pc, z, -26.426256783374397453);
+    pc = fma(pc, z, 60.244641371876660363);
+    pc = fma(pc, z, -85.456817206693727736);
+    pc = fma(pc, z, 64.939394022668291491);
+    pc = fma(pc, z, -19.739208802178717238);
+    const double C = fma(pc, z, 1.0);
+    // k mod 4 = 0: (S, C); 1: (C, -S); 2: (-S, -C); 3: (-C, S)
+    const bool swap = (k & 1) != 0;
+    const double a = swap ? C : S, b = swap ? S : C;
+    const int sa = (int)(((unsigned)k & 2u) << 30);        // sign bit of sin: quadrants 2, 3
+    const int sb = (int)(((unsigned)(k + 1) & 2u) << 30);  // sign bit of cos: quadrants 1, 2
+    *sn = __hiloint2double(__double2hiint(a) ^ sa, __double2loint(a));
+    *cs = __hiloint2double(__double2hiint(b) ^ sb, __double2loint(b));
+}
+
+// A frequency prepared for phase evaluation against observation times of type T, and the phasor e^{2 pi i f t}.
+//   float : f = hi + lo (two floats); f t = p + e exactly (fma), p reduced by rintf, low terms added after the reduction:
+//           about 2^-48 relative to f t, no FP64 instruction.
+//   double: exact-product phase (phase_cycles_exact) and the reduced-argument sincos above.
+template <typename T> struct PhaseFreq;
+template <> struct PhaseFreq<float> {
+    float hi, lo;
+    __device__ __forceinline__ void set(double f) { hi = (float)f; lo = (float)(f - (double)hi); }
+    __device__ __forceinline__ float cycles(float t) const
+    {
+        const float p = hi * t;
+        const float e = fmaf(hi, t, -p);
+        return (p - rintf(p)) + fmaf(lo, t, e);
+    }
+    template <bool FAST> __device__ __forceinline__ void phasor(float t, float* s, float* c) const
+    {
+        sincos_cycles<FAST>(cycles(t), s, c);
+    }
+};
+template <> struct PhaseFreq<double> {
+    double f;
+    __device__ __forceinline__ void set(double f_) { f = f_; }
+    __device__ __forceinline__ double cycles(double t) const { return phase_cycles_exact(f, t); }
+    template <bool FAST> __device__ __forceinline__ void phasor(double t, double* s, double* c) const
+    {
+        sincos_cycles_reduced(cycles(t), s, c);
+    }
+};
+
 }  // namespace lsp

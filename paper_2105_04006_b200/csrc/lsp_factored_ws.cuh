@@ -54,10 +54,13 @@ struct WsMeta {          // one per ring stage, written by producer thread 0
     int pad;
 };
 
+// producer scratch per buffer (complex elements): u [JC][8], v [JC][8], then JC reals (y) rounded up to 8 complex slots
+constexpr int kWsScratchElems = 16 * 8 + 16 * 8 + 8;
 template <typename T> constexpr size_t ws_smem_bytes()
 {
     return (size_t)WsCfg<T>::STAGES * WsCfg<T>::STAGE_ELEMS * 2 * sizeof(T)      // operand ring
            + (size_t)FactoredCfg<T>::TILE * 3 * sizeof(T)              // epilogue exchange + staged powers
+           + (size_t)2 * kWsScratchElems * 2 * sizeof(T)               // producer scratch, double-buffered
            + WsCfg<T>::STAGES * (2 * sizeof(unsigned long long) + sizeof(WsMeta)) + 64;
 }
 
@@ -128,7 +131,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     V2* ring = reinterpret_cast<V2*>(smem_raw);
     V2* sX = ring + (size_t)S * STAGE;                         // [TILE] exchanged sums
     T* sP = reinterpret_cast<T*>(sX + TILE);                   // [TILE] staged powers
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(sP + TILE);
+    V2* scratch = reinterpret_cast<V2*>(sP + TILE);            // [2][kWsScratchElems] producer phasor scratch
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(scratch + 2 * kWsScratchElems);
     unsigned long long* empty = full + S;
     WsMeta* meta = reinterpret_cast<WsMeta*>(empty + S);
     __shared__ Best sbest[kWsConsumers / 32];
@@ -146,12 +150,22 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
 
     if (tid >= kWsConsumers) {
         // =========================================== producers ===============================================
+        // a_gj = y_j e^{i alpha_gj} with alpha_gj = 2 pi f(c_g) t_j and g = 8 g1 + g0.  f(c_g) = f(c_g0) + g1 (8 L df), so
+        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}:
+        // a stage of JC = 16 observations needs 2 x 8 x 16 phasors (two per producer thread, phase 1, into a small
+        // scratch) and G x JC complex products (phase 2) instead of G x JC sincos.  The b_mj are evaluated directly.
+        // Sincos calls per thread per stage drop from 12 (FP32) / 10 (FP64) to 6 / 4, and they are the reduced-argument
+        // kind (lsp_common.cuh): in FP64 the library sincospi cost the FP64 pipe a quarter of its cycles.
         const int ptid = tid - kWsConsumers;
         const int gen_g = ptid & (G - 1);
         const int gen_m = ptid & (NL - 1);
         const int gen_pos_a = operand_pos<TH, NGI, EPC>(gen_g);
         const int gen_pos_b = operand_pos<TM, NMI, EPC>(gen_m);
-        const double f_beta = ((double)gen_m + 0.5) * gp.df;                       // (m + 1/2) df
+        const int p_q = ptid & 7, p_j = ptid >> 3;                                 // phase 1: phasor index, observation
+        static_assert(JC == 16 && kWsProducers == 128 && G == 64, "producer work split");
+        PhaseFreq<T> f_u, f_v, f_b;
+        f_v.set((double)(8 * p_q) * (double)L * gp.df);                            // v_{g1 = p_q}
+        f_b.set(((double)gen_m + 0.5) * gp.df);                                    // (m + 1/2) df
         constexpr int NA = (G * JC) / kWsProducers;                                // a-elements per thread per chunk
         constexpr int NB = (NL * JC + kWsProducers - 1) / kWsProducers;            // b-elements per thread per chunk
         long long item = blockIdx.x;      // first item is static; the rest come from the global counter
@@ -166,40 +180,58 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             }
             const WsItem w = ws_decode<TILE>(gp, item, offsets);
             const T mean = stats ? (T)stats[w.obj].mean : T(0);
-            const double f_centre = gp.f_min + ((double)(w.K0 + (int64_t)gen_g * L + NL) - 0.5) * gp.df;   // f(c_g)
+            f_u.set(gp.f_min + ((double)(w.K0 + (int64_t)p_q * L + NL) - 0.5) * gp.df);      // f(c_{g0 = p_q})
             if (ptid == 0) s_next_item = (long long)gridDim.x + (long long)atomicAdd(work_counter, 1ULL);
             int64_t jb = w.j0;
             do {      // at least one chunk per item, so empty objects still reach the epilogue
-                // loads first, so their latency overlaps the wait for a free stage
-                T ta[NA], ya[NA], tb[NB];
-#pragma unroll
-                for (int it = 0; it < NA; ++it) {
-                    const int64_t j = jb + (ptid + it * kWsProducers) / G;
-                    ta[it] = (j < w.j1) ? t[w.lo + j] : T(0);
-                    ya[it] = (j < w.j1) ? y[w.lo + j] - mean : T(0);
-                }
+                // loads first, so their latency overlaps the phase-1 arithmetic and the wait for a free stage
+                const bool live1 = (jb + p_j) < w.j1;
+                const T t1 = live1 ? t[w.lo + jb + p_j] : T(0);
+                const T y1 = (live1 && p_q == 0) ? y[w.lo + jb + p_j] - mean : T(0);
+                T tb[NB];
 #pragma unroll
                 for (int it = 0; it < NB; ++it) {
                     const int64_t j = jb + (ptid + it * kWsProducers) / NL;
                     tb[it] = (j < w.j1) ? t[w.lo + j] : T(0);
                 }
+                // ---- phase 1: u and v of (p_q, p_j) into the scratch (zero beyond the item's range)
+                V2* sU = scratch + (size_t)(c & 1) * kWsScratchElems;                // [JC][8]
+                V2* sV = sU + JC * 8;                                                // [JC][8]
+                T* sY = reinterpret_cast<T*>(sV + JC * 8);                           // [JC]
+                {
+                    T sn, cs;
+                    V2 u, v;
+                    f_u.template phasor<FAST>(t1, &sn, &cs);
+                    u.x = live1 ? cs : T(0);
+                    u.y = live1 ? sn : T(0);
+                    f_v.template phasor<FAST>(t1, &sn, &cs);
+                    v.x = cs;
+                    v.y = sn;
+                    sU[p_j * 8 + p_q] = u;
+                    sV[p_j * 8 + p_q] = v;
+                    if (p_q == 0) sY[p_j] = y1;
+                }
+                named_bar_sync(1, kWsProducers);
                 const int s = c % S;
                 mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
                 V2* sA1 = ring + (size_t)s * STAGE;
                 V2* sA2 = sA1 + JC * G;
                 V2* sB1 = sA2 + JC * G;
                 V2* sB2 = sB1 + JC * NL;
+                // ---- phase 2: a = y u v, a2 = (u v)^2 for this thread's group and NA observations
 #pragma unroll
                 for (int it = 0; it < NA; ++it) {
-                    const int jj = (ptid + it * kWsProducers) / G;
-                    T sn, cs;
-                    sincos_cycles<FAST>(phase_for<T>(f_centre, ta[it]), &sn, &cs);
+                    const int jj = (ptid + it * kWsProducers) / G;                  // 2 it + (ptid >> 6)
+                    const V2 u = sU[jj * 8 + (gen_g & 7)];
+                    const V2 v = sV[jj * 8 + (gen_g >> 3)];
+                    const T yj = sY[jj];
+                    const T ec = fma(u.x, v.x, -u.y * v.y);
+                    const T es = fma(u.x, v.y, u.y * v.x);
                     V2 a1, a2;
-                    a1.x = ya[it] * cs;              // a  = y e^{i alpha}   (y = 0 beyond the item's range)
-                    a1.y = ya[it] * sn;
-                    const bool live = (jb + jj) < w.j1;
-                    a2.x = live ? fma(cs, cs, -sn * sn) : T(0);      // a2 = e^{2 i alpha}
-                    a2.y = live ? T(2) * cs * sn : T(0);
+                    a1.x = yj * ec;                  // a  = y e^{i alpha}   (u = 0, y = 0 beyond the item's range)
+                    a1.y = yj * es;
+                    a2.x = fma(ec, ec, -es * es);    // a2 = e^{2 i alpha}
+                    a2.y = T(2) * ec * es;
                     sA1[jj * G + gen_pos_a] = a1;
                     sA2[jj * G + gen_pos_a] = a2;
                 }
@@ -209,7 +241,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                     if ((NL * JC) % kWsProducers != 0 && e >= NL * JC) break;
                     const int jj = e / NL;
                     T sn, cs;
-                    sincos_cycles<FAST>(phase_for<T>(f_beta, tb[it]), &sn, &cs);
+                    f_b.template phasor<FAST>(tb[it], &sn, &cs);
                     V2 b1, b2;
                     b1.x = cs;                        // b  = e^{i beta}
                     b1.y = sn;
