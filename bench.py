@@ -83,7 +83,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"])
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="precision of the primary line")
     ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
     ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored", "tensor"])
@@ -96,7 +96,7 @@ def parse_args():
 def workload_for(name: str, dtype: str, rank: int):
     from workloads import make_config
     from workloads.configs import config_seed  # noqa: F401  (seed recipe: DESIGN.md "Input recipe")
-    cfg = {"c2": 2, "c3": 3, "c4": 4}[name]
+    cfg = {"c2": 2, "c3": 3, "c4": 4, "c5": 5}[name]
     # weak scaling: rank r draws its own object(s) from the same generator with sweep-point index r
     return make_config(cfg, dtype=dtype, point=rank)
 
@@ -374,6 +374,106 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     return out, w
 
 
+def c4_overlap(args, pkg, torch, device, flush):
+    """SURVEY.md 8(d) "C4 overlap": T_c = compute only (periodograms to a device buffer), T_d = D2H only of the resident
+    N_o x N_f buffer with the library's chunking (chunk_bytes pieces round-robin over n_copy_streams streams into the
+    pinned destination), T = the pipelined call.  hidden = (T_c + T_d - T) / min(T_c, T_d); "fully overlapped" means
+    T <= 1.05 max(T_c, T_d) + one chunk's latency."""
+    w = workload_for("c4", "f32", 0)
+    dev = torch.device("cuda", device)
+    n_streams, chunk_bytes = 3, 64 << 20
+    plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, "f32", kernel=args.kernel, device=device, n_copy_streams=n_streams,
+                    chunk_bytes=chunk_bytes)
+    h_off = torch.from_numpy(w.offsets)
+    d_off, d_t, d_y = h_off.to(dev), torch.from_numpy(w.t).to(dev), torch.from_numpy(w.y).to(dev)
+    d_out = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32, device=dev)
+    h_out = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32).pin_memory()
+    row = w.n_freq * 4
+    objs_per_chunk = max(1, chunk_bytes // row)
+    streams = [torch.cuda.Stream(device=dev) for _ in range(n_streams)]
+
+    def t_compute():
+        plan.periodogram_batched(d_off, d_t, d_y, out=d_out, h_offsets=h_off)
+
+    def t_copy():
+        cur = torch.cuda.current_stream()
+        for i, o0 in enumerate(range(0, w.n_obj, objs_per_chunk)):
+            st = streams[i % n_streams]
+            st.wait_stream(cur)
+            with torch.cuda.stream(st):
+                h_out[o0:o0 + objs_per_chunk].copy_(d_out[o0:o0 + objs_per_chunk], non_blocking=True)
+        for st in streams:
+            cur.wait_stream(st)
+
+    def t_pipe():
+        plan.periodogram_batched(d_off, d_t, d_y, host_out=h_out, h_offsets=h_off)
+
+    def timeit(fn, reps=3):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(reps):
+            flush()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            best = min(best, a.elapsed_time(b))
+        return best
+
+    tc, td, tp = timeit(t_compute), timeit(t_copy), timeit(t_pipe)
+    plan.destroy()
+    gb = w.n_obj * row / 1e9
+    return {"T_compute_ms": tc, "T_d2h_ms": td, "T_pipelined_ms": tp, "d2h_GBps": gb / (td * 1e-3),
+            "hidden_fraction": (tc + td - tp) / min(tc, td), "T_over_max": tp / max(tc, td),
+            "fully_overlapped": bool(tp <= 1.05 * max(tc, td) + td / max(1, -(-w.n_obj // objs_per_chunk))),
+            "chunk_bytes": chunk_bytes, "n_copy_streams": n_streams, "bytes": w.n_obj * row}
+
+
+def run_c5(args, pkg, torch, device, flush):
+    """BASELINE.json configs[4]: single object, N_t x N_f sweep in FP32 and FP64; pairs/s and roofline fraction per
+    point (device-resident, full periodogram; kernel time from CUDA events on the launching stream)."""
+    from workloads import make_config, C5_NT, C5_NF
+    dev = torch.device("cuda", device)
+    rows = []
+    for dtype in ("f32", "f64"):
+        pipe_ops, _ = pkg.lsp_pipe_peak(1 if dtype == "f32" else 2, device)
+        tdt = torch.float32 if dtype == "f32" else torch.float64
+        for i, nt in enumerate(C5_NT):
+            for j, nf in enumerate(C5_NF):
+                w = make_config(5, dtype=dtype, n_t=nt, n_freq=nf, point=i * len(C5_NF) + j)
+                plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, dtype, kernel=args.kernel, fast_math=args.fast_math and dtype == "f32",
+                                device=device)
+                plan.set_timing(True)
+                h_off = torch.from_numpy(w.offsets)
+                d_off, d_t, d_y = h_off.to(dev), torch.from_numpy(w.t).to(dev), torch.from_numpy(w.y).to(dev)
+                d_out = torch.empty((1, nf), dtype=tdt, device=dev)
+                steps = max(3, min(args.steps, int(2e12 / w.pairs) + 3))
+                for _ in range(max(3, args.warmup)):
+                    plan.periodogram_batched(d_off, d_t, d_y, out=d_out, h_offsets=h_off)
+                torch.cuda.synchronize()
+                tot, kms = 0.0, 0.0
+                for _ in range(steps):
+                    flush()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    plan.periodogram_batched(d_off, d_t, d_y, out=d_out, h_offsets=h_off)
+                    b.record()
+                    torch.cuda.synchronize()
+                    tot += a.elapsed_time(b)
+                    kms += plan.last_kernel_ms()
+                info = plan.last_call_info()
+                rf = roofline(info["kernel"], dtype, args.fast_math and dtype == "f32", w.pairs, kms / steps, pipe_ops)
+                rows.append({"dtype": dtype, "n_t": nt, "n_freq": nf, "pairs": w.pairs, "kernel": info["kernel"],
+                             "n_split": info["n_split"], "ms_per_step": tot / steps, "kernel_ms": kms / steps,
+                             "pairs_per_s": w.pairs * steps / (tot * 1e-3), "bound": rf["bound"], "roofline_frac": rf["frac"],
+                             "frac_executed": rf.get("frac_executed")})
+                plan.destroy()
+    return rows
+
+
 def run_b200(args, rank: int, world: int, local_rank: int):
     import torch
     if not torch.cuda.is_available():
@@ -390,6 +490,20 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     def flush():
         flush_buf.fill_(1)
 
+    if args.workload == "c5":
+        if rank == 0:
+            rows = run_c5(args, pkg, torch, local_rank, flush)
+            f32 = [r for r in rows if r["dtype"] == "f32"]
+            tot_pairs = sum(r["pairs"] for r in f32)
+            tot_ms = sum(r["ms_per_step"] for r in f32)
+            print(json.dumps({"metric": METRIC, "value": tot_pairs / (tot_ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+                              "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_ms, "higher_is_better": True,
+                              "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                              "config": {"workload": "BASELINE.json configs[4]: single-object sweep N_t x N_f, FP32 and FP64, "
+                                                     "full periodogram; value = FP32 pairs of the 12 points / their summed time",
+                                         "l2": "flushed between steps"},
+                              "sweep": rows}), flush=True)
+        return
     primary, w = run_leg(args, pkg, torch, dist, rank, world, local_rank, args.dtype, flush, True)
     other = None
     variants = {}
@@ -403,6 +517,9 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                                                    kernel="factored", fast=False, with_e2e=False)
             variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
                                                     kernel="auto", fast=True, with_e2e=False)
+    overlap = None
+    if args.workload == "c4" and rank == 0 and world == 1:
+        overlap = c4_overlap(args, pkg, torch, local_rank, flush)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = cpu_baseline(w, args.cpu_seconds)
@@ -425,6 +542,8 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                                                                   "gpu_launches", "kernel")}
         for name, v in variants.items():
             line[name] = {k: v[k] for k in ("value", "ms_per_step", "kernel_ms_per_step", "roofline", "gpu_launches", "kernel")}
+        if overlap is not None:
+            line["d2h_overlap"] = overlap
         if cpu is not None:
             line["cpu_baseline"] = cpu
         print(json.dumps(line), flush=True)

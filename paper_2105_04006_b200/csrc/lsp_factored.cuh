@@ -90,6 +90,13 @@ __device__ __forceinline__ void cmac(float2& acc_r, float2& acc_i, float ar, flo
 }
 __device__ __forceinline__ void cmac(double2& acc_r, double2& acc_i, double ar, double ai, double2 b)
 {
+#ifdef LSP_DFMA_ASM
+    asm("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc_r.x) : "d"(ar), "d"(b.x));
+    asm("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc_r.y) : "d"(ar), "d"(b.y));
+    asm("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc_i.x) : "d"(ai), "d"(b.x));
+    asm("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc_i.y) : "d"(ai), "d"(b.y));
+    return;
+#endif
     acc_r.x = fma(ar, b.x, acc_r.x);
     acc_r.y = fma(ar, b.y, acc_r.y);
     acc_i.x = fma(ai, b.x, acc_i.x);

@@ -36,6 +36,10 @@ constexpr int kWsThreads = kWsConsumers + kWsProducers;
 #ifndef LSP_WS_STAGES_F64
 #define LSP_WS_STAGES_F64 4
 #endif
+#ifndef LSP_WS_CONS_UNROLL
+#define LSP_WS_CONS_UNROLL 16
+#endif
+constexpr int kWsConsUnroll = LSP_WS_CONS_UNROLL;     // observations unrolled in the consumers' contraction loop
 template <typename T> struct WsCfg;
 template <> struct WsCfg<float> {
     static constexpr int JC = LSP_WS_JC_F32;         // observations per ring stage
@@ -291,7 +295,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             if (item < 0) break;
             const V2* A = ring + (size_t)s * STAGE + offA;
             const V2* B = ring + (size_t)s * STAGE + offB;
-#pragma unroll
+#pragma unroll(kWsConsUnroll)
             for (int jj = 0; jj < JC; ++jj) {                  // step 4
                 V2 av[TH], bv[TM];
                 if constexpr (EPC == 2) {           // one LDS.128 = two complex operands
