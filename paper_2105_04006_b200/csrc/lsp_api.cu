@@ -129,7 +129,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
         s.tp.n_ops = c.fast_math ? 2 : 4;
         s.tp.a_stage_bytes = s.tp.n_ops * 128 * kTcKB * 2;
         s.tp.b_stage_bytes = s.tp.n_ops * 2 * (int)nl * kTcKB * 2;
-        s.tp.stages = (int)std::min<int64_t>(8, (int64_t)(p->smem_optin - 16384) / (s.tp.a_stage_bytes + s.tp.b_stage_bytes));
+        s.tp.stages = (int)std::min<int64_t>(8, (int64_t)(p->smem_optin - 24576) / (s.tp.a_stage_bytes + s.tp.b_stage_bytes));
         s.tile = s.tp.tile;
         s.direct_r = 0;
         slots = p->sm_count;

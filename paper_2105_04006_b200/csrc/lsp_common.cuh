@@ -186,6 +186,34 @@ __device__ __forceinline__ void sincos_cycles_reduced(double r, double* sn, doub
     *cs = __hiloint2double(__double2hiint(b) ^ sb, __double2loint(b));
 }
 
+// FP32 version for a reduced r in about [-1/2, 1/2] cycles: k = round(4 r) by the magic-constant add, s = r - k/4 exact, Taylor
+// series on |2 pi s| <= pi/4 (truncation 1.8e-9 for sin, 2.5e-8 for cos: below half an ulp of 1), quadrant by selects and
+// sign flips: ~22 FMA/ALU-pipe instructions and no XU instruction (sincospif: ~40 with FRND / F2I).
+__device__ __forceinline__ void sincos_cycles_reduced(float r, float* sn, float* cs)
+{
+    const float magic = 12582912.0f;                       // 1.5 * 2^23: the low mantissa bits of (x + magic) are round(x)
+    const float tq = fmaf(r, 4.0f, magic);
+    const unsigned k = __float_as_uint(tq);                // 0x4B400000 + round(4 r): the two low bits are the quadrant
+    const float kf = tq - magic;
+    const float s = fmaf(kf, -0.25f, r);
+    const float z = s * s;
+    float ps = 42.058693944897653f;
+    ps = fmaf(ps, z, -76.705859753061386f);
+    ps = fmaf(ps, z, 81.605249276075054f);
+    ps = fmaf(ps, z, -41.341702240399760f);
+    ps = fmaf(ps, z, 6.2831853071795865f);
+    const float S = ps * s;
+    float pc = 60.244641371876660f;
+    pc = fmaf(pc, z, -85.456817206693728f);
+    pc = fmaf(pc, z, 64.939394022668291f);
+    pc = fmaf(pc, z, -19.739208802178717f);
+    const float C = fmaf(pc, z, 1.0f);
+    const bool swap = (k & 1u) != 0;
+    const float a = swap ? C : S, b = swap ? S : C;
+    *sn = __uint_as_float(__float_as_uint(a) ^ ((k & 2u) << 30));
+    *cs = __uint_as_float(__float_as_uint(b) ^ (((k + 1u) & 2u) << 30));
+}
+
 // A frequency prepared for phase evaluation against observation times of type T, and the phasor e^{2 pi i f t}.
 //   float : f = hi + lo (two floats); f t = p + e exactly (fma), p reduced by rintf, low terms added after the reduction:
 //           about 2^-48 relative to f t, no FP64 instruction.

@@ -34,6 +34,8 @@
 #pragma once
 #include <cuda_fp16.h>
 
+#include <type_traits>
+
 #include "lsp_factored_ws.cuh"
 
 namespace lsp {
@@ -47,7 +49,10 @@ constexpr int kTcGenGroupThreads = 256;                               // threads
 // register split (setmaxnreg, per 4-warp group): 128 x 40 + 256 x 120 + 512 x 56 = 64512 = 896 x 72
 constexpr int kTcCtrlRegs = 40, kTcEpiRegs = 120, kTcGenRegs = 56;
 constexpr int kTcEpiThreads = kTcEpiWarps * 32;
-constexpr int kTcScratchQuad = 16 * 4 + 2;   // float2 per observation quad of the generator scratch (+16 B: conflict-free LDS.128)
+// Generator scratch (floats): three planes (cos, sin, -sin) of [observation quad j/4][phasor q][j%4]; a quad row is 16 x 4
+// floats + 16 floats of padding so that the two quads a quarter-warp reads fall into different banks (conflict-free LDS.128).
+constexpr int kTcScratchQuad = 16 * 4 + 16;
+constexpr int kTcScratchPlane = 4 * kTcScratchQuad;
 constexpr float kTcUnitScale = 256.0f;         // scale of the unit-modulus A_W operands (keeps the FP16 low part normal)
 
 struct TensorParams {
@@ -247,6 +252,19 @@ __device__ __forceinline__ void tc_commit(unsigned long long* bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// mbarrier wait for roles whose waits are long when they are not the bottleneck (generators on a full ring, epilogue on
+// unfinished accumulators): back off between polls so the spinning warps do not take issue slots from the working ones.
+__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* bar, unsigned parity)
+{
+    unsigned done;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    while (!done) {
+        __nanosleep(40);
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    }
+}
 __device__ __forceinline__ bool elect_one()
 {
     unsigned pred;
@@ -325,7 +343,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
     __shared__ Best sbest[kTcEpiWarps];
-    __shared__ __align__(16) float2 s_uv[2][2][4 * kTcScratchQuad];  // generator scratch: [group][buffer][j/4][phasor q][j%4], padded
+    __shared__ __align__(16) float s_uv[2][2][3 * kTcScratchPlane];  // generator scratch: [group][buffer][plane][j/4][phasor q][j%4]
     __shared__ __align__(16) float s_yv[2][2][kTcKB];                // scaled, centred y of the stage
 
     const int tid = threadIdx.x, lane = tid & 31;
@@ -447,19 +465,22 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const TensorObj ob = objs[w.obj_local];
             const bool have = w.kb1 > w.kb0;
             if (have) {
-                mbar_wait(tmem_full, n_acc & 1);
+                mbar_wait_backoff(tmem_full, n_acc & 1);
                 tc_fence_after();
             }
             float bp = -1.0f;                                     // running maximum (P >= 0; NaN never compares greater)
-            int bk = 0x7fffffff;
+            int bi = -1;                                          // its position m = 16 ch + i in this lane's sequence
             const float n_hat = kTcUnitScale * (float)w.n_t;
+            const float nn = n_hat * n_hat, nn_eps = 2e-6f * nn;
             const int n_valid = (int)min((int64_t)tp.tile, (int64_t)gp.n_freq - w.K0);     // frequencies of this tile on the grid
             const bool ragged = n_valid < tp.tile;
             T* otile = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq + w.K0 : nullptr;
             float4* stile = (gp.n_split > 1) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
             const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
             bool released = false;
-            for (int ch = ch0; ch < ch1; ++ch) {
+            // one chunk = 16 accumulator columns of each of the four TMEM regions; RAG = the tile overhangs the grid
+            auto chunk = [&](int ch, auto rag_tag) {
+                constexpr bool RAG = decltype(rag_tag)::value;
                 const int m0 = ch * 16;
                 float zr[16], zi[16], wr[16], wi[16];
                 if (have) {
@@ -483,59 +504,103 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
 #pragma unroll
                 for (int v4 = 0; v4 < 4; ++v4) {
                     if (4 * v4 >= i_lim) break;
-                    float pw[4];
+                    float za[4], zb[4], wa[4], wb[4], pw[4];
+                    bool bad = false;
 #pragma unroll
                     for (int e = 0; e < 4; ++e) {
                         const int i = 4 * v4 + e;
                         // partner lane (xor 16) holds the other row of the same group
                         const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
                         const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
-                        // Re lane: (zr, zi) = (Srr, Sri), (p0, p1) = (Sir, Sii): up   Z = (Srr - Sii) + i (Sri + Sir)
-                        // Im lane: (zr, zi) = (Sir, Sii), (p0, p1) = (Srr, Sri): down Z = (Srr + Sii) + i (Sir - Sri)
-                        const float za = zr[i] - p1, zb = zi[i] + p0;
-                        const float wa = wr[i] - q1, wb = wi[i] + q0;
-                        const float xc = is_im ? zb : za, xs = is_im ? za : zb;
-                        const float c2 = is_im ? wb : wa, s2 = is_im ? wa : wb;
-                        if (stile) {                   // split-N_t: un-scaled partial sums for lsp_combine_kernel
-                            const int kl = is_im ? kl0 - i : kl0 + i;
-                            if (kl < n_valid)
-                                stile[kl] = make_float4(xc * ob.zinv, xs * ob.zinv, c2 * (1.0f / kTcUnitScale), s2 * (1.0f / kTcUnitScale));
-                        } else {
-                            pw[e] = power_from_sums<float>(xc, xs, c2, s2, n_hat, ob.pscale);
-                        }
+                        // Re lane: (zr, zi) = (Srr, Sri), (p0, p1) = (Sir, Sii): up   Z = (Srr - Sii) + i (Sri + Sir) = za + i zb
+                        // Im lane: (zr, zi) = (Sir, Sii), (p0, p1) = (Srr, Sri): down Z = (Srr + Sii) + i (Sir - Sri) = zb + i za
+                        za[e] = zr[i] - p1;  zb[e] = zi[i] + p0;
+                        wa[e] = wr[i] - q1;  wb[e] = wi[i] + q0;
+                        // Step 5 (lsp_common.cuh power_from_sums) written on (za, zb): swapping xc <-> xs only flips the sign
+                        // of the c2 term, so with (c, s) = (wa, wb) on Re lanes and (-wb, wa) on Im lanes
+                        //   P = [ n (A + B) - c (A - B) - 2 s za zb ] / (n^2 - wa^2 - wb^2),  A = za^2, B = zb^2.
+                        const float cc = is_im ? -wb[e] : wa[e], ss = is_im ? wa[e] : wb[e];
+                        const float A = __fmul_rn(za[e], za[e]), B = __fmul_rn(zb[e], zb[e]);
+                        const float den = nn - fmaf(wa[e], wa[e], __fmul_rn(wb[e], wb[e]));
+                        const float num = fmaf(-2.0f * ss, __fmul_rn(za[e], zb[e]), fmaf(-cc, A - B, __fmul_rn(n_hat, A + B)));
+                        bad = bad || !(den > nn_eps);
+                        pw[e] = __fdividef(num, den) * ob.pscale;
                     }
-                    if (stile) continue;
-                    // element e of the 4-vector in ascending frequency: up -> pw[e], down -> pw[3 - e]
-                    const int klv = is_im ? (kl0 - 4 * v4 - 3) : (kl0 + 4 * v4);
-                    const float e0 = is_im ? pw[3] : pw[0], e1 = is_im ? pw[2] : pw[1];
-                    const float e2 = is_im ? pw[1] : pw[2], e3 = is_im ? pw[0] : pw[3];
-                    if (!ragged) {
-                        if (otile) {
-                            if (vec_ok) {
-                                *reinterpret_cast<float4*>(otile + klv) = make_float4(e0, e1, e2, e3);
-                            } else {
-                                otile[klv] = (T)e0; otile[klv + 1] = (T)e1; otile[klv + 2] = (T)e2; otile[klv + 3] = (T)e3;
-                            }
-                        }
-                        if (partials) {
-                            if (e0 > bp || (e0 == bp && klv < bk)) { bp = e0; bk = klv; }
-                            if (e1 > bp || (e1 == bp && klv + 1 < bk)) { bp = e1; bk = klv + 1; }
-                            if (e2 > bp || (e2 == bp && klv + 2 < bk)) { bp = e2; bk = klv + 2; }
-                            if (e3 > bp || (e3 == bp && klv + 3 < bk)) { bp = e3; bk = klv + 3; }
-                        }
-                    } else {
-                        const float ev[4] = {e0, e1, e2, e3};
+                    if (bad) {                                    // vanishing denominator (reading a6): the full epilogue, rarely
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            pw[e] = power_from_sums<float>(is_im ? zb[e] : za[e], is_im ? za[e] : zb[e], is_im ? wb[e] : wa[e],
+                                                           is_im ? wa[e] : wb[e], n_hat, ob.pscale);
+                    }
+                    if (partials) {
+                        // up lanes meet their frequencies in ascending, down lanes in descending order: "lowest index wins
+                        // ties" is "first wins" for the former and "last wins" for the latter
 #pragma unroll
                         for (int e = 0; e < 4; ++e) {
-                            const int kl = klv + e;
-                            if (kl < n_valid) {
-                                if (otile) otile[kl] = (T)ev[e];
-                                if (partials && (ev[e] > bp || (ev[e] == bp && kl < bk))) { bp = ev[e]; bk = kl; }
-                            }
+                            const int i = 4 * v4 + e;
+                            bool take = (pw[e] > bp) || (is_im && pw[e] == bp);
+                            if (RAG) take = take && ((is_im ? kl0 - i : kl0 + i) < n_valid);
+                            bi = take ? (m0 + i) : bi;
+                            bp = take ? pw[e] : bp;
+                        }
+                    }
+                    if (otile) {
+                        // element e of the 4-vector in ascending frequency: up -> pw[e], down -> pw[3 - e]
+                        const int klv = is_im ? (kl0 - 4 * v4 - 3) : (kl0 + 4 * v4);
+                        const float e0 = is_im ? pw[3] : pw[0], e1 = is_im ? pw[2] : pw[1];
+                        const float e2 = is_im ? pw[1] : pw[2], e3 = is_im ? pw[0] : pw[3];
+                        if (!RAG && vec_ok) {
+                            *reinterpret_cast<float4*>(otile + klv) = make_float4(e0, e1, e2, e3);
+                        } else {
+                            if (klv < n_valid) otile[klv] = (T)e0;
+                            if (klv + 1 < n_valid) otile[klv + 1] = (T)e1;
+                            if (klv + 2 < n_valid) otile[klv + 2] = (T)e2;
+                            if (klv + 3 < n_valid) otile[klv + 3] = (T)e3;
                         }
                     }
                 }
+            };
+            // split-N_t: un-scaled partial sums (xc, xs, c2, s2) per frequency for lsp_combine_kernel
+            auto chunk_sums = [&](int ch) {
+                const int m0 = ch * 16;
+                float zr[16], zi[16], wr[16], wi[16];
+                if (have) {
+                    tc_ld16(ta + m0, zr);
+                    tc_ld16(ta + NL + m0, zi);
+                    tc_ld16(ta + 256 + m0, wr);
+                    tc_ld16(ta + 256 + NL + m0, wi);
+                    tc_ld_wait();
+                    if (ch == ch1 - 1) {
+                        tc_fence_before();
+                        mbar_arrive(tmem_empty);
+                        released = true;
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) zr[i] = zi[i] = wr[i] = wi[i] = 0.f;
+                }
+                const int i_lim = min(16, NL - m0);
+                const int kl0 = is_im ? (kc - 1 - m0) : (kc + m0);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
+                    const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
+                    const float za = zr[i] - p1, zb = zi[i] + p0, wa = wr[i] - q1, wb = wi[i] + q0;
+                    const float xc = is_im ? zb : za, xs = is_im ? za : zb;
+                    const float c2 = is_im ? wb : wa, s2 = is_im ? wa : wb;
+                    const int kl = is_im ? kl0 - i : kl0 + i;
+                    if (i < i_lim && kl < n_valid)
+                        stile[kl] = make_float4(xc * ob.zinv, xs * ob.zinv, c2 * (1.0f / kTcUnitScale), s2 * (1.0f / kTcUnitScale));
+                }
+            };
+            if (stile) {
+                for (int ch = ch0; ch < ch1; ++ch) chunk_sums(ch);
+            } else if (ragged) {
+                for (int ch = ch0; ch < ch1; ++ch) chunk(ch, std::true_type{});
+            } else {
+                for (int ch = ch0; ch < ch1; ++ch) chunk(ch, std::false_type{});
             }
+            const int bk = (bi < 0) ? 0x7fffffff : (is_im ? kc - 1 - bi : kc + bi);
             if (have) {
                 if (!released) {                                  // a warp without chunks (NL <= 16) still signs off
                     tc_fence_before();
@@ -621,89 +686,108 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 seek(cu);
             }
         };
-        Cursor cur;
-        cur.item = blockIdx.x;
-        seek(cur);
-        if (grp == 1 && cur.item < total_items) step(cur);
-        int st = grp;                                             // ring slot of this group's current stage
+        // cur = the group's stage being built (its t, y already in registers); its successor's (t, y) are loaded before
+        // the current stage is processed.
+        Cursor p1;
+        p1.item = blockIdx.x;
+        seek(p1);
+        if (grp == 1 && p1.item < total_items) step(p1);
+        int st = grp;                                             // ring slot of the stage phase 2 writes
         unsigned eph = 1;                                         // parity of the "empty" phase to wait for
         if (st >= S) { st -= S; eph ^= 1; }
         unsigned it = 0;
-        float t_cur = 0.f, y_cur = 0.f;
-        if (cur.item < total_items) {
-            const int j = cur.kb * kTcKB + j1;
-            if (j < cur.n_t) { t_cur = (float)t[cur.lo + j]; y_cur = (float)y[cur.lo + j]; }
-        }
-        float2* s_uvg = &s_uv[grp][0][0];
+        float* s_uvg = &s_uv[grp][0][0];
         float* s_yvg = &s_yv[grp][0][0];
-        while (cur.item < total_items) {
-            // ---- the group's next stage (two ring stages ahead) and its (t, y)
-            Cursor nxt = cur;
-            step(nxt);
-            if (nxt.item < total_items) step(nxt);
-            float t_nxt = 0.f, y_nxt = 0.f;
-            if (nxt.item < total_items) {
-                const int jn = nxt.kb * kTcKB + j1;
-                if (jn < nxt.n_t) { t_nxt = (float)t[nxt.lo + jn]; y_nxt = (float)y[nxt.lo + jn]; }
+        auto fetch = [&](const Cursor& cu, float& tv, float& yv_) {
+            tv = 0.f;
+            yv_ = 0.f;
+            if (cu.item < total_items) {
+                const int j = cu.kb * kTcKB + j1;
+                if (j < cu.n_t) { tv = (float)t[cu.lo + j]; yv_ = (float)y[cu.lo + j]; }
             }
-            // ---- phase 1: one phasor per thread
+        };
+        auto phase1 = [&](const Cursor& cu, float tv, float yv_, int buf) {
+            float* suv = s_uvg + buf * (3 * kTcScratchPlane);
+            const bool live = (cu.kb * kTcKB + j1) < cu.n_t;
+            const float p = cu.f_hi * tv;
+            const float e = fmaf(cu.f_hi, tv, -p);
+            const float r = (p - rintf(p)) + fmaf(cu.f_lo, tv, e);
+            float sn, cs;
+            if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
+            cs = live ? cs : 0.f;
+            sn = live ? sn : 0.f;
+            suv[sc_w] = cs;
+            suv[kTcScratchPlane + sc_w] = sn;
+            if (q1 < 8) suv[2 * kTcScratchPlane + sc_w] = -sn;
+            if (q1 == 0) s_yvg[buf * kTcKB + j1] = live ? (yv_ - cu.mean) * cu.yscale : 0.f;
+        };
+        float t_p1, y_p1;
+        fetch(p1, t_p1, y_p1);
+        while (p1.item < total_items) {
             const int buf = it & 1;
-            float2* suv = s_uvg + buf * (4 * kTcScratchQuad);
-            float* syv = s_yvg + buf * kTcKB;
-            {
-                const bool live = (cur.kb * kTcKB + j1) < cur.n_t;
-                const float p = cur.f_hi * t_cur;
-                const float e = fmaf(cur.f_hi, t_cur, -p);
-                const float r = (p - rintf(p)) + fmaf(cur.f_lo, t_cur, e);
-                float sn, cs;
-                sincos_cycles<FAST>(r, &sn, &cs);
-                suv[sc_w] = live ? make_float2(cs, sn) : make_float2(0.f, 0.f);
-                if (q1 == 0) syv[j1] = live ? (y_cur - cur.mean) * cur.yscale : 0.f;
-            }
+            const float* suv = s_uvg + buf * (3 * kTcScratchPlane);
+            const float* syv = s_yvg + buf * kTcKB;
+            // ---- phase 1 of this stage, then the loads of the group's next stage (two ring stages ahead)
+            phase1(p1, t_p1, y_p1, buf);
+            step(p1);
+            if (p1.item < total_items) step(p1);
+            float t_pf, y_pf;
+            fetch(p1, t_pf, y_pf);
             named_bar_sync(4 + grp, kTcGenGroupThreads);
-            // ---- phase 2: products, FP16 split, operand stores
-            const float4 u01 = *reinterpret_cast<const float4*>(&suv[sc_u]);
-            const float4 u23 = *reinterpret_cast<const float4*>(&suv[sc_u + 2]);
-            const float4 v01 = *reinterpret_cast<const float4*>(&suv[sc_v]);
-            const float4 v23 = *reinterpret_cast<const float4*>(&suv[sc_v + 2]);
+            const float4 ucv = *reinterpret_cast<const float4*>(&suv[sc_u]);
+            const float4 usv = *reinterpret_cast<const float4*>(&suv[kTcScratchPlane + sc_u]);
+            const float4 unv = *reinterpret_cast<const float4*>(&suv[2 * kTcScratchPlane + sc_u]);
+            const float4 vcv = *reinterpret_cast<const float4*>(&suv[sc_v]);
+            const float4 vsv = *reinterpret_cast<const float4*>(&suv[kTcScratchPlane + sc_v]);
             const float4 yv = *reinterpret_cast<const float4*>(&syv[8 * c + 4 * hsel]);
-            const float uc[4] = {u01.x, u01.z, u23.x, u23.z}, us[4] = {u01.y, u01.w, u23.y, u23.w};
-            const float vc[4] = {v01.x, v01.z, v23.x, v23.z}, vs[4] = {v01.y, v01.w, v23.y, v23.w};
-            const float yj[4] = {yv.x, yv.y, yv.z, yv.w};
-            float ar[4], ai[4], a2r[4], a2i[4];
+            // ---- phase 2: products (packed FP32x2), FP16 split, operand stores
+            float2 ar[2], ai[2], a2r[2], a2i[2];
+            {
+                const float2 k256 = make_float2(kTcUnitScale, kTcUnitScale), km256 = make_float2(-kTcUnitScale, -kTcUnitScale);
+                const float2 k512 = make_float2(2.f * kTcUnitScale, 2.f * kTcUnitScale);
+                const float2 uc[2] = {make_float2(ucv.x, ucv.y), make_float2(ucv.z, ucv.w)};
+                const float2 us[2] = {make_float2(usv.x, usv.y), make_float2(usv.z, usv.w)};
+                const float2 un[2] = {make_float2(unv.x, unv.y), make_float2(unv.z, unv.w)};
+                const float2 vc[2] = {make_float2(vcv.x, vcv.y), make_float2(vcv.z, vcv.w)};
+                const float2 vs[2] = {make_float2(vsv.x, vsv.y), make_float2(vsv.z, vsv.w)};
+                const float2 yy[2] = {make_float2(yv.x, yv.y), make_float2(yv.z, yv.w)};
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const float ec = fmaf(uc[i], vc[i], -us[i] * vs[i]);
-                const float es = fmaf(uc[i], vs[i], us[i] * vc[i]);
-                ar[i] = yj[i] * ec;
-                ai[i] = yj[i] * es;
-                const float e256 = kTcUnitScale * ec;
-                a2r[i] = fmaf(e256, ec, -(kTcUnitScale * es) * es);
-                a2i[i] = (2.f * e256) * es;
+                for (int h = 0; h < 2; ++h) {
+                    const float2 ec = __ffma2_rn(uc[h], vc[h], __fmul2_rn(un[h], vs[h]));      // uc vc - us vs
+                    const float2 es = __ffma2_rn(uc[h], vs[h], __fmul2_rn(us[h], vc[h]));      // uc vs + us vc
+                    ar[h] = __fmul2_rn(yy[h], ec);
+                    ai[h] = __fmul2_rn(yy[h], es);
+                    const float2 e256 = __fmul2_rn(ec, k256), n256 = __fmul2_rn(es, km256);
+                    a2r[h] = __ffma2_rn(e256, ec, __fmul2_rn(n256, es));                       // 256 (ec^2 - es^2)
+                    a2i[h] = __fmul2_rn(__fmul2_rn(ec, k512), es);                             // 512 ec es
+                }
             }
-            mbar_wait(&empty[st], eph);
+            mbar_wait_backoff(&empty[st], eph);
             const unsigned sa = smem_u32(smem) + (unsigned)st * (unsigned)stage_bytes;
-            auto put = [&](int plane, int off, __half2 v0, __half2 v1) {
-                asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane * A_PLANE + off),
-                             "r"(*reinterpret_cast<unsigned*>(&v0)), "r"(*reinterpret_cast<unsigned*>(&v1)) : "memory");
+            // hi = fp16x2(x), lo = fp16x2(x - hi): one packed convert, two unpacks, one FFMA2, one packed convert per pair
+            auto put = [&](int plane_hi, int plane_lo, int off, const float2 (&x)[2]) {
+                const float2 m1 = make_float2(-1.f, -1.f);
+                const __half2 h0 = __floats2half2_rn(x[0].x, x[0].y), h1 = __floats2half2_rn(x[1].x, x[1].y);
+                asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane_hi * A_PLANE + off),
+                             "r"(*reinterpret_cast<const unsigned*>(&h0)), "r"(*reinterpret_cast<const unsigned*>(&h1)) : "memory");
+                if (!FAST) {
+                    const float2 r0 = __ffma2_rn(__half22float2(h0), m1, x[0]), r1 = __ffma2_rn(__half22float2(h1), m1, x[1]);
+                    const __half2 l0 = __floats2half2_rn(r0.x, r0.y), l1 = __floats2half2_rn(r1.x, r1.y);
+                    asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane_lo * A_PLANE + off),
+                                 "r"(*reinterpret_cast<const unsigned*>(&l0)), "r"(*reinterpret_cast<const unsigned*>(&l1)) : "memory");
+                }
             };
-            __half2 h0, h1, l0, l1;
-            split_half2(ar[0], ar[1], &h0, &l0);  split_half2(ar[2], ar[3], &h1, &l1);
-            put(0, off_re, h0, h1);  if (!FAST) put(2, off_re, l0, l1);
-            split_half2(ai[0], ai[1], &h0, &l0);  split_half2(ai[2], ai[3], &h1, &l1);
-            put(0, off_im, h0, h1);  if (!FAST) put(2, off_im, l0, l1);
-            split_half2(a2r[0], a2r[1], &h0, &l0);  split_half2(a2r[2], a2r[3], &h1, &l1);
-            put(1, off_re, h0, h1);  if (!FAST) put(NOPS - 1, off_re, l0, l1);
-            split_half2(a2i[0], a2i[1], &h0, &l0);  split_half2(a2i[2], a2i[3], &h1, &l1);
-            put(1, off_im, h0, h1);  if (!FAST) put(NOPS - 1, off_im, l0, l1);
+            put(0, 2, off_re, ar);
+            put(0, 2, off_im, ai);
+            put(1, NOPS - 1, off_re, a2r);
+            put(1, NOPS - 1, off_im, a2i);
             fence_proxy_async();            // generic-proxy stores -> visible to the tensor core's async proxy
             mbar_arrive(&full[st]);
             st += 2;
             if (st >= S) { st -= S; eph ^= 1; }
             ++it;
-            t_cur = t_nxt;
-            y_cur = y_nxt;
-            cur = nxt;
+            t_p1 = t_pf;
+            y_p1 = y_pf;
         }
     }
     // teardown: everyone is done with TMEM before it is freed
