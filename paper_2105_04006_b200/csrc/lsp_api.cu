@@ -246,7 +246,8 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
         gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
         gq.n_freq = (int)c.n_freq;
         gq.obj_base = (int)obj_base;
-        lsp_tensor_stats_kernel<float><<<(unsigned)n_obj_launch, 128, 0, st>>>(d_off, (const float*)d_y, (TensorObj*)p->tc_objs.ptr,
+        const int stats_threads = n_obj_launch < 64 ? 1024 : 128;     // a lone long object gets a full CTA
+        lsp_tensor_stats_kernel<float><<<(unsigned)n_obj_launch, stats_threads, 0, st>>>(d_off, (const float*)d_y, (TensorObj*)p->tc_objs.ptr,
                                                                             (int)obj_base, c.center, c.normalize);
         lsp_tensor_scan_kernel<<<1, 1024, 0, st>>>(d_off, (TensorObj*)p->tc_objs.ptr, (int)obj_base, (int)n_obj_launch);
         if (kb_bound > 0) {

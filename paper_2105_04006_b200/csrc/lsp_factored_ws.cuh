@@ -28,18 +28,14 @@ constexpr int kWsThreads = kWsConsumers + kWsProducers;
 #define LSP_WS_JC_F32 16
 #endif
 #ifndef LSP_WS_JC_F64
-#define LSP_WS_JC_F64 16
-#endif
+#define LSP_WS_JC_F64 32      // FP64: 32-observation stages x 2 (same bytes as 16 x 4): the consumers' loop-carried register
+#endif                        // permutation (~105 moves per unrolled stage, each displacing a DFMA) is paid half as often
 #ifndef LSP_WS_STAGES_F32
 #define LSP_WS_STAGES_F32 4
 #endif
 #ifndef LSP_WS_STAGES_F64
-#define LSP_WS_STAGES_F64 4
+#define LSP_WS_STAGES_F64 2
 #endif
-#ifndef LSP_WS_CONS_UNROLL
-#define LSP_WS_CONS_UNROLL 16
-#endif
-constexpr int kWsConsUnroll = LSP_WS_CONS_UNROLL;     // observations unrolled in the consumers' contraction loop
 template <typename T> struct WsCfg;
 template <> struct WsCfg<float> {
     static constexpr int JC = LSP_WS_JC_F32;         // observations per ring stage
@@ -58,13 +54,13 @@ struct WsMeta {          // one per ring stage, written by producer thread 0
     int pad;
 };
 
-// producer scratch per buffer (complex elements): u [JC][8], v [JC][8], then JC reals (y) rounded up to 8 complex slots
-constexpr int kWsScratchElems = 16 * 8 + 16 * 8 + 8;
+// producer scratch per buffer (complex elements): u [JC][8], v [JC][8], then JC reals (y) = JC / 2 complex slots
+template <typename T> __host__ __device__ constexpr int ws_scratch_elems() { return WsCfg<T>::JC * 16 + WsCfg<T>::JC / 2; }
 template <typename T> constexpr size_t ws_smem_bytes()
 {
     return (size_t)WsCfg<T>::STAGES * WsCfg<T>::STAGE_ELEMS * 2 * sizeof(T)      // operand ring
            + (size_t)FactoredCfg<T>::TILE * 3 * sizeof(T)              // epilogue exchange + staged powers
-           + (size_t)2 * kWsScratchElems * 2 * sizeof(T)               // producer scratch, double-buffered
+           + (size_t)2 * ws_scratch_elems<T>() * 2 * sizeof(T)         // producer scratch, double-buffered
            + WsCfg<T>::STAGES * (2 * sizeof(unsigned long long) + sizeof(WsMeta)) + 64;
 }
 
@@ -88,6 +84,19 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
             "selp.u32 %0, 1, 0, p;\n\t}"
             : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     } while (!done);
+}
+// The same wait with a back-off between polls, for the role that is NOT the bottleneck (its waits are long): a spinning warp
+// takes issue slots from the working warps of its scheduler, and in FP64 every such slot displaces a DFMA.
+__device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigned parity, unsigned ns)
+{
+    unsigned done;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    while (!done) {
+        __nanosleep(ns);
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    }
 }
 __device__ __forceinline__ void named_bar_sync(int id, int n_threads)
 {
@@ -135,8 +144,9 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     V2* ring = reinterpret_cast<V2*>(smem_raw);
     V2* sX = ring + (size_t)S * STAGE;                         // [TILE] exchanged sums
     T* sP = reinterpret_cast<T*>(sX + TILE);                   // [TILE] staged powers
-    V2* scratch = reinterpret_cast<V2*>(sP + TILE);            // [2][kWsScratchElems] producer phasor scratch
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(scratch + 2 * kWsScratchElems);
+    constexpr int SCR = ws_scratch_elems<T>();
+    V2* scratch = reinterpret_cast<V2*>(sP + TILE);            // [2][SCR] producer phasor scratch
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(scratch + 2 * SCR);
     unsigned long long* empty = full + S;
     WsMeta* meta = reinterpret_cast<WsMeta*>(empty + S);
     __shared__ Best sbest[kWsConsumers / 32];
@@ -166,7 +176,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
         const int gen_pos_a = operand_pos<TH, NGI, EPC>(gen_g);
         const int gen_pos_b = operand_pos<TM, NMI, EPC>(gen_m);
         const int p_q = ptid & 7, p_j = ptid >> 3;                                 // phase 1: phasor index, observation
-        static_assert(JC == 16 && kWsProducers == 128 && G == 64, "producer work split");
+        static_assert(JC % 16 == 0 && kWsProducers == 128 && G == 64, "producer work split");
+        constexpr int NP = JC / 16;                                                // (u, v) pairs per thread per chunk
         PhaseFreq<T> f_u, f_v, f_b;
         f_v.set((double)(8 * p_q) * (double)L * gp.df);                            // v_{g1 = p_q}
         f_b.set(((double)gen_m + 0.5) * gp.df);                                    // (m + 1/2) df
@@ -189,35 +200,41 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             int64_t jb = w.j0;
             do {      // at least one chunk per item, so empty objects still reach the epilogue
                 // loads first, so their latency overlaps the phase-1 arithmetic and the wait for a free stage
-                const bool live1 = (jb + p_j) < w.j1;
-                const T t1 = live1 ? t[w.lo + jb + p_j] : T(0);
-                const T y1 = (live1 && p_q == 0) ? y[w.lo + jb + p_j] - mean : T(0);
+                T t1[NP], y1[NP];
+#pragma unroll
+                for (int h = 0; h < NP; ++h) {
+                    const bool live1 = (jb + p_j + 16 * h) < w.j1;
+                    t1[h] = live1 ? t[w.lo + jb + p_j + 16 * h] : T(0);
+                    y1[h] = (live1 && p_q == 0) ? y[w.lo + jb + p_j + 16 * h] - mean : T(0);
+                }
                 T tb[NB];
 #pragma unroll
                 for (int it = 0; it < NB; ++it) {
                     const int64_t j = jb + (ptid + it * kWsProducers) / NL;
                     tb[it] = (j < w.j1) ? t[w.lo + j] : T(0);
                 }
-                // ---- phase 1: u and v of (p_q, p_j) into the scratch (zero beyond the item's range)
-                V2* sU = scratch + (size_t)(c & 1) * kWsScratchElems;                // [JC][8]
+                // ---- phase 1: u and v of (p_q, p_j + 16 h) into the scratch (zero beyond the item's range)
+                V2* sU = scratch + (size_t)(c & 1) * SCR;                            // [JC][8]
                 V2* sV = sU + JC * 8;                                                // [JC][8]
                 T* sY = reinterpret_cast<T*>(sV + JC * 8);                           // [JC]
-                {
+#pragma unroll
+                for (int h = 0; h < NP; ++h) {
+                    const bool live1 = (jb + p_j + 16 * h) < w.j1;
                     T sn, cs;
                     V2 u, v;
-                    f_u.template phasor<FAST>(t1, &sn, &cs);
+                    f_u.template phasor<FAST>(t1[h], &sn, &cs);
                     u.x = live1 ? cs : T(0);
                     u.y = live1 ? sn : T(0);
-                    f_v.template phasor<FAST>(t1, &sn, &cs);
+                    f_v.template phasor<FAST>(t1[h], &sn, &cs);
                     v.x = cs;
                     v.y = sn;
-                    sU[p_j * 8 + p_q] = u;
-                    sV[p_j * 8 + p_q] = v;
-                    if (p_q == 0) sY[p_j] = y1;
+                    sU[(p_j + 16 * h) * 8 + p_q] = u;
+                    sV[(p_j + 16 * h) * 8 + p_q] = v;
+                    if (p_q == 0) sY[p_j + 16 * h] = y1[h];
                 }
                 named_bar_sync(1, kWsProducers);
                 const int s = c % S;
-                mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
+                mbar_wait_sleep(&empty[s], ((c / S) & 1) ^ 1, 100);
                 V2* sA1 = ring + (size_t)s * STAGE;
                 V2* sA2 = sA1 + JC * G;
                 V2* sB1 = sA2 + JC * G;
@@ -295,7 +312,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             if (item < 0) break;
             const V2* A = ring + (size_t)s * STAGE + offA;
             const V2* B = ring + (size_t)s * STAGE + offB;
-#pragma unroll(kWsConsUnroll)
+#pragma unroll
             for (int jj = 0; jj < JC; ++jj) {                  // step 4
                 V2 av[TH], bv[TM];
                 if constexpr (EPC == 2) {           // one LDS.128 = two complex operands

@@ -81,7 +81,7 @@ template <typename T>
 __global__ void lsp_tensor_stats_kernel(const int64_t* __restrict__ offsets, const T* __restrict__ y, TensorObj* __restrict__ objs,
                                         int obj_base, int center, int normalize)
 {
-    __shared__ double red[3][8];
+    __shared__ double red[3][32];
     const int64_t obj = (int64_t)blockIdx.x + obj_base;
     const int64_t lo = offsets[obj], n = offsets[obj + 1] - lo;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -128,21 +128,33 @@ __global__ void lsp_tensor_stats_kernel(const int64_t* __restrict__ offsets, con
 // ---- pre-pass 2: exclusive scan of ceil(N_t / 16) over the launch's objects (single CTA) -----------------------
 __global__ void lsp_tensor_scan_kernel(const int64_t* __restrict__ offsets, TensorObj* __restrict__ objs, int obj_base, int n_obj)
 {
-    __shared__ int64_t part[1024];
-    const int tid = threadIdx.x, nt = blockDim.x;
+    __shared__ int64_t wsum[32];
+    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
     const int per = (n_obj + nt - 1) / nt;
     const int o0 = min(n_obj, tid * per), o1 = min(n_obj, o0 + per);
     int64_t s = 0;
     for (int o = o0; o < o1; ++o) s += tc_n_kb(offsets[obj_base + o + 1] - offsets[obj_base + o]);
-    part[tid] = s;
+    // block-wide exclusive scan of the per-thread totals: warp shuffles, then the warp totals
+    int64_t inc = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int64_t v = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += v;
+    }
+    if (lane == 31) wsum[wid] = inc;
     __syncthreads();
-    if (tid == 0) {
-        int64_t run = 0;
-        for (int i = 0; i < nt; ++i) { const int64_t v = part[i]; part[i] = run; run += v; }
-        objs[n_obj].kb_off = run;              // total number of table blocks
+    if (wid == 0) {
+        int64_t w = (lane < (nt >> 5)) ? wsum[lane] : 0, winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int64_t v = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += v;
+        }
+        wsum[lane] = winc - w;                     // exclusive offset of each warp
+        if (lane == 31) objs[n_obj].kb_off = winc; // total number of table blocks
     }
     __syncthreads();
-    int64_t run = part[tid];
+    int64_t run = wsum[wid] + inc - s;              // exclusive prefix of this thread's first object
     for (int o = o0; o < o1; ++o) {
         objs[o].kb_off = run;
         run += tc_n_kb(offsets[obj_base + o + 1] - offsets[obj_base + o]);
