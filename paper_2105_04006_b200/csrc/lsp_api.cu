@@ -47,11 +47,13 @@ struct lsp_plan {
     DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
     DeviceBuffer stats;           // ObjStats[n_obj]
     DeviceBuffer counter;         // work counter of the persistent kernel
+    DeviceBuffer ws_table;        // tile-independent phasors V, B1, B2 of every observation (factored WS path pre-pass)
     DeviceBuffer tc_objs;         // TensorObj[n_obj_launch]   (tensor path pre-pass)
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
+    int64_t ws_table_obs = 0;     // observations the table was built for (this call)
     int64_t* h_offsets_pinned = nullptr;
     size_t   h_offsets_cap = 0;
 
@@ -204,9 +206,14 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
         cudaError_t e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return e;
         const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
+        using V2 = typename FactoredCfg<T>::V2;
+        const int64_t rows = p->ws_table_obs + WsCfg<T>::JC;
+        const V2* tabV = (const V2*)p->ws_table.ptr;
+        const V2* tabB1 = tabV + rows * 8;
+        const V2* tabB2 = tabB1 + rows * FactoredCfg<T>::NL;
         kern<<<ctas, kWsThreads, ws_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
                                                           (V4*)sums, n_obj_launch, (long long)grid,
-                                                          (unsigned long long*)p->counter.ptr);
+                                                          (unsigned long long*)p->counter.ptr, tabV, tabB1, tabB2);
     } else if (s.kernel == LSP_KERNEL_FACTORED) {
         auto kern = lsp_factored_kernel<T, FAST>;
         static bool attr_done = false;     // per instantiation
@@ -396,6 +403,32 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
             lsp_object_stats_kernel<float><<<(unsigned)n_obj, 128, 0, st>>>(d_off, (const float*)d_y, (ObjStats*)p->stats.ptr, c.center, c.normalize);
         else
             lsp_object_stats_kernel<double><<<(unsigned)n_obj, 128, 0, st>>>(d_off, (const double*)d_y, (ObjStats*)p->stats.ptr, c.center, c.normalize);
+        LSP_CUDA(p, cudaGetLastError());
+        ++p->n_launches;
+    }
+
+    if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws && total_obs >= 0) {
+        // pre-pass of the factored WS path: tile-independent phasors of every observation, once per call
+        GridParams gq{};
+        gq.f_min = c.f_min;
+        gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
+        gq.n_freq = (int)c.n_freq;
+        p->ws_table_obs = total_obs;
+        const size_t bytes = c.dtype == LSP_F32 ? ws_table_bytes<float>(total_obs) : ws_table_bytes<double>(total_obs);
+        lsp_status e = ensure(p, p->ws_table, bytes);
+        if (e != LSP_OK) return e;
+        const int64_t jc = c.dtype == LSP_F32 ? WsCfg<float>::JC : WsCfg<double>::JC;
+        const int64_t nl = c.dtype == LSP_F32 ? FactoredCfg<float>::NL : FactoredCfg<double>::NL;
+        const int64_t rows = total_obs + jc;
+        const unsigned blocks = (unsigned)std::min<int64_t>((rows * (8 + nl) + 255) / 256, (int64_t)p->sm_count * 32);
+        if (c.dtype == LSP_F32) {
+            float2* v = (float2*)p->ws_table.ptr;
+            if (c.fast_math) lsp_ws_table_kernel<float, true><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+            else lsp_ws_table_kernel<float, false><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+        } else {
+            double2* v = (double2*)p->ws_table.ptr;
+            lsp_ws_table_kernel<double, false><<<blocks, 256, 0, st>>>(gq, (const double*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+        }
         LSP_CUDA(p, cudaGetLastError());
         ++p->n_launches;
     }
@@ -658,7 +691,7 @@ void lsp_destroy(lsp_plan* p)
     for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
-    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
     cudaGetLastError();

@@ -124,13 +124,83 @@ __device__ __forceinline__ WsItem ws_decode(const GridParams& gp, long long item
     return w;
 }
 
+// ---- pre-pass: the tile-independent phasors of every observation --------------------------------------------------
+// v_{g1 j} = e^{2 pi i (8 g1 L df) t_j} (g1 < 8), b_mj = e^{2 pi i (m + 1/2) df t_j} and b2 = b^2 (m < NL) depend on the
+// observation only, not on the frequency tile, so they are evaluated once per call instead of once per (tile, observation)
+// by the producers.  Three planes indexed by the GLOBAL observation number (CSR position), each padded by JC zero rows so a
+// chunk that runs past an object's end still reads finite values (they meet a = 0):
+//   V  [n_obs + JC][8]     complex
+//   B1 [n_obs + JC][NL]    complex, columns already in the consumers' operand order (operand_pos)
+//   B2 [n_obs + JC][NL]
+template <typename T> constexpr size_t ws_table_row_elems() { return 8 + 2 * (size_t)FactoredCfg<T>::NL; }
+template <typename T> constexpr size_t ws_table_bytes(int64_t n_obs)
+{
+    return (size_t)(n_obs + WsCfg<T>::JC) * ws_table_row_elems<T>() * 2 * sizeof(T);
+}
+template <typename T, bool FAST>
+__global__ void __launch_bounds__(256)
+lsp_ws_table_kernel(GridParams gp, const T* __restrict__ t, int64_t n_obs, typename FactoredCfg<T>::V2* __restrict__ tabV,
+                    typename FactoredCfg<T>::V2* __restrict__ tabB1, typename FactoredCfg<T>::V2* __restrict__ tabB2)
+{
+    using C = FactoredCfg<T>;
+    using V2 = typename C::V2;
+    constexpr int NL = C::NL, L = 2 * NL, ROW = 8 + NL;            // phasors evaluated per observation
+    constexpr int NMI = NL / C::TM;
+    const int64_t rows = n_obs + WsCfg<T>::JC;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < rows * ROW; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t j = idx / ROW;
+        const int e = (int)(idx - j * ROW);
+        V2 z;
+        z.x = z.y = T(0);
+        PhaseFreq<T> f;
+        if (e < 8) {
+            if (j < n_obs) {
+                f.set((double)(8 * e) * (double)L * gp.df);
+                T sn, cs;
+                f.template phasor<FAST>(t[j], &sn, &cs);
+                z.x = cs;
+                z.y = sn;
+            }
+            tabV[j * 8 + e] = z;
+        } else {
+            const int m = e - 8;
+            V2 z2 = z;
+            if (j < n_obs) {
+                f.set(((double)m + 0.5) * gp.df);
+                T sn, cs;
+                f.template phasor<FAST>(t[j], &sn, &cs);
+                z.x = cs;
+                z.y = sn;
+                z2.x = fma(cs, cs, -sn * sn);
+                z2.y = T(2) * cs * sn;
+            }
+            const int pos = operand_pos<C::TM, NMI, C::EPC>(m);
+            tabB1[j * NL + pos] = z;
+            tabB2[j * NL + pos] = z2;
+        }
+    }
+}
+
+// 1-D TMA (bulk async copy) global -> shared, completion on an mbarrier's transaction count
+__device__ __forceinline__ void ws_mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void ws_bulk_g2s(void* smem_dst, const void* gmem_src, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
 template <typename T, bool FAST>
 __global__ void __launch_bounds__(kWsThreads, 1)
 lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
                        const T* __restrict__ y, const ObjStats* __restrict__ stats,
                        T* __restrict__ out_power, Best* __restrict__ partials,
                        typename Vec4<T>::type* __restrict__ sums, int64_t n_obj_launch,
-                       long long total_items, unsigned long long* __restrict__ work_counter)
+                       long long total_items, unsigned long long* __restrict__ work_counter,
+                       const typename FactoredCfg<T>::V2* __restrict__ tabV, const typename FactoredCfg<T>::V2* __restrict__ tabB1,
+                       const typename FactoredCfg<T>::V2* __restrict__ tabB2)
 {
     using C = FactoredCfg<T>;
     using V2 = typename C::V2;
@@ -155,7 +225,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     const int tid = threadIdx.x;
     if (tid == 0) {
         for (int s = 0; s < S; ++s) {
-            mbar_init(&full[s], kWsProducers);
+            mbar_init(&full[s], kWsProducers + 1);     // + the expect_tx arrival of the B-operand bulk copies
             mbar_init(&empty[s], kWsConsumers / 32);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -165,31 +235,27 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     if (tid >= kWsConsumers) {
         // =========================================== producers ===============================================
         // a_gj = y_j e^{i alpha_gj} with alpha_gj = 2 pi f(c_g) t_j and g = 8 g1 + g0.  f(c_g) = f(c_g0) + g1 (8 L df), so
-        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}:
-        // a stage of JC = 16 observations needs 2 x 8 x 16 phasors (two per producer thread, phase 1, into a small
-        // scratch) and G x JC complex products (phase 2) instead of G x JC sincos.  The b_mj are evaluated directly.
-        // Sincos calls per thread per stage drop from 12 (FP32) / 10 (FP64) to 6 / 4, and they are the reduced-argument
-        // kind (lsp_common.cuh): in FP64 the library sincospi cost the FP64 pipe a quarter of its cycles.
+        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}.
+        // Only u depends on the frequency tile: v, b and b2 come from the per-call table (lsp_ws_table_kernel).  Per stage a
+        // producer thread evaluates JC/16 phasors u (reduced-argument sincos, lsp_common.cuh) and copies as many v into a small
+        // scratch (phase 1), then forms G JC / 128 complex products a = y u v, a2 = (u v)^2 (phase 2); the b / b2 rows of the
+        // stage are two bulk copies (TMA) from the table straight into the ring, completing on the stage's full barrier.
         const int ptid = tid - kWsConsumers;
         const int gen_g = ptid & (G - 1);
-        const int gen_m = ptid & (NL - 1);
         const int gen_pos_a = operand_pos<TH, NGI, EPC>(gen_g);
-        const int gen_pos_b = operand_pos<TM, NMI, EPC>(gen_m);
         const int p_q = ptid & 7, p_j = ptid >> 3;                                 // phase 1: phasor index, observation
         static_assert(JC % 16 == 0 && kWsProducers == 128 && G == 64, "producer work split");
-        constexpr int NP = JC / 16;                                                // (u, v) pairs per thread per chunk
-        PhaseFreq<T> f_u, f_v, f_b;
-        f_v.set((double)(8 * p_q) * (double)L * gp.df);                            // v_{g1 = p_q}
-        f_b.set(((double)gen_m + 0.5) * gp.df);                                    // (m + 1/2) df
+        constexpr int NP = JC / 16;                                                // u phasors per thread per chunk
+        PhaseFreq<T> f_u;
         constexpr int NA = (G * JC) / kWsProducers;                                // a-elements per thread per chunk
-        constexpr int NB = (NL * JC + kWsProducers - 1) / kWsProducers;            // b-elements per thread per chunk
+        constexpr unsigned B_BYTES = (unsigned)(JC * NL * sizeof(V2));             // one of the two B planes of a stage
         long long item = blockIdx.x;      // first item is static; the rest come from the global counter
         unsigned c = 0;
         while (true) {
             if (item >= total_items) {
                 const int s = c % S;
                 mbar_wait(&empty[s], ((c / S) & 1) ^ 1);
-                if (ptid == 0) { meta[s].item = -1; meta[s].last = 1; }
+                if (ptid == 0) { meta[s].item = -1; meta[s].last = 1; mbar_arrive(&full[s]); }      // stands in for the expect_tx arrival
                 mbar_arrive(&full[s]);
                 break;
             }
@@ -201,19 +267,16 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             do {      // at least one chunk per item, so empty objects still reach the epilogue
                 // loads first, so their latency overlaps the phase-1 arithmetic and the wait for a free stage
                 T t1[NP], y1[NP];
+                V2 v1[NP];
 #pragma unroll
                 for (int h = 0; h < NP; ++h) {
-                    const bool live1 = (jb + p_j + 16 * h) < w.j1;
-                    t1[h] = live1 ? t[w.lo + jb + p_j + 16 * h] : T(0);
-                    y1[h] = (live1 && p_q == 0) ? y[w.lo + jb + p_j + 16 * h] - mean : T(0);
+                    const int64_t j = jb + p_j + 16 * h;
+                    const bool live1 = j < w.j1;
+                    t1[h] = live1 ? t[w.lo + j] : T(0);
+                    y1[h] = (live1 && p_q == 0) ? y[w.lo + j] - mean : T(0);
+                    v1[h] = tabV[(w.lo + j) * 8 + p_q];                              // padded table: always in range, finite
                 }
-                T tb[NB];
-#pragma unroll
-                for (int it = 0; it < NB; ++it) {
-                    const int64_t j = jb + (ptid + it * kWsProducers) / NL;
-                    tb[it] = (j < w.j1) ? t[w.lo + j] : T(0);
-                }
-                // ---- phase 1: u and v of (p_q, p_j + 16 h) into the scratch (zero beyond the item's range)
+                // ---- phase 1: u of (p_q, p_j + 16 h) (zero beyond the item's range) and v into the scratch
                 V2* sU = scratch + (size_t)(c & 1) * SCR;                            // [JC][8]
                 V2* sV = sU + JC * 8;                                                // [JC][8]
                 T* sY = reinterpret_cast<T*>(sV + JC * 8);                           // [JC]
@@ -221,15 +284,12 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 for (int h = 0; h < NP; ++h) {
                     const bool live1 = (jb + p_j + 16 * h) < w.j1;
                     T sn, cs;
-                    V2 u, v;
+                    V2 u;
                     f_u.template phasor<FAST>(t1[h], &sn, &cs);
                     u.x = live1 ? cs : T(0);
                     u.y = live1 ? sn : T(0);
-                    f_v.template phasor<FAST>(t1[h], &sn, &cs);
-                    v.x = cs;
-                    v.y = sn;
                     sU[(p_j + 16 * h) * 8 + p_q] = u;
-                    sV[(p_j + 16 * h) * 8 + p_q] = v;
+                    sV[(p_j + 16 * h) * 8 + p_q] = v1[h];
                     if (p_q == 0) sY[p_j + 16 * h] = y1[h];
                 }
                 named_bar_sync(1, kWsProducers);
@@ -239,6 +299,11 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 V2* sA2 = sA1 + JC * G;
                 V2* sB1 = sA2 + JC * G;
                 V2* sB2 = sB1 + JC * NL;
+                if (ptid == 0) {          // b, b2 rows of observations [jb, jb + JC) of this object: table -> ring (async proxy)
+                    ws_mbar_arrive_expect_tx(&full[s], 2 * B_BYTES);
+                    ws_bulk_g2s(sB1, tabB1 + (w.lo + jb) * NL, B_BYTES, &full[s]);
+                    ws_bulk_g2s(sB2, tabB2 + (w.lo + jb) * NL, B_BYTES, &full[s]);
+                }
                 // ---- phase 2: a = y u v, a2 = (u v)^2 for this thread's group and NA observations
 #pragma unroll
                 for (int it = 0; it < NA; ++it) {
@@ -255,21 +320,6 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                     a2.y = T(2) * ec * es;
                     sA1[jj * G + gen_pos_a] = a1;
                     sA2[jj * G + gen_pos_a] = a2;
-                }
-#pragma unroll
-                for (int it = 0; it < NB; ++it) {
-                    const int e = ptid + it * kWsProducers;
-                    if ((NL * JC) % kWsProducers != 0 && e >= NL * JC) break;
-                    const int jj = e / NL;
-                    T sn, cs;
-                    f_b.template phasor<FAST>(tb[it], &sn, &cs);
-                    V2 b1, b2;
-                    b1.x = cs;                        // b  = e^{i beta}
-                    b1.y = sn;
-                    b2.x = fma(cs, cs, -sn * sn);     // b2 = e^{2 i beta}
-                    b2.y = T(2) * cs * sn;
-                    sB1[jj * NL + gen_pos_b] = b1;
-                    sB2[jj * NL + gen_pos_b] = b2;
                 }
                 jb += JC;
                 if (ptid == 0) { meta[s].item = item; meta[s].last = (jb >= w.j1) ? 1 : 0; }
