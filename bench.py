@@ -43,6 +43,11 @@ TENSOR_PRODUCTS = {False: 3, True: 1}
 TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 burst; fp16 : bf16 nominal ratio is 1)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel on config 2, from the committed
+# `ncu --set full` captures (profiles/r01_ncu_full_*.csv; commands in profiles/r01_README.md).  Other workloads: null.
+NCU_TRAFFIC_C2 = {("tensor", False): 21.87e6 + 58.68e6, ("factored", "f32"): 5.94e6 + 0.37e6, ("factored", "f64"): 6.65e6 + 42.69e6}
+
+
 def measured_tensor_peak():
     """(TFLOP/s, provenance) -- the driver-written cuBLAS bf16 burst figure; FP16 runs at the same nominal rate."""
     try:
@@ -52,15 +57,18 @@ def measured_tensor_peak():
         return TENSOR_PEAK_FALLBACK, "of fallback (B200_PROFILING.md 1.59 PFLOP/s bf16 burst; fp16:bf16 = 1)"
 
 
-def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float):
+def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float, workload: str = ""):
     """Roofline object of the dominant kernel: achieved = algorithmic flop per launch
     (8 flop per (t,f) pair x pairs) / mean launch duration measured with CUDA events on the launching stream."""
     achieved = pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
+    traffic = None
+    if workload == "c2":
+        traffic = NCU_TRAFFIC_C2.get((kernel, bool(fast)) if kernel == "tensor" else (kernel, dtype))
     if kernel == "tensor":
         peak, prov = measured_tensor_peak()
         prod = TENSOR_PRODUCTS[bool(fast)]
         return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
+                "traffic": traffic, "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
                 "peak_is": prov,
                 "executed_flop_per_pair": FLOP_PER_PAIR * prod,
                 "executed_tflops": achieved * prod, "frac_executed": achieved * prod / peak,
@@ -70,7 +78,7 @@ def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pip
     if kernel != "factored":       # direct kernel (tiny grids): XU/issue bound, no flop roofline claimed
         return {"bound": "alu", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
                 "kernel": "lsp_direct_kernel", "flop_per_pair": None}
-    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+    return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
             "kernel": "lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double"),
             "flop_per_pair": FLOP_PER_PAIR,
             "peak_is": "derived: 148 SMs x %d %s FMA lanes/clk/SM x 2 flop x 1965 MHz (clocks.max.sm)" % (lanes, "FP32" if dtype == "f32" else "FP64"),
@@ -359,7 +367,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
         "kernel": info["kernel"], "n_split": info["n_split"], "fast_math": fast,
         "kernel_ms_per_step": k_ms,
         "gpu_launches": dev_launches,
-        "roofline": roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops),
+        "roofline": roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, args.workload),
     }
     if with_e2e:
         e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, args.steps, args.warmup, flush)
