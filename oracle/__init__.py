@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "lsp_oracle.c")
+_SRC_GLS = os.path.join(_HERE, "gls_oracle.c")      # generalised LSP (floating mean + errors)
 _LIB = os.path.join(_HERE, "liblsp_oracle.so")
 _lib = None
 
@@ -26,9 +27,9 @@ _f64p = ctypes.POINTER(ctypes.c_double)
 
 def build(force: bool = False) -> str:
     """Compile oracle/lsp_oracle.c -> oracle/liblsp_oracle.so if missing or stale."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC), os.path.getmtime(_SRC_GLS)):
         tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, _SRC_GLS, "-lm"])
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -45,6 +46,9 @@ def _load():
         lib.lsp_oracle_best.argtypes = [ctypes.c_int64, _i64p, ctypes.c_int64, _f64p, ctypes.c_double, ctypes.c_double,
                                         _i64p, _f64p, _f64p]
         lib.lsp_oracle_best.restype = None
+        lib.gls_oracle_periodogram.argtypes = [ctypes.c_int64, _i64p, _f64p, _f64p, _f64p, ctypes.c_double, ctypes.c_double,
+                                               ctypes.c_int64, ctypes.c_int64, _i64p, _f64p, ctypes.c_int]
+        lib.gls_oracle_periodogram.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -102,3 +106,23 @@ def best(offsets, power, f_min: float, f_max: float, n_freq: int):
     lib.lsp_oracle_best(n_obj, _p(off, _i64p), int(n_freq), _p(pw, _f64p), float(f_min), float(f_max),
                         _p(idx, _i64p), _p(bp, _f64p), _p(per, _f64p))
     return idx, bp, per
+
+
+def periodogram_generalized(offsets, t, y, sigma, f_min: float, f_max: float, n_freq: int, *, k_list=None, n_threads: int = 0):
+    """Generalised LSP (floating mean, weights sigma^-2) of a CSR batch: P = (chi0^2 - chi^2(f)) / chi0^2 in [0, 1]
+    (oracle/gls_oracle.c; PAPER.md:L31, L417-419).  power[n_obj, n_k] in FP64."""
+    lib = _load()
+    off = np.ascontiguousarray(offsets, dtype=np.int64)
+    tt = np.ascontiguousarray(t, dtype=np.float64)
+    yy = np.ascontiguousarray(y, dtype=np.float64)
+    ss = np.ascontiguousarray(sigma, dtype=np.float64)
+    n_obj = int(off.size - 1)
+    if off[0] != 0 or int(off[-1]) != tt.size or tt.size != yy.size or tt.size != ss.size:
+        raise ValueError("bad CSR batch")
+    kl = None if k_list is None else np.ascontiguousarray(k_list, dtype=np.int64)
+    n_k = int(n_freq) if kl is None else int(kl.size)
+    out = np.empty((n_obj, n_k), dtype=np.float64)
+    if lib.gls_oracle_periodogram(n_obj, _p(off, _i64p), _p(tt, _f64p), _p(yy, _f64p), _p(ss, _f64p), float(f_min), float(f_max),
+                                  int(n_freq), n_k, _p(kl, _i64p), _p(out, _f64p), int(n_threads)) < 0:
+        raise ValueError("gls_oracle_periodogram: bad argument")
+    return out
