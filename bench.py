@@ -482,6 +482,42 @@ def run_c5(args, pkg, torch, device, flush):
     return rows
 
 
+def run_generalized(args, pkg, torch, device, flush, dtype: str):
+    """The generalised mode (floating mean + errors) on the same workload, device-resident: pairs/s counts
+    N_t x N_f once (the paper's convention: it quotes the generalised periodogram as 2.06-2.14x the standard one's time)."""
+    import numpy as np
+    w = workload_for(args.workload, dtype, 0)
+    dev = torch.device("cuda", device)
+    rng = np.random.Generator(np.random.PCG64(977))
+    sigma = (0.2 * rng.uniform(0.5, 2.0, w.n_obs)).astype(w.t.dtype)
+    plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, dtype, device=device)
+    h_off = torch.from_numpy(w.offsets)
+    d_off, d_t, d_y, d_s = h_off.to(dev), torch.from_numpy(w.t).to(dev), torch.from_numpy(w.y).to(dev), torch.from_numpy(sigma).to(dev)
+    best_only = args.workload == "c3"
+    out = None if best_only else torch.empty((w.n_obj, w.n_freq), dtype=d_t.dtype, device=dev)
+    steps = max(3, min(args.steps, 10))
+
+    def step():
+        plan.periodogram_generalized(d_off, d_t, d_y, d_s, out=out, best=best_only, want_power=not best_only, h_offsets=h_off)
+
+    for _ in range(3):
+        step()
+    torch.cuda.synchronize()
+    tot = 0.0
+    for _ in range(steps):
+        flush()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        step()
+        b.record()
+        torch.cuda.synchronize()
+        tot += a.elapsed_time(b)
+    info = plan.last_call_info()
+    plan.destroy()
+    return {"dtype": dtype, "value": w.pairs * steps / (tot * 1e-3), "unit": UNIT, "ms_per_step": tot / steps, "steps": steps,
+            "kernel": info["kernel"], "gpu_launches": info["launches"] * steps}
+
+
 def run_b200(args, rank: int, world: int, local_rank: int):
     import torch
     if not torch.cuda.is_available():
@@ -525,6 +561,14 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                                                    kernel="factored", fast=False, with_e2e=False)
             variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
                                                     kernel="auto", fast=True, with_e2e=False)
+    gls = None
+    if not args.no_secondary and args.workload in ("c2", "c3") and rank == 0 and world == 1:
+        gls = {}
+        for dt in (("f32", "f64") if args.workload == "c2" else ("f32",)):
+            g = run_generalized(args, pkg, torch, local_rank, flush, dt)
+            std_ms = primary["ms_per_step"] if dt == primary["dtype"] else (other["ms_per_step"] if other else None)
+            g["time_vs_standard_same_dtype"] = (g["ms_per_step"] / std_ms) if std_ms else None
+            gls[dt] = g
     overlap = None
     if args.workload == "c4" and rank == 0 and world == 1:
         overlap = c4_overlap(args, pkg, torch, local_rank, flush)
@@ -550,6 +594,8 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                                                                   "gpu_launches", "kernel")}
         for name, v in variants.items():
             line[name] = {k: v[k] for k in ("value", "ms_per_step", "kernel_ms_per_step", "roofline", "gpu_launches", "kernel")}
+        if gls:
+            line["generalized"] = gls
         if overlap is not None:
             line["d2h_overlap"] = overlap
         if cpu is not None:

@@ -122,6 +122,29 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj,
                            void* cuda_stream);
 
 /*
+ * Generalised Lomb-Scargle periodogram: floating mean + per-point errors (section 4.11; Zechmeister &
+ * Kuerster 2009).  With weights w_j = sigma_j^-2 / sum sigma^-2 the output is the relative chi^2 reduction
+ *     P(f_k) = (chi0^2 - chi^2(f_k)) / chi0^2  in [0, 1],
+ * chi0^2 of the weighted-mean model, chi^2(f) of the weighted least-squares fit a cos 2 pi f t + b sin 2 pi f t + c
+ * (reading a15).  Same grid, layout and best-period conventions as lsp_periodogram_batched; `center` and
+ * `normalize` of the plan do not apply (the mean floats; the power is normalised by construction).
+ *   d_sigma      DEVICE, offsets[n_obj] elements of the plan's dtype, all > 0 (1-sigma errors of y).
+ *   d_out_power  DEVICE, n_obj * n_freq elements, or NULL when only the best period is wanted.
+ *   d_best_*     DEVICE, n_obj elements each: all three or none.
+ * Asynchronous on cuda_stream.  Runs the standard contraction kernels three times (sums of w (y - ybar) e^{i theta},
+ * w e^{i theta} and w e^{2 i theta}) and one combine kernel: about 3x the cost of lsp_periodogram_batched.
+ * kernel = AUTO selects as lsp_periodogram_batched does, except that it falls back from the tensor-core kernel to the FMA-pipe
+ * one when the batch's operand table would exceed the plan's budget (LSP_ERR_UNSUPPORTED if kernel = TENSOR was forced).
+ * Other errors as lsp_periodogram_batched.
+ */
+lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj,
+                                       const int64_t* d_offsets, const int64_t* h_offsets,
+                                       const void* d_t, const void* d_y, const void* d_sigma,
+                                       void* d_out_power,
+                                       void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                                       void* cuda_stream);
+
+/*
  * End-to-end form of the two calls above for callers whose data lives on the HOST (the paper's own call
  * shape: H2D of the concatenated (t, y) arrays, kernel, D2H of periodograms and/or periods,
  * PAPER.md:L85-91, L103-117).  Every pointer is a HOST pointer (pinned memory lets the copies overlap;

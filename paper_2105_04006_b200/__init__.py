@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     lsp_destroy,
     lsp_periodogram_batched,
     lsp_periodogram_batched_host,
+    lsp_periodogram_generalized,
     lsp_pipe_peak,
     lsp_plan_create,
     lsp_version,

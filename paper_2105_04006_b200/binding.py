@@ -23,7 +23,8 @@ _KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LS
             "tensor": LSP_KERNEL_TENSOR}
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
-EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host", "lsp_destroy",
+EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host",
+           "lsp_periodogram_generalized", "lsp_destroy",
            "lsp_last_error",
            "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_pipe_peak", "lsp_version")
 
@@ -64,6 +65,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_best_period.restype = ctypes.c_int
     lib.lsp_periodogram_batched_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsp_periodogram_batched_host.restype = ctypes.c_int
+    lib.lsp_periodogram_generalized.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.lsp_periodogram_generalized.restype = ctypes.c_int
     lib.lsp_destroy.argtypes = [vp]
     lib.lsp_destroy.restype = None
     lib.lsp_last_error.argtypes = [vp]
@@ -129,6 +132,15 @@ def lsp_periodogram_batched_host(plan, n_obj: int, h_offsets, h_t, h_y, h_out_po
     _check(load_library().lsp_periodogram_batched_host(plan, int(n_obj), _dptr(h_offsets), _dptr(h_t), _dptr(h_y),
                                                        _dptr(h_out_power), _dptr(h_best_period), _dptr(h_best_power),
                                                        _dptr(h_best_index), _stream_ptr(stream)), plan)
+
+
+def lsp_periodogram_generalized(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y, d_sigma, d_out_power=None,
+                                d_best_period=None, d_best_power=None, d_best_index=None, stream=None) -> None:
+    """Generalised LSP (floating mean + errors; include/lsp.h): device tensors, asynchronous on `stream`."""
+    h_ptr = None if h_offsets is None else ctypes.c_void_p(h_offsets.data_ptr())
+    _check(load_library().lsp_periodogram_generalized(plan, int(n_obj), _dptr(d_offsets), h_ptr, _dptr(d_t), _dptr(d_y),
+                                                      _dptr(d_sigma), _dptr(d_out_power), _dptr(d_best_period),
+                                                      _dptr(d_best_power), _dptr(d_best_index), _stream_ptr(stream)), plan)
 
 
 def lsp_destroy(plan) -> None:
@@ -251,6 +263,25 @@ class Plan:
                 raise TypeError("best_out must be host tensors (period, power, index[int64]) of n_obj elements")
         lsp_periodogram_batched_host(self._plan, n_obj, h_offsets, h_t, h_y, host_out, bp, bw, bi, stream)
         return host_out, best_out
+
+    def periodogram_generalized(self, offsets, t, y, sigma, *, out=None, best: bool = False, want_power: bool = True,
+                                h_offsets=None, stream=None):
+        """Generalised LSP: (power [n_obj, n_freq] or None, best = (period, power, index) or None), device tensors."""
+        n_obj = self._check_inputs(offsets, t, y)
+        if sigma.dtype != self.torch_dtype or not sigma.is_cuda or not sigma.is_contiguous() or sigma.numel() != y.numel():
+            raise TypeError("sigma must be a contiguous CUDA tensor like y")
+        power = None
+        if want_power:
+            power = out if out is not None else torch.empty((n_obj, self.n_freq), dtype=self.torch_dtype, device=self.device)
+            if not power.is_cuda or power.dtype != self.torch_dtype or power.numel() != n_obj * self.n_freq or not power.is_contiguous():
+                raise TypeError("out must be a contiguous CUDA tensor [n_obj, n_freq] of the plan dtype")
+        bp = bw = bi = None
+        if best:
+            bp = torch.empty(n_obj, dtype=self.torch_dtype, device=self.device)
+            bw = torch.empty(n_obj, dtype=self.torch_dtype, device=self.device)
+            bi = torch.empty(n_obj, dtype=torch.int64, device=self.device)
+        lsp_periodogram_generalized(self._plan, n_obj, offsets, h_offsets, t, y, sigma, power, bp, bw, bi, stream)
+        return power, ((bp, bw, bi) if best else None)
 
     def best_period(self, offsets, t, y, *, out=None, h_offsets=None, stream=None):
         """Fused best period: (period, power, index) device tensors; the periodogram is never materialised."""

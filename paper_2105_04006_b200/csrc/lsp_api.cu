@@ -18,6 +18,7 @@
 
 #include "lsp_factored_ws.cuh"
 #include "lsp_tensor.cuh"
+#include "lsp_gls.cuh"
 #include "lsp_peak.cuh"
 
 using namespace lsp;
@@ -54,6 +55,7 @@ struct lsp_plan {
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
+    DeviceBuffer gls_x, gls_yy, gls_sums;        // generalised mode: x_A / x_B arrays, chi0^2 per object, 3 passes of partial sums
     int64_t* h_offsets_pinned = nullptr;
     size_t   h_offsets_cap = 0;
 
@@ -238,7 +240,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 // `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed globally.
 lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
                      const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
-                     cudaStream_t st)
+                     cudaStream_t st, void* ext_sums = nullptr)      // ext_sums: write partial sums there and stop (generalised mode)
 {
     const lsp_config& c = p->cfg;
     if (s.kernel == LSP_KERNEL_TENSOR) {
@@ -278,7 +280,9 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
     const ObjStats* stats = (c.center || c.normalize) ? (const ObjStats*)p->stats.ptr : nullptr;
     void* sums = nullptr;
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
-    if (s.n_split > 1) {
+    if (ext_sums) {
+        sums = ext_sums;
+    } else if (s.n_split > 1) {
         const size_t need = (size_t)s.n_split * n_obj_launch * c.n_freq * 4 * elem_size(c);
         lsp_status e = ensure(p, p->sums, need);
         if (e != LSP_OK) return e;
@@ -319,7 +323,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
     ++p->n_launches;
     if (ev1) LSP_CUDA(p, cudaEventRecord(ev1, st));
 
-    if (s.n_split > 1) {
+    if (s.n_split > 1 && !ext_sums) {
         const int64_t grid = n_obj_launch * n_cparts;
         if (c.dtype == LSP_F32)
             lsp_combine_kernel<float><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, d_off, stats, (const float4*)sums, (float*)out,
@@ -352,6 +356,37 @@ lsp_status run_finalize(lsp_plan* p, int64_t obj_base, int64_t n_obj_launch, int
     else
         lsp_finalize_best_kernel<double><<<grid, wpb * 32, 0, st>>>(gp, d_off, (const Best*)p->partials.ptr, n_parts, n_obj_launch,
                                                                     (double*)d_best_period, (double*)d_best_power, d_best_index);
+    LSP_CUDA(p, cudaGetLastError());
+    ++p->n_launches;
+    return LSP_OK;
+}
+
+// Pre-pass of the factored WS path: tile-independent phasors of every observation on the plan's CURRENT grid, once per call
+// (per pass in the generalised mode).
+lsp_status build_ws_table(lsp_plan* p, const Schedule& s, const void* d_t, int64_t total_obs, cudaStream_t st)
+{
+    const lsp_config& c = p->cfg;
+    if (!(s.kernel == LSP_KERNEL_FACTORED && p->use_ws)) return LSP_OK;
+    GridParams gq{};
+    gq.f_min = c.f_min;
+    gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gq.n_freq = (int)c.n_freq;
+    p->ws_table_obs = total_obs;
+    const size_t bytes = c.dtype == LSP_F32 ? ws_table_bytes<float>(total_obs) : ws_table_bytes<double>(total_obs);
+    lsp_status e = ensure(p, p->ws_table, bytes);
+    if (e != LSP_OK) return e;
+    const int64_t jc = c.dtype == LSP_F32 ? WsCfg<float>::JC : WsCfg<double>::JC;
+    const int64_t nl = c.dtype == LSP_F32 ? FactoredCfg<float>::NL : FactoredCfg<double>::NL;
+    const int64_t rows = total_obs + jc;
+    const unsigned blocks = (unsigned)std::min<int64_t>((rows * (8 + nl) + 255) / 256, (int64_t)p->sm_count * 32);
+    if (c.dtype == LSP_F32) {
+        float2* v = (float2*)p->ws_table.ptr;
+        if (c.fast_math) lsp_ws_table_kernel<float, true><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+        else lsp_ws_table_kernel<float, false><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+    } else {
+        double2* v = (double2*)p->ws_table.ptr;
+        lsp_ws_table_kernel<double, false><<<blocks, 256, 0, st>>>(gq, (const double*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
+    }
     LSP_CUDA(p, cudaGetLastError());
     ++p->n_launches;
     return LSP_OK;
@@ -407,30 +442,9 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         ++p->n_launches;
     }
 
-    if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws && total_obs >= 0) {
-        // pre-pass of the factored WS path: tile-independent phasors of every observation, once per call
-        GridParams gq{};
-        gq.f_min = c.f_min;
-        gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
-        gq.n_freq = (int)c.n_freq;
-        p->ws_table_obs = total_obs;
-        const size_t bytes = c.dtype == LSP_F32 ? ws_table_bytes<float>(total_obs) : ws_table_bytes<double>(total_obs);
-        lsp_status e = ensure(p, p->ws_table, bytes);
+    {
+        lsp_status e = build_ws_table(p, s, d_t, total_obs, st);
         if (e != LSP_OK) return e;
-        const int64_t jc = c.dtype == LSP_F32 ? WsCfg<float>::JC : WsCfg<double>::JC;
-        const int64_t nl = c.dtype == LSP_F32 ? FactoredCfg<float>::NL : FactoredCfg<double>::NL;
-        const int64_t rows = total_obs + jc;
-        const unsigned blocks = (unsigned)std::min<int64_t>((rows * (8 + nl) + 255) / 256, (int64_t)p->sm_count * 32);
-        if (c.dtype == LSP_F32) {
-            float2* v = (float2*)p->ws_table.ptr;
-            if (c.fast_math) lsp_ws_table_kernel<float, true><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
-            else lsp_ws_table_kernel<float, false><<<blocks, 256, 0, st>>>(gq, (const float*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
-        } else {
-            double2* v = (double2*)p->ws_table.ptr;
-            lsp_ws_table_kernel<double, false><<<blocks, 256, 0, st>>>(gq, (const double*)d_t, total_obs, v, v + rows * 8, v + rows * (8 + nl));
-        }
-        LSP_CUDA(p, cudaGetLastError());
-        ++p->n_launches;
     }
 
     int n_parts = 0;
@@ -627,6 +641,118 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj, const int64_t* d_offse
                     cuda_stream);
 }
 
+lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
+                                       const void* d_t, const void* d_y, const void* d_sigma, void* d_out_power,
+                                       void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
+{
+    lsp_plan* p = plan;
+    if (!p) return LSP_ERR_INVALID_ARG;
+    p->n_launches = p->n_pairs = p->n_chunks = 0;
+    p->t_used = 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
+    const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
+    if (n_best != 0 && n_best != 3) return fail(p, LSP_ERR_INVALID_ARG, "best_period/best_power/best_index: give all three or none");
+    const bool want_best = n_best == 3;
+    if (n_obj == 0) return LSP_OK;
+    if (!d_out_power && !want_best) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
+    if (!d_offsets) return fail(p, LSP_ERR_INVALID_ARG, "d_offsets is NULL");
+    if (n_obj > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "n_obj too large");
+    LSP_CUDA(p, cudaSetDevice(p->cfg.device));
+    int64_t total_obs;
+    if (h_offsets) {
+        if (h_offsets[0] != 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[0] != 0");
+        for (int64_t o = 0; o < n_obj; ++o)
+            if (h_offsets[o + 1] < h_offsets[o]) return fail(p, LSP_ERR_INVALID_ARG, "offsets decrease at object %lld", (long long)o);
+        total_obs = h_offsets[n_obj];
+    } else {
+        if (!p->h_offsets_pinned) LSP_CUDA(p, cudaMallocHost((void**)&p->h_offsets_pinned, sizeof(int64_t)));
+        LSP_CUDA(p, cudaMemcpyAsync(p->h_offsets_pinned, d_offsets + n_obj, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaStreamSynchronize(st));
+        total_obs = p->h_offsets_pinned[0];
+        if (total_obs < 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[n_obj] < 0");
+    }
+    if (total_obs > 0 && (!d_t || !d_y || !d_sigma)) return fail(p, LSP_ERR_INVALID_ARG, "d_t / d_y / d_sigma is NULL");
+
+    // The three passes run the standard kernels on derived inputs: y is already weighted and centred (center / normalize off),
+    // pass C runs on the doubled grid.  The configuration is restored before returning.
+    const lsp_config saved = p->cfg;
+    struct Restore { lsp_plan* p; lsp_config c; ~Restore() { p->cfg = c; } } restore{p, saved};
+    p->cfg.center = p->cfg.normalize = 0;
+    const lsp_config& c = p->cfg;
+    const size_t es = elem_size(c);
+    lsp_status e;
+    if ((e = ensure(p, p->gls_x, std::max<size_t>(16, (size_t)2 * total_obs * es))) != LSP_OK) return e;
+    if ((e = ensure(p, p->gls_yy, (size_t)n_obj * sizeof(double))) != LSP_OK) return e;
+    void* xa = p->gls_x.ptr;
+    void* xb = (char*)p->gls_x.ptr + (size_t)total_obs * es;
+    if (c.dtype == LSP_F32)
+        lsp_gls_prep_kernel<float><<<(unsigned)n_obj, 256, 0, st>>>(d_offsets, (const float*)d_y, (const float*)d_sigma, (float*)xa, (float*)xb, (double*)p->gls_yy.ptr);
+    else
+        lsp_gls_prep_kernel<double><<<(unsigned)n_obj, 256, 0, st>>>(d_offsets, (const double*)d_y, (const double*)d_sigma, (double*)xa, (double*)xb, (double*)p->gls_yy.ptr);
+    LSP_CUDA(p, cudaGetLastError());
+    ++p->n_launches;
+
+    Schedule s = make_schedule(p, n_obj, total_obs);
+    if (s.kernel == LSP_KERNEL_TENSOR &&
+        (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget) {
+        // the tensor path's operand table of the whole batch does not fit: AUTO falls back to the FMA-pipe kernel
+        if (saved.kernel != LSP_KERNEL_AUTO)
+            return fail(p, LSP_ERR_UNSUPPORTED, "generalised mode on the tensor path: batch too large for the operand table (use kernel = factored)");
+        p->cfg.kernel = LSP_KERNEL_FACTORED;
+        s = make_schedule(p, n_obj, total_obs);
+    }
+    s.n_split = std::max(2, s.n_split);           // the split form is the one that leaves sums, not powers, in memory
+    p->kernel_used = s.kernel;
+    p->n_split = s.n_split;
+    p->n_pairs = 3 * total_obs * c.n_freq;
+    // objects per round so that the three sums buffers stay within ~12 GB
+    const size_t per_obj = (size_t)3 * s.n_split * c.n_freq * 4 * es;
+    const int64_t objs_per_round = std::max<int64_t>(1, (int64_t)(((size_t)12 << 30) / per_obj));
+    const size_t row_bytes = (size_t)c.n_freq * es;
+    const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
+    for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_round) {
+        const int64_t no = std::min(objs_per_round, n_obj - o0);
+        const size_t pass_bytes = (size_t)s.n_split * no * c.n_freq * 4 * es;
+        if ((e = ensure(p, p->gls_sums, 3 * pass_bytes)) != LSP_OK) return e;
+        int n_parts = 0;
+        for (int pass = 0; pass < 3; ++pass) {
+            p->cfg.f_min = saved.f_min * (pass == 2 ? 2.0 : 1.0);
+            p->cfg.f_max = saved.f_max * (pass == 2 ? 2.0 : 1.0);
+            if ((e = build_ws_table(p, s, d_t, total_obs, st)) != LSP_OK) return e;
+            e = run_range(p, s, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st,
+                          (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes);
+            if (e != LSP_OK) return e;
+        }
+        p->cfg.f_min = saved.f_min;
+        p->cfg.f_max = saved.f_max;
+        GridParams gp;
+        gp.f_min = c.f_min;
+        gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+        gp.n_freq = (int)c.n_freq;
+        gp.n_tiles = s.n_tiles;
+        gp.n_split = s.n_split;
+        gp.obj_base = (int)o0;
+        if (want_best && (e = ensure(p, p->partials, (size_t)no * n_cparts * sizeof(Best))) != LSP_OK) return e;
+        Best* partials = want_best ? (Best*)p->partials.ptr : nullptr;
+        void* out = d_out_power ? (char*)d_out_power + (size_t)o0 * row_bytes : nullptr;
+        const int64_t grid = no * n_cparts;
+        if (c.dtype == LSP_F32) {
+            const float4* sa = (const float4*)p->gls_sums.ptr;
+            lsp_gls_combine_kernel<float><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, (const double*)p->gls_yy.ptr, sa,
+                sa + pass_bytes / sizeof(float4), sa + 2 * (pass_bytes / sizeof(float4)), (float*)out, partials, n_cparts, no);
+        } else {
+            const double4* sa = (const double4*)p->gls_sums.ptr;
+            lsp_gls_combine_kernel<double><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, (const double*)p->gls_yy.ptr, sa,
+                sa + pass_bytes / sizeof(double4), sa + 2 * (pass_bytes / sizeof(double4)), (double*)out, partials, n_cparts, no);
+        }
+        LSP_CUDA(p, cudaGetLastError());
+        ++p->n_launches;
+        if (want_best && (e = run_finalize(p, o0, no, n_cparts, d_offsets, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+    }
+    return LSP_OK;
+}
+
 lsp_status lsp_periodogram_batched_host(lsp_plan* plan, int64_t n_obj, const int64_t* h_offsets, const void* h_t,
                                         const void* h_y, void* h_out_power, void* h_best_period, void* h_best_power,
                                         int64_t* h_best_index, void* cuda_stream)
@@ -691,7 +817,7 @@ void lsp_destroy(lsp_plan* p)
     for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
-    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->gls_x, &p->gls_yy, &p->gls_sums, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
     cudaGetLastError();

@@ -299,3 +299,59 @@ def test_deterministic_and_no_h_offsets(lsp):
         c, _ = plan.periodogram_batched(off, t, y, stream=s)
         s.synchronize()
         assert torch.equal(a, c)
+
+
+# ---- generalised LSP (floating mean + errors) against oracle/gls_oracle.c ---------------------
+def _with_errors(w: Workload, seed: int):
+    """Seeded per-point errors for a workload (heteroscedastic, 0.5x-2x a base sigma) and an offset the floating mean must
+    absorb; drawn in FP64, rounded once to the workload's dtype like t and y."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    base = 0.05 if w.name.startswith(("c3", "c4")) else 0.2
+    sigma = (base * rng.uniform(0.5, 2.0, w.n_obs)).astype(w.t.dtype)
+    y = (w.y.astype(np.float64) + 7.25).astype(w.t.dtype)
+    return y, sigma
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("kernel", ["auto", "direct", "factored", "tensor"])
+def test_generalized_batch_parity(lsp, oracle, dtype, kernel):
+    import torch
+    if kernel == "tensor" and dtype == "f64":
+        pytest.skip("the tensor-core kernel is FP32-mode only")
+    w = make_config(3, n_obj=5, n_freq=6000, dtype=dtype)
+    y, sigma = _with_errors(w, 77)
+    P_ref = oracle.periodogram_generalized(w.offsets, w.t, y, sigma, w.f_min, w.f_max, w.n_freq)
+    off, t, _ = to_device(w)
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, dtype, kernel=kernel) as plan:
+        P, best = plan.periodogram_generalized(off, t, torch.from_numpy(y).cuda(), torch.from_numpy(sigma).cuda(), best=True,
+                                               h_offsets=torch.from_numpy(w.offsets))
+        info = plan.last_call_info()
+        P = P.cpu().numpy().astype(np.float64)
+        best = tuple(x.cpu().numpy() for x in best)
+        # the plan's own grid is restored: a standard call afterwards still matches the standard oracle
+        P_std, _ = plan.periodogram_batched(off, t, to_device(w)[2])
+        assert_power_parity(P_std.cpu().numpy().astype(np.float64), oracle_full(oracle, w), dtype, "standard call after generalised")
+    assert info["n_split"] >= 2
+    assert np.all(P >= -TOL[dtype]) and np.all(P <= 1.0 + TOL[dtype])
+    assert_power_parity(P, P_ref, dtype, f"generalised {kernel}")
+    assert_best_parity(best, P_ref, w, dtype, oracle, f"generalised {kernel}")
+
+
+def test_generalized_single_object_and_edge_cases(lsp, oracle):
+    import torch
+    w = make_config(2, n_t=3000, n_freq=20000, dtype="f64")
+    y, sigma = _with_errors(w, 5)
+    # add an empty object and a single-point object: P = 0 rows
+    off = np.array([0, w.n_obs, w.n_obs, w.n_obs + 1], dtype=np.int64)
+    t = np.concatenate([w.t, w.t[:1]])
+    y = np.concatenate([y, y[:1]])
+    sigma = np.concatenate([sigma, sigma[:1]])
+    P_ref = oracle.periodogram_generalized(off, t, y, sigma, w.f_min, w.f_max, w.n_freq)
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f64") as plan:
+        P, best = plan.periodogram_generalized(torch.from_numpy(off).cuda(), torch.from_numpy(t).cuda(), torch.from_numpy(y).cuda(),
+                                               torch.from_numpy(sigma).cuda(), best=True)
+        P = P.cpu().numpy()
+        _, _, idx = (x.cpu().numpy() for x in best)
+    assert np.max(np.abs(P[0] - P_ref[0])) <= TOL["f64"] * P_ref[0].max()
+    assert np.all(P[1] == 0.0) and np.all(P[2] == 0.0) and idx[1] == -1
+    assert idx[0] == int(np.argmax(P_ref[0]))
