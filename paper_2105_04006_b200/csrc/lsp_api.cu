@@ -52,6 +52,7 @@ struct lsp_plan {
     DeviceBuffer tc_objs;         // TensorObj[n_obj_launch]   (tensor path pre-pass)
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
+    int tc_stages_b = 3;          // B-operand ring depth of the tensor kernel
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
@@ -133,7 +134,9 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
         s.tp.n_ops = c.fast_math ? 2 : 4;
         s.tp.a_stage_bytes = s.tp.n_ops * 128 * kTcKB * 2;
         s.tp.b_stage_bytes = s.tp.n_ops * 2 * (int)nl * kTcKB * 2;
-        s.tp.stages = (int)std::min<int64_t>(8, (int64_t)(p->smem_optin - 24576) / (s.tp.a_stage_bytes + s.tp.b_stage_bytes));
+        // B ring: 3 stages (LSP_TC_SB overrides); A ring: whatever else fits, at most 8
+        s.tp.stages_b = p->tc_stages_b;
+        s.tp.stages = (int)std::max<int64_t>(2, std::min<int64_t>(8, ((int64_t)(p->smem_optin - 18432) - (int64_t)s.tp.stages_b * s.tp.b_stage_bytes) / s.tp.a_stage_bytes));
         s.tile = s.tp.tile;
         s.direct_r = 0;
         slots = p->sm_count;
@@ -183,7 +186,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
     if (s.kernel == LSP_KERNEL_TENSOR) {
         if constexpr (std::is_same<T, float>::value) {
             auto kern = lsp_tensor_kernel<float, FAST>;
-            const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
+            const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.stages_b, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
             static size_t attr_smem = 0;       // per instantiation
             if (smem > attr_smem) {
                 cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -591,6 +594,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     p->sm_count = prop.multiProcessorCount;
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
     if (const char* b = getenv("LSP_TABLE_BUDGET_MB")) p->tc_table_budget = (size_t)std::max(1L, atol(b)) << 20;
+    if (const char* b = getenv("LSP_TC_SB")) p->tc_stages_b = (int)std::min(6L, std::max(2L, atol(b)));
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
         cudaStream_t s;

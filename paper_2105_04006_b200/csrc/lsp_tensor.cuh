@@ -59,7 +59,8 @@ struct TensorParams {
     int nl;             // NL: half-width of a frequency group (multiple of 8, <= 128); group width L = 2 NL = MMA N
     int tile;           // frequencies per tile = 64 * 2 NL
     int n_ops;          // FP16 operand planes per stage side: 4 (accurate: hi and lo of Z- and W-operands) or 2 (fast)
-    int stages;         // ring depth
+    int stages;         // A-operand ring depth (generators -> MMA)
+    int stages_b;       // B-operand ring depth (TMA -> MMA): shallower, the copies are fast and B stages are twice as large
     int b_stage_bytes;  // n_ops * 2 NL * 32
     int a_stage_bytes;  // n_ops * 128 * 32
 };
@@ -330,9 +331,9 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
     return w;
 }
 
-constexpr size_t tc_smem_bytes(int stages, int a_stage, int b_stage)
+constexpr size_t tc_smem_bytes(int stages_a, int stages_b, int a_stage, int b_stage)
 {
-    return 1024 /* alignment slack */ + (size_t)stages * (size_t)(a_stage + b_stage) + 256;
+    return 1024 /* alignment slack */ + (size_t)stages_a * (size_t)a_stage + (size_t)stages_b * (size_t)b_stage + 512;
 }
 
 template <typename T, bool FAST>
@@ -346,12 +347,17 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     constexpr int A_PLANE = 128 * kTcKB * 2;                  // bytes of one A plane: 128 rows x 16 x FP16
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    const int S = tp.stages;
-    const int stage_bytes = tp.a_stage_bytes + tp.b_stage_bytes;
+    // Two rings: A stages (16 KB, written by the generators) and B stages (up to 32 KB, filled by TMA).  The A ring is the
+    // deep one: while the epilogue of a short item holds TMEM, the generators keep building the next item's stages.
+    const int S = tp.stages, SB = tp.stages_b;
+    const int stage_bytes = tp.a_stage_bytes;                 // A ring stride
     const int b_plane = 2 * tp.nl * kTcKB * 2;                // bytes of one B plane
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem + (size_t)S * stage_bytes);
+    unsigned char* smem_b = smem + (size_t)S * tp.a_stage_bytes;
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem_b + (size_t)SB * tp.b_stage_bytes);   // A ring
     unsigned long long* empty = full + 8;
-    unsigned long long* tmem_full = empty + 8;
+    unsigned long long* full_b = empty + 8;                   // B ring
+    unsigned long long* empty_b = full_b + 8;
+    unsigned long long* tmem_full = empty_b + 8;
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
     __shared__ Best sbest[kTcEpiWarps];
@@ -362,8 +368,12 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // broadcast: the compiler may treat the role as warp-uniform
     if (tid == 0) {
         for (int s = 0; s < S; ++s) {
-            mbar_init(&full[s], kTcGenGroupThreads + 1);
+            mbar_init(&full[s], kTcGenGroupThreads);
             mbar_init(&empty[s], 1);
+        }
+        for (int s = 0; s < SB; ++s) {
+            mbar_init(&full_b[s], 1);
+            mbar_init(&empty_b[s], 1);
         }
         mbar_init(tmem_full, 1);
         mbar_init(tmem_empty, kTcEpiThreads);
@@ -385,17 +395,16 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             int st = 0;
             unsigned ph = 1;                                      // parity of the "empty" phase to wait for
             const unsigned b_bytes = (unsigned)tp.b_stage_bytes;
-            unsigned char* dst0 = smem + tp.a_stage_bytes;
             for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
                 const TcItem w = tc_decode(gp, tp, item, offsets);
                 const unsigned char* src = reinterpret_cast<const unsigned char*>(table) +
                                            (size_t)(objs[w.obj_local].kb_off + w.kb0) * (size_t)b_bytes;
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
-                    mbar_wait(&empty[st], ph);
-                    mbar_arrive_expect_tx(&full[st], b_bytes);
-                    tma_bulk_g2s(dst0 + (size_t)st * stage_bytes, src, b_bytes, &full[st]);
+                    mbar_wait(&empty_b[st], ph);
+                    mbar_arrive_expect_tx(&full_b[st], b_bytes);
+                    tma_bulk_g2s(smem_b + (size_t)st * b_bytes, src, b_bytes, &full_b[st]);
                     src += b_bytes;
-                    if (++st == S) { st = 0; ph ^= 1; }
+                    if (++st == SB) { st = 0; ph ^= 1; }
                 }
             }
         }
@@ -408,15 +417,15 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const unsigned a_lbo = 16 * 128, b_lbo = (unsigned)(2 * tp.nl / 8) * 128, sbo = 128;
             // Descriptors of stage 0; stage s adds s * stage_bytes / 16 to the 14-bit start-address field (the whole ring
             // lies below 256 KB, so the field never carries into the LBO bits).
-            const unsigned sa0 = smem_u32(smem), sb0 = sa0 + tp.a_stage_bytes;
+            const unsigned sa0 = smem_u32(smem), sb0 = smem_u32(smem_b);
             const uint64_t a_zh0 = tc_smem_desc(sa0, a_lbo, sbo), a_wh0 = tc_smem_desc(sa0 + A_PLANE, a_lbo, sbo);
             const uint64_t a_zl0 = tc_smem_desc(sa0 + 2 * A_PLANE, a_lbo, sbo), a_wl0 = tc_smem_desc(sa0 + 3 * A_PLANE, a_lbo, sbo);
             const uint64_t b_zh0 = tc_smem_desc(sb0, b_lbo, sbo), b_wh0 = tc_smem_desc(sb0 + b_plane, b_lbo, sbo);
             const uint64_t b_zl0 = tc_smem_desc(sb0 + 2 * b_plane, b_lbo, sbo), b_wl0 = tc_smem_desc(sb0 + 3 * b_plane, b_lbo, sbo);
-            const uint64_t stage_inc = (uint64_t)(stage_bytes >> 4);
-            int st = 0;
-            unsigned ph = 0, n_acc = 0;
-            uint64_t so = 0;                                      // st * stage_inc
+            const uint64_t stage_inc = (uint64_t)(tp.a_stage_bytes >> 4), stage_inc_b = (uint64_t)(tp.b_stage_bytes >> 4);
+            int st = 0, stb = 0;
+            unsigned ph = 0, phb = 0, n_acc = 0;
+            uint64_t so = 0, sob = 0;                             // st * stage_inc, stb * stage_inc_b
             for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
                 const TcItem w = tc_decode(gp, tp, item, offsets);
                 const int kb0 = __shfl_sync(0xffffffffu, w.kb0, 0), kb1 = __shfl_sync(0xffffffffu, w.kb1, 0);
@@ -425,27 +434,31 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 tc_fence_after();
                 unsigned acc = 0;
                 for (int kb = kb0; kb < kb1; ++kb) {
+                    mbar_wait(&full_b[stb], phb);
                     mbar_wait(&full[st], ph);
                     tc_fence_after();
                     if (elect_one()) {
                         // planes: 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
                         if (!FAST) {
-                            tc_mma_f16(tmem, a_zl0 + so, b_zh0 + so, idesc, acc);
-                            tc_mma_f16(tmem, a_zh0 + so, b_zl0 + so, idesc, 1u);
-                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + so, idesc, 1u);
-                            tc_mma_f16(tmem + 256, a_wl0 + so, b_wh0 + so, idesc, acc);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wl0 + so, idesc, 1u);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + so, idesc, 1u);
+                            tc_mma_f16(tmem, a_zl0 + so, b_zh0 + sob, idesc, acc);
+                            tc_mma_f16(tmem, a_zh0 + so, b_zl0 + sob, idesc, 1u);
+                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + sob, idesc, 1u);
+                            tc_mma_f16(tmem + 256, a_wl0 + so, b_wh0 + sob, idesc, acc);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wl0 + sob, idesc, 1u);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + sob, idesc, 1u);
                         } else {
-                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + so, idesc, acc);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + so, idesc, acc);
+                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + sob, idesc, acc);
+                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + sob, idesc, acc);
                         }
-                        tc_commit(&empty[st]);                   // stage st is free once these MMAs have read it
+                        tc_commit(&empty[st]);                   // both stages are free once these MMAs have read them
+                        tc_commit(&empty_b[stb]);
                     }
                     __syncwarp();
                     acc = 1u;
                     so += stage_inc;
+                    sob += stage_inc_b;
                     if (++st == S) { st = 0; ph ^= 1; so = 0; }
+                    if (++stb == SB) { stb = 0; phb ^= 1; sob = 0; }
                 }
                 if (elect_one()) tc_commit(tmem_full);           // accumulators complete
                 __syncwarp();
