@@ -75,9 +75,21 @@ def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pip
                 "note": "FP16 hi+lo split operands: %d tcgen05 products per algorithmic MAC" % prod}
     lanes = FP32_LANES if dtype == "f32" else FP64_LANES
     peak = N_SM * lanes * 2 * SM_MAX_HZ / 1e12
-    if kernel != "factored":       # direct kernel (tiny grids): XU/issue bound, no flop roofline claimed
-        return {"bound": "alu", "achieved": None, "peak": peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
-                "kernel": "lsp_direct_kernel", "flop_per_pair": None}
+    if kernel != "factored":
+        # Paper-shaped direct kernel (SURVEY.md 8(d) "Algorithmic work per pair"): FP32 fast = 2 MUFU per pair against the XU
+        # pipe (16 lanes/clk/SM); FP32 accurate = ~17 FMA-pipe instructions per pair against 128 lanes/clk/SM; FP64 = ~24
+        # FP64-pipe instructions per pair against 64 lanes/clk/SM.  Unit: 1e12 pipe operations per second.
+        if dtype == "f32" and fast:
+            ops, lanes_, what = 2.0, 16, "MUFU (XU pipe)"
+        elif dtype == "f32":
+            ops, lanes_, what = 17.0, 128, "FMA-pipe instructions"
+        else:
+            ops, lanes_, what = 24.0, 64, "FP64-pipe instructions"
+        pk = N_SM * lanes_ * SM_MAX_HZ / 1e12
+        ach = pairs * ops / (k_ms * 1e-3) / 1e12
+        return {"bound": "alu", "achieved": ach, "peak": pk, "unit": "Top/s", "frac": ach / pk, "traffic": None,
+                "kernel": "lsp_direct_kernel", "ops_per_pair": ops,
+                "peak_is": "derived: 148 SMs x %d lanes/clk/SM x 1965 MHz, %s" % (lanes_, what)}
     return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
             "kernel": "lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double"),
             "flop_per_pair": FLOP_PER_PAIR,
@@ -561,6 +573,17 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                                                    kernel="factored", fast=False, with_e2e=False)
             variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
                                                     kernel="auto", fast=True, with_e2e=False)
+            # the paper-shaped kernel (thread = frequency, one sincos per pair): __sincosf-class vs accurate sincos
+            # (PAPER.md:L423-433), the comparison north_star asks for
+            saved_steps = args.steps
+            args.steps = max(3, min(args.steps, 5))
+            variants["direct_fp32_sincosf"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
+                                                         kernel="direct", fast=True, with_e2e=False)
+            variants["direct_fp32_accurate"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
+                                                          kernel="direct", fast=False, with_e2e=False)
+            variants["direct_fp64"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f64", flush, False,
+                                                 kernel="direct", fast=False, with_e2e=False)
+            args.steps = saved_steps
     gls = None
     if not args.no_secondary and args.workload in ("c2", "c3") and rank == 0 and world == 1:
         gls = {}

@@ -355,3 +355,48 @@ def test_generalized_single_object_and_edge_cases(lsp, oracle):
     assert np.max(np.abs(P[0] - P_ref[0])) <= TOL["f64"] * P_ref[0].max()
     assert np.all(P[1] == 0.0) and np.all(P[2] == 0.0) and idx[1] == -1
     assert idx[0] == int(np.argmax(P_ref[0]))
+
+
+# ---- full-size config 4 and config 5 corners, in the launch configurations bench.py times -----------------------
+def test_config4_full_size_sampled(lsp, oracle):
+    """BASELINE config 4 at full size (2,000 objects, N_f = 5e5, 4.0 GB of periodograms to pinned host over the copy streams with
+    the library's default chunking); the oracle checks sampled (object, frequency) values and whole-row properties."""
+    import torch
+    w = make_config(4)
+    off, t, y = to_device(w)
+    host = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32).pin_memory()
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f32") as plan:
+        plan.periodogram_batched(off, t, y, host_out=host, h_offsets=torch.from_numpy(w.offsets))
+        info = plan.last_call_info()
+    assert info["kernel"] == "tensor" and info["chunks"] == -(-w.n_obj // ((64 << 20) // (w.n_freq * 4)))
+    P = host.numpy()
+    rng = np.random.default_rng(44)
+    pick = np.sort(rng.choice(w.n_obj, 6, replace=False))
+    pick = np.unique(np.concatenate([pick, [0, w.n_obj - 1]]))          # first and last chunk too
+    ks = np.unique(np.concatenate([rng.integers(0, w.n_freq, 400), [0, 1, w.n_freq - 2, w.n_freq - 1]])).astype(np.int64)
+    sub = w.take_objects(pick)
+    P_ref = oracle.periodogram(sub.offsets, sub.t, sub.y, w.f_min, w.f_max, w.n_freq, k_list=ks)
+    for i, o in enumerate(pick):
+        row = P[o].astype(np.float64)
+        yy = sub.y[sub.offsets[i]:sub.offsets[i + 1]].astype(np.float64)
+        pmax = max(P_ref[i].max(), float(row.max()))
+        assert np.max(np.abs(row[ks] - P_ref[i])) <= TOL["f32"] * pmax, f"object {o}"
+        assert row.min() >= -TOL["f32"] * pmax and row.max() <= 0.5 * float(yy @ yy) * (1 + TOL["f32"])
+    assert np.isfinite(P[::97]).all()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("n_t,n_freq,point", [(1024, 100_000, 0), (65536, 4_000_000, 11)])
+def test_config5_corner_points_sampled(lsp, oracle, dtype, n_t, n_freq, point):
+    """The smallest and the largest point of BASELINE config 5's sweep at full size; sampled frequencies + the peak window."""
+    w = make_config(5, dtype=dtype, n_t=n_t, n_freq=n_freq, point=point)
+    P, best, info = gpu_full(lsp, w)
+    rng = np.random.default_rng(5 + point)
+    ks = np.unique(np.concatenate([rng.integers(0, n_freq, 96 if n_t > 10000 else 600), [0, n_freq - 1],
+                                   np.clip(np.arange(-8, 9) + int(best[2][0]), 0, n_freq - 1)])).astype(np.int64)
+    P_ref = oracle.periodogram(w.offsets, w.t, w.y, w.f_min, w.f_max, w.n_freq, k_list=ks)
+    pmax = max(P_ref.max(), P[0].max())
+    assert np.max(np.abs(P[0, ks] - P_ref[0])) <= TOL[dtype] * pmax
+    assert abs(P_ref[0].max() - best[1][0]) <= TOL[dtype] * pmax
+    yy = w.y.astype(np.float64)
+    assert P.min() >= -TOL[dtype] * pmax and P.max() <= 0.5 * float(yy @ yy) * (1 + TOL[dtype])
