@@ -94,8 +94,11 @@ lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan
  *                one small synchronous D2H on the call's stream)
  *   d_t, d_y     DEVICE, offsets[n_obj] elements of cfg.dtype: times and magnitudes, concatenated
  *   out_power    n_obj * n_freq elements of cfg.dtype, row-major by object:
- *                a DEVICE pointer when out_is_host == 0, else a HOST pointer (pinned for overlap; pageable
- *                memory works but serialises) filled through the plan's chunk ring and copy streams
+ *                a DEVICE pointer when out_is_host == 0, else a HOST pointer filled through the plan's chunk ring and copy
+ *                streams: a pinned (or registered) buffer is written directly by the async copies and overlaps with compute;
+ *                a pageable one is handed to cudaMemcpyAsync as it is (works, does not overlap), or, with
+ *                LSP_PAGEABLE=staged in the environment at plan creation, goes through a plan-owned pinned staging ring and
+ *                per-chunk host-side copies run by the copy streams' callback threads (PAPER.md:L117's scheme)
  *   d_best_*     DEVICE, optional (all three NULL or all three non-NULL): per object best period
  *                (cfg.dtype), its power (cfg.dtype) and grid index (int64; -1 and NaN period when N_t = 0)
  *   cuda_stream  cudaStream_t as void* (NULL = default stream).  Device-output calls are asynchronous

@@ -44,6 +44,12 @@ struct lsp_plan {
     std::vector<cudaEvent_t> slot_ready, slot_free;
     std::vector<char> slot_used;
     DeviceBuffer ring;            // n_slots * slot_bytes
+    void*  stage_host = nullptr;  // pinned staging ring for a PAGEABLE host destination (n_slots * slot_bytes)
+    size_t stage_host_bytes = 0;
+    struct HostCopy { void* dst; const void* src; size_t bytes; };
+    std::vector<HostCopy> host_copies;           // arguments of the per-chunk host memcpy callbacks (stable during a call)
+    int pageable_mode = 1;        // 1 = plain cudaMemcpyAsync to a pageable destination (default: faster on the measured host),
+                                  // 0 = staged (pinned ring + host-side copies; LSP_PAGEABLE=staged)
     DeviceBuffer partials;        // Best[n_obj * n_parts]
     DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
     DeviceBuffer stats;           // ObjStats[n_obj]
@@ -509,6 +515,29 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         lsp_status e = ensure(p, p->ring, slot_bytes * n_slots);
         if (e != LSP_OK) return e;
     }
+    // A pinned (or registered) destination is written directly by the async copies.  A pageable one is either handed to
+    // cudaMemcpyAsync as it is (the driver stages it; default) or goes the paper's way (L117; LSP_PAGEABLE=staged): D2H into a
+    // pinned staging slot, then a host-side memcpy into the caller's buffer run by the copy stream's callback thread, the
+    // slot's "free" event covering both the device slot and its staging twin.  Measured on config 4 (4 GB): pinned 76 ms,
+    // pageable plain 229 ms, pageable staged 283 ms -- the callback threads' memcpy (~14 GB/s) is slower than the driver's
+    // own staging on this host, the opposite of the paper's Pascal-era result (Fig. 8: up to 1.91x for staging).
+    bool staged = false;
+    {
+        cudaPointerAttributes attr{};
+        const cudaError_t pe = cudaPointerGetAttributes(&attr, out_power);
+        if (pe != cudaSuccess) cudaGetLastError();
+        staged = (pe != cudaSuccess || attr.type == cudaMemoryTypeUnregistered) && p->pageable_mode == 0;
+    }
+    if (staged) {
+        if (p->stage_host_bytes < slot_bytes * n_slots) {
+            if (p->stage_host) LSP_CUDA(p, cudaFreeHost(p->stage_host));
+            p->stage_host = nullptr;
+            p->stage_host_bytes = 0;
+            LSP_CUDA(p, cudaMallocHost(&p->stage_host, slot_bytes * n_slots));
+            p->stage_host_bytes = slot_bytes * n_slots;
+        }
+        p->host_copies.assign((size_t)((n_obj + objs_per_chunk - 1) / objs_per_chunk), lsp_plan::HostCopy{});
+    }
     std::fill(p->slot_used.begin(), p->slot_used.end(), 0);
     // a chunk's schedule is made for the chunk's own object count, so small chunks still split observations
     int64_t chunk = 0;
@@ -529,8 +558,21 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         LSP_CUDA(p, cudaEventRecord(p->slot_ready[slot], st));
         cudaStream_t cs = p->copy_streams[chunk % p->copy_streams.size()];
         LSP_CUDA(p, cudaStreamWaitEvent(cs, p->slot_ready[slot], 0));
-        LSP_CUDA(p, cudaMemcpyAsync((char*)out_power + (size_t)o0 * row_bytes, dslot, (size_t)no * row_bytes,
-                                    cudaMemcpyDeviceToHost, cs));
+        if (staged) {
+            char* hslot = (char*)p->stage_host + (size_t)slot * slot_bytes;
+            LSP_CUDA(p, cudaMemcpyAsync(hslot, dslot, (size_t)no * row_bytes, cudaMemcpyDeviceToHost, cs));
+            lsp_plan::HostCopy& hc = p->host_copies[(size_t)chunk];
+            hc.dst = (char*)out_power + (size_t)o0 * row_bytes;
+            hc.src = hslot;
+            hc.bytes = (size_t)no * row_bytes;
+            LSP_CUDA(p, cudaLaunchHostFunc(cs, [](void* u) {
+                const lsp_plan::HostCopy* h = (const lsp_plan::HostCopy*)u;
+                memcpy(h->dst, h->src, h->bytes);
+            }, &hc));
+        } else {
+            LSP_CUDA(p, cudaMemcpyAsync((char*)out_power + (size_t)o0 * row_bytes, dslot, (size_t)no * row_bytes,
+                                        cudaMemcpyDeviceToHost, cs));
+        }
         LSP_CUDA(p, cudaEventRecord(p->slot_free[slot], cs));
         p->slot_used[slot] = 1;
     }
@@ -594,6 +636,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     p->sm_count = prop.multiProcessorCount;
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
     if (const char* b = getenv("LSP_TABLE_BUDGET_MB")) p->tc_table_budget = (size_t)std::max(1L, atol(b)) << 20;
+    if (const char* b = getenv("LSP_PAGEABLE")) p->pageable_mode = strcmp(b, "staged") == 0 ? 0 : 1;
     if (const char* b = getenv("LSP_TC_SB")) p->tc_stages_b = (int)std::min(6L, std::max(2L, atol(b)));
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
@@ -824,6 +867,7 @@ void lsp_destroy(lsp_plan* p)
     for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->gls_x, &p->gls_yy, &p->gls_sums, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
+    if (p->stage_host) cudaFreeHost(p->stage_host);
     cudaGetLastError();
     delete p;
 }

@@ -181,11 +181,17 @@ def test_config4_shape_host_output_streams(lsp, oracle):
     # summation order (not the result) can differ
     assert np.max(np.abs(host.numpy() - dev.cpu().numpy())) <= 1e-5 * P_ref.max()
     assert_best_parity(tuple(x.cpu().numpy() for x in best), P_ref, w, "f32", oracle)
-    # pageable destination also works (serialised)
-    pageable = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32)
-    with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f32", fast_math=True, chunk_bytes=1 << 20) as plan:
-        plan.periodogram_batched(off, t, y, host_out=pageable)
-    assert np.max(np.abs(pageable.numpy() - host.numpy())) <= 1e-5 * P_ref.max()
+    # pageable destination: plain cudaMemcpyAsync (default) and the paper's staging scheme
+    import os
+    for mode in ("plain", "staged"):
+        os.environ["LSP_PAGEABLE"] = mode
+        try:
+            pageable = torch.full((w.n_obj, w.n_freq), float("nan"), dtype=torch.float32)
+            with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f32", fast_math=True, chunk_bytes=1 << 20) as plan:
+                plan.periodogram_batched(off, t, y, host_out=pageable)
+        finally:
+            os.environ.pop("LSP_PAGEABLE", None)
+        assert np.max(np.abs(pageable.numpy() - host.numpy())) <= 1e-5 * P_ref.max(), mode
 
 
 # ---- config 5 shape: large N_t / small N_f -> observation split path ----------------------------------------
