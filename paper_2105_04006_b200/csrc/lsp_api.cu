@@ -953,7 +953,7 @@ lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, doubl
 
 const char* lsp_version(void)
 {
-    return "lsp-b200 0.2 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05)";
+    return "lsp-b200 0.3 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05; modes: standard, generalised)";
 }
 
 }  // extern "C"

@@ -30,7 +30,7 @@
 // chunks are contiguous (no bank conflicts).
 // Operands a, b are generated into a double-buffered shared-memory chunk (JC observations) by all threads
 // (phase in FP64 -> range-reduced -> MUFU or accurate sincos) while the previous chunk is being contracted.
-// No tensor cores: see DESIGN.md for why this path is not tcgen05.
+// This file is the FMA-pipe / FP64-pipe form of the contraction; lsp_tensor.cuh runs the same contraction on tcgen05 (FP32 mode).
 //
 // Work item = (object, frequency tile, observation split) as in the direct kernel; n_split > 1 writes the
 // four sums per frequency for lsp_combine_kernel (split-N_t path for large-N_t / small-N_f problems).
