@@ -59,6 +59,7 @@ struct lsp_plan {
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     int tc_stages_b = 3;          // B-operand ring depth of the tensor kernel
+    int tc_roles = 0;             // 0 = by item length, 1 = force (8 epilogue warps, 2 generator groups), 2 = force (4, 3); LSP_TC_ROLES
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
@@ -140,9 +141,8 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
         s.tp.n_ops = c.fast_math ? 2 : 4;
         s.tp.a_stage_bytes = s.tp.n_ops * 128 * kTcKB * 2;
         s.tp.b_stage_bytes = s.tp.n_ops * 2 * (int)nl * kTcKB * 2;
-        // B ring: 3 stages (LSP_TC_SB overrides); A ring: whatever else fits, at most 8
+        // B ring: 3 stages (LSP_TC_SB overrides); A ring: whatever else fits, at most 8 (sized after the split is known)
         s.tp.stages_b = p->tc_stages_b;
-        s.tp.stages = (int)std::max<int64_t>(2, std::min<int64_t>(8, ((int64_t)(p->smem_optin - 18432) - (int64_t)s.tp.stages_b * s.tp.b_stage_bytes) / s.tp.a_stage_bytes));
         s.tile = s.tp.tile;
         s.direct_r = 0;
         slots = p->sm_count;
@@ -177,6 +177,14 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
         }
     }
     s.n_split = (int)split;
+    if (k == LSP_KERNEL_TENSOR) {
+        // role shape by item length: stages (16 observations) per work item
+        const int64_t avg_nt = n_obj > 0 ? total_obs / n_obj : 0;
+        const int64_t stages_per_item = (avg_nt / kTcKB) / std::max<int64_t>(1, split);
+        s.tp.long_items = (p->tc_roles == 0) ? (stages_per_item >= 48 ? 1 : 0) : (p->tc_roles == 2 ? 1 : 0);
+        const int reserve = (s.tp.long_items ? tc_static_smem<3>() : tc_static_smem<2>()) + 2048;
+        s.tp.stages = (int)std::max<int64_t>(3, std::min<int64_t>(8, ((int64_t)(p->smem_optin - reserve) - (int64_t)s.tp.stages_b * s.tp.b_stage_bytes) / s.tp.a_stage_bytes));
+    }
     return s;
 }
 
@@ -191,18 +199,23 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (s.kernel == LSP_KERNEL_TENSOR) {
         if constexpr (std::is_same<T, float>::value) {
-            auto kern = lsp_tensor_kernel<float, FAST>;
             const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.stages_b, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
-            static size_t attr_smem = 0;       // per instantiation
-            if (smem > attr_smem) {
-                cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-                if (e != cudaSuccess) return e;
-                attr_smem = smem;
-            }
             const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
-            kern<<<ctas, kTcThreads, smem, st>>>(gp, s.tp, d_off, (const float*)d_t, (const float*)d_y,
-                                                 (const TensorObj*)p->tc_objs.ptr, (const __half*)p->tc_table.ptr, (float*)out,
-                                                 partials, (float4*)sums, n_obj_launch, (long long)grid);
+            auto go = [&](auto kern, int threads, size_t& attr_smem) -> cudaError_t {
+                if (smem > attr_smem) {
+                    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                    if (e != cudaSuccess) return e;
+                    attr_smem = smem;
+                }
+                kern<<<ctas, threads, smem, st>>>(gp, s.tp, d_off, (const float*)d_t, (const float*)d_y,
+                                                  (const TensorObj*)p->tc_objs.ptr, (const __half*)p->tc_table.ptr, (float*)out,
+                                                  partials, (float4*)sums, n_obj_launch, (long long)grid);
+                return cudaSuccess;
+            };
+            static size_t attr_short = 0, attr_long = 0;       // per FAST instantiation
+            cudaError_t e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 3>, TcRoles<4, 3>::kThreads, attr_long)
+                                            : go(lsp_tensor_kernel<float, FAST, 8, 2>, TcRoles<8, 2>::kThreads, attr_short);
+            if (e != cudaSuccess) return e;
         } else {
             return cudaErrorInvalidValue;      // rejected at plan creation
         }
@@ -637,6 +650,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
     if (const char* b = getenv("LSP_TABLE_BUDGET_MB")) p->tc_table_budget = (size_t)std::max(1L, atol(b)) << 20;
     if (const char* b = getenv("LSP_PAGEABLE")) p->pageable_mode = strcmp(b, "staged") == 0 ? 0 : 1;
+    if (const char* b = getenv("LSP_TC_ROLES")) p->tc_roles = (int)std::min(2L, std::max(0L, atol(b)));
     if (const char* b = getenv("LSP_TC_SB")) p->tc_stages_b = (int)std::min(6L, std::max(2L, atol(b)));
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {

@@ -43,16 +43,26 @@ namespace lsp {
 constexpr int kTcGroups = 64;                  // frequency groups per tile (128 MMA rows)
 constexpr int kTcKB = 16;                      // observations per MMA / ring stage (kind::f16: K = 16)
 constexpr int kTcMaxNL = 128;                  // N = 2 NL <= 256
-constexpr int kTcGenWarps = 16, kTcEpiWarps = 8;                      // generators: two groups of 8 warps
-constexpr int kTcThreads = (4 + kTcEpiWarps + kTcGenWarps) * 32;      // 896: 72 registers per thread at launch
-constexpr int kTcGenGroupThreads = 256;                               // threads that build one ring stage
-// register split (setmaxnreg, per 4-warp group): 128 x 40 + 256 x 120 + 512 x 56 = 64512 = 896 x 72
-constexpr int kTcCtrlRegs = 40, kTcEpiRegs = 120, kTcGenRegs = 56;
-constexpr int kTcEpiThreads = kTcEpiWarps * 32;
 // Generator scratch (floats): three planes (cos, sin, -sin) of [observation quad j/4][phasor q][j%4]; a quad row is 16 x 4
 // floats + 16 floats of padding so that the two quads a quarter-warp reads fall into different banks (conflict-free LDS.128).
 constexpr int kTcScratchQuad = 16 * 4 + 16;
 constexpr int kTcScratchPlane = 4 * kTcScratchQuad;
+constexpr int kTcGenGroupThreads = 256;                               // threads that build one ring stage
+// Warp roles of one CTA: 4 control warps, EW epilogue warps, NG generator groups of 8 warps.  Two shapes are built:
+//   (EW, NG) = (8, 2): 896 threads -- short items (batches of short light curves): the per-item epilogue is on the critical path
+//   (EW, NG) = (4, 3): 1024 threads -- long items (hundreds of stages): the generators are, the epilogue is rare
+// Registers are re-split with setmaxnreg (per 4-warp group): control 40, generators 56, epilogue what is left
+// (120 resp. 136): 128 x 40 + 256 x 120 + 512 x 56 = 64512 = 896 x 72;  128 x 40 + 128 x 136 + 768 x 56 = 65536 = 1024 x 64.
+template <int EW, int NG> struct TcRoles {
+    static constexpr int kThreads = (4 + EW + 8 * NG) * 32;
+    static constexpr int kEpiThreads = EW * 32;
+    static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8;
+    static constexpr int kCtrlRegs = 40, kGenRegs = 56;
+    static constexpr int kEpiRegs = ((kLaunchRegs * kThreads - 128 * kCtrlRegs - 8 * NG * 32 * kGenRegs) / kEpiThreads) / 8 * 8;
+    static_assert(EW % 4 == 0 && kThreads <= 1024 && kEpiRegs >= 96 && kEpiRegs <= 255, "role split");
+};
+// static shared memory of the kernel (generator scratch etc.) + alignment slack, for the host's ring sizing
+template <int NG> constexpr int tc_static_smem() { return NG * 2 * (3 * kTcScratchPlane + kTcKB) * 4 + 1024; }
 constexpr float kTcUnitScale = 256.0f;         // scale of the unit-modulus A_W operands (keeps the FP16 low part normal)
 
 struct TensorParams {
@@ -61,6 +71,7 @@ struct TensorParams {
     int n_ops;          // FP16 operand planes per stage side: 4 (accurate: hi and lo of Z- and W-operands) or 2 (fast)
     int stages;         // A-operand ring depth (generators -> MMA)
     int stages_b;       // B-operand ring depth (TMA -> MMA): shallower, the copies are fast and B stages are twice as large
+    int long_items;     // 1: many stages per item -> the (4 epilogue warps, 3 generator groups) shape; 0: (8, 2)
     int b_stage_bytes;  // n_ops * 2 NL * 32
     int a_stage_bytes;  // n_ops * 128 * 32
 };
@@ -336,13 +347,15 @@ constexpr size_t tc_smem_bytes(int stages_a, int stages_b, int a_stage, int b_st
     return 1024 /* alignment slack */ + (size_t)stages_a * (size_t)a_stage + (size_t)stages_b * (size_t)b_stage + 512;
 }
 
-template <typename T, bool FAST>
-__global__ void __launch_bounds__(kTcThreads, 1)
+template <typename T, bool FAST, int EW, int NG>
+__global__ void __launch_bounds__((TcRoles<EW, NG>::kThreads), 1)
 lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
                   const T* __restrict__ y, const TensorObj* __restrict__ objs, const __half* __restrict__ table,
                   T* __restrict__ out_power, Best* __restrict__ partials, float4* __restrict__ sums,
                   int64_t n_obj_launch, long long total_items)
 {
+    using R = TcRoles<EW, NG>;
+    constexpr int kTcEpiWarps = EW, kTcEpiThreads = R::kEpiThreads;
     constexpr int NOPS = FAST ? 2 : 4;
     constexpr int A_PLANE = 128 * kTcKB * 2;                  // bytes of one A plane: 128 rows x 16 x FP16
     extern __shared__ unsigned char smem_dyn[];
@@ -361,8 +374,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
     __shared__ Best sbest[kTcEpiWarps];
-    __shared__ __align__(16) float s_uv[2][2][3 * kTcScratchPlane];  // generator scratch: [group][buffer][plane][j/4][phasor q][j%4]
-    __shared__ __align__(16) float s_yv[2][2][kTcKB];                // scaled, centred y of the stage
+    __shared__ __align__(16) float s_uv[NG][2][3 * kTcScratchPlane]; // generator scratch: [group][buffer][plane][j/4][phasor q][j%4]
+    __shared__ __align__(16) float s_yv[NG][2][kTcKB];               // scaled, centred y of the stage
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // broadcast: the compiler may treat the role as warp-uniform
@@ -388,7 +401,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     tc_fence_after();
     const unsigned tmem = tmem_base_s;
 
-    if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcCtrlRegs));
+    if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kCtrlRegs));
     if (warp == 0) {
         // =============================== TMA producer: B stages from the per-object table ========================
         if (lane == 0) {
@@ -472,16 +485,17 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         // the frequency above the group centre (k = c + m), the Im lane the one below (k = c - 1 - m), so all 32 lanes
         // produce distinct powers.  Indices are tile-local 32-bit integers; the argmax runs in FP32 + int and is widened
         // once per item; bounds are only checked on the grid's ragged last tile.
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kTcEpiRegs));
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R::kEpiRegs));
         const int ew = warp - 4;
         const int q = warp & 3;                                   // TMEM lane quadrant this warp may access
-        const int half_sel = ew >> 2;                             // which half of the m range
+        const int half_sel = ew >> 2;                             // which part of the m range (EW / 4 parts)
+        constexpr int kParts = EW / 4;
         const int etid = tid - 128;
         const bool is_im = lane >= 16;
         const int g = 16 * q + (lane & 15);
         const int NL = tp.nl, L = 2 * NL;
         const int n_chunks = (NL + 15) >> 4;                      // 16-column chunks over m (NL is a multiple of 8)
-        const int ch0 = (n_chunks * half_sel) / 2, ch1 = (n_chunks * (half_sel + 1)) / 2;
+        const int ch0 = (n_chunks * half_sel) / kParts, ch1 = (n_chunks * (half_sel + 1)) / kParts;
         const bool vec_ok = (gp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(out_power) & 15) == 0);
         const int kc = g * L + NL;                                // tile-local index of the first frequency above the centre
         unsigned n_acc = 0;
@@ -662,9 +676,9 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         // Two groups of 8 warps take alternate ring stages, so one group's latencies (sincos chain, group barrier,
         // LDS, mbarrier wait, proxy fence) are covered by the other group's instructions on the same schedulers.
         // t / y of a group's NEXT stage (of this or a later work item) are loaded before its current stage is processed.
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kTcGenRegs));
-        const int gw = warp - (4 + kTcEpiWarps);                  // 0..15
-        const int grp = gw >> 3;                                  // generator group: stages with (stage number & 1) == grp
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kGenRegs));
+        const int gw = warp - (4 + kTcEpiWarps);                  // 0 .. 8 NG - 1
+        const int grp = gw >> 3;                                  // generator group: stages with (stage number mod NG) == grp
         const int gw8 = gw & 7;
         const int gtid = (tid - (4 + kTcEpiWarps) * 32) & (kTcGenGroupThreads - 1);      // 0..255 inside the group
         // phase 1 role: phasor q (0-7: u_g0, 8-15: v_g1) of observation j1 of the stage
@@ -716,10 +730,11 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         Cursor p1;
         p1.item = blockIdx.x;
         seek(p1);
-        if (grp == 1 && p1.item < total_items) step(p1);
+        for (int i = 0; i < grp; ++i)
+            if (p1.item < total_items) step(p1);
         int st = grp;                                             // ring slot of the stage phase 2 writes
         unsigned eph = 1;                                         // parity of the "empty" phase to wait for
-        if (st >= S) { st -= S; eph ^= 1; }
+        while (st >= S) { st -= S; eph ^= 1; }
         unsigned it = 0;
         float* s_uvg = &s_uv[grp][0][0];
         float* s_yvg = &s_yv[grp][0][0];
@@ -754,8 +769,9 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const float* syv = s_yvg + buf * kTcKB;
             // ---- phase 1 of this stage, then the loads of the group's next stage (two ring stages ahead)
             phase1(p1, t_p1, y_p1, buf);
-            step(p1);
-            if (p1.item < total_items) step(p1);
+#pragma unroll
+            for (int i = 0; i < NG; ++i)
+                if (p1.item < total_items) step(p1);
             float t_pf, y_pf;
             fetch(p1, t_pf, y_pf);
             named_bar_sync(4 + grp, kTcGenGroupThreads);
@@ -808,8 +824,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             put(1, NOPS - 1, off_im, a2i);
             fence_proxy_async();            // generic-proxy stores -> visible to the tensor core's async proxy
             mbar_arrive(&full[st]);
-            st += 2;
-            if (st >= S) { st -= S; eph ^= 1; }
+            st += NG;
+            while (st >= S) { st -= S; eph ^= 1; }
             ++it;
             t_p1 = t_pf;
             y_p1 = y_pf;
