@@ -310,7 +310,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
         if (e != LSP_OK) return e;
         sums = p->sums.ptr;
     }
-    *n_parts_out = (s.n_split > 1) ? n_cparts : s.n_tiles;
+    *n_parts_out = (s.n_split > 1 || ext_sums) ? n_cparts : s.n_tiles;
     if (want_best) {     // partials are indexed by the launch-local object: each launch's finalize follows it in-stream
         lsp_status e = ensure(p, p->partials, (size_t)n_obj_launch * (size_t)*n_parts_out * sizeof(Best));
         if (e != LSP_OK) return e;
@@ -333,8 +333,8 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
         LSP_CUDA(p, cudaEventRecord(ev0, st));
     }
     cudaError_t e;
-    void* main_out = (s.n_split > 1) ? nullptr : out;
-    Best* main_partials = (s.n_split > 1) ? nullptr : partials;
+    void* main_out = sums ? nullptr : out;             // kernels write partial sums instead of powers iff `sums` is set
+    Best* main_partials = sums ? nullptr : partials;
     if (c.dtype == LSP_F32) {
         e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st)
                         : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st);
@@ -763,7 +763,6 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
         p->cfg.kernel = LSP_KERNEL_FACTORED;
         s = make_schedule(p, n_obj, total_obs);
     }
-    s.n_split = std::max(2, s.n_split);           // the split form is the one that leaves sums, not powers, in memory
     p->kernel_used = s.kernel;
     p->n_split = s.n_split;
     p->n_pairs = 3 * total_obs * c.n_freq;

@@ -132,7 +132,7 @@ lsp_direct_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* _
         const int64_t k = (int64_t)wi.tile * (TPB * R) + r * TPB + tid;
         if (k >= gp.n_freq) continue;
         const T c2 = T(2) * cc[r] - n_part, s2 = T(2) * cs[r];   // sum cos 2wt, sum sin 2wt
-        if (gp.n_split > 1) {
+        if (sums) {      // split-N_t (or the generalised mode): partial sums, not powers
             sums[((int64_t)wi.split * n_obj_launch + wi.obj_local) * gp.n_freq + k] = make_vec4<T>(xc[r], xs[r], c2, s2);
         } else {
             const T scale = stats ? (T)stats[obj].scale : T(1);
@@ -144,7 +144,7 @@ lsp_direct_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* _
             mine = best_of(mine, b);
         }
     }
-    if (partials && gp.n_split == 1) {
+    if (partials && !sums) {
         const Best b = block_best(mine, sbest);
         if (tid == 0) partials[wi.obj_local * gp.n_tiles + wi.tile] = b;
     }

@@ -283,7 +283,7 @@ lsp_factored_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T*
     Best mine;
     mine.p = -1.0;
     mine.k = INT64_MAX;
-    const bool stage = (gp.n_split == 1) && (out_power != nullptr);
+    const bool stage = !sums && (out_power != nullptr);
     if (!is_w) {
         const T scale = stats ? (T)stats[obj].scale : T(1);
 #pragma unroll
@@ -304,7 +304,7 @@ lsp_factored_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T*
                         xc = acc_r[a][c].x + acc_i[a][c].y;
                         xs = acc_i[a][c].x - acc_r[a][c].y;
                     }
-                    if (gp.n_split > 1) {
+                    if (sums) {
                         if (k < gp.n_freq)
                             sums[((int64_t)wi.split * n_obj_launch + wi.obj_local) * gp.n_freq + k] = make_vec4<T>(xc, xs, w.x, w.y);
                     } else {
@@ -326,7 +326,7 @@ lsp_factored_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T*
         const int n_valid = (int)min((int64_t)TILE, (int64_t)gp.n_freq - K0);
         for (int i = tid; i < n_valid; i += TPB) dst[i] = sP[i];
     }
-    if (partials && gp.n_split == 1) {
+    if (partials && !sums) {
         const Best b = block_best(mine, sbest);
         if (tid == 0) partials[wi.obj_local * gp.n_tiles + wi.tile] = b;
     }

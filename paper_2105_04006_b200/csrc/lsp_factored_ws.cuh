@@ -418,7 +418,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             Best mine;
             mine.p = -1.0;
             mine.k = INT64_MAX;
-            const bool stage_out = (gp.n_split == 1) && (out_power != nullptr);
+            const bool stage_out = !sums && (out_power != nullptr);
 #pragma unroll
             for (int a = 0; a < TH; ++a)
 #pragma unroll
@@ -441,7 +441,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                         }
                         const V2 z = is_w ? other : me;      // (xc, xs)
                         const V2 ww = is_w ? me : other;     // (c2, s2)
-                        if (gp.n_split > 1) {
+                        if (sums) {
                             if (k < gp.n_freq)
                                 sums[((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + k] = make_vec4<T>(z.x, z.y, ww.x, ww.y);
                         } else {
@@ -462,7 +462,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 const int n_valid = (int)min((int64_t)TILE, (int64_t)gp.n_freq - w.K0);
                 for (int i = tid; i < n_valid; i += kWsConsumers) dst[i] = sP[i];
             }
-            if (partials && gp.n_split == 1) {
+            if (partials && !sums) {
                 mine = warp_best(mine);
                 if (lane == 0) sbest[tid >> 5] = mine;
                 named_bar_sync(2, kWsConsumers);

@@ -12,7 +12,7 @@
 //     pass B: x = w,            f' = f      -> (C, S)
 //     pass C: x = w,            f' = 2 f    -> (c2, s2)      (the doubled grid is linear too)
 // so the generalised mode runs the unmodified direct / factored / tensor kernels three times in their split-N_t form (partial
-// sums to global memory, n_split >= 2) and combines here.  Cost 3x the standard periodogram (the paper's own implementation:
+// sums to global memory; any n_split) and combines here.  Cost 3x the standard periodogram (the paper's own implementation:
 // 2.06-2.14x, L419); a weighted W slot in the kernels would make it 2x.
 #pragma once
 #include "lsp_direct.cuh"

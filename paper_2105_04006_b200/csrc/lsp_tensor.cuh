@@ -514,7 +514,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const int n_valid = (int)min((int64_t)tp.tile, (int64_t)gp.n_freq - w.K0);     // frequencies of this tile on the grid
             const bool ragged = n_valid < tp.tile;
             T* otile = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq + w.K0 : nullptr;
-            float4* stile = (gp.n_split > 1) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
+            float4* stile = sums ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
             const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
             bool released = false;
             // one chunk = 16 accumulator columns of each of the four TMEM regions; RAG = the tile overhangs the grid
@@ -647,7 +647,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 }
                 ++n_acc;
             }
-            if (partials && gp.n_split == 1) {
+            if (partials && !stile) {
                 Best mine;
                 mine.p = (double)bp;
                 mine.k = (bk == 0x7fffffff) ? INT64_MAX : w.K0 + (int64_t)bk;
