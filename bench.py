@@ -45,7 +45,7 @@ TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 bu
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel on config 2, from the committed
 # `ncu --set full` captures (profiles/r01_ncu_full_*.csv; commands in profiles/r01_README.md).  Other workloads: null.
-NCU_TRAFFIC_C2 = {("tensor", False): 21.87e6 + 58.68e6, ("factored", "f32"): 5.94e6 + 0.37e6, ("factored", "f64"): 6.65e6 + 42.69e6}
+NCU_TRAFFIC_C2 = {("tensor", False): 20.83e6 + 58.40e6, ("factored", "f32"): 5.94e6 + 0.37e6, ("factored", "f64"): 6.65e6 + 42.69e6}
 
 
 def measured_tensor_peak():
