@@ -1,10 +1,13 @@
-// lsp_peak.cuh -- register-only pipe-peak microbenchmarks: the measured denominators of the ALU roofline
-// (DESIGN.md "Roofline").  MEASURED_PEAKS.json only carries HBM and BF16 tensor numbers; the periodogram is
-// bound by the FMA / FP64 / XU pipes, so those are measured here with the same clocks the kernels see.
-#pragma once
-#include "lsp_common.cuh"
+// bench_peak.cu -- register-only pipe-peak microbenchmarks for bench.py: the MEASURED denominators that ride beside the
+// derived ALU roofline.  MEASURED_PEAKS.json only carries HBM and BF16 tensor numbers; the FMA-pipe
+// kernels are bound by the FMA / FP64 / XU pipes, so those are measured here with the same clocks the kernels see.
+// Bench-only helper: built into libbench_peak.so by bench.py / __graft_entry__.build(); NOT part of liblsp_b200.so or its ABI.
+#include <cuda_runtime.h>
+#include <stdint.h>
 
-namespace lsp {
+#include <algorithm>
+
+namespace {
 
 constexpr int kPeakThreads = 256;
 constexpr int kPeakIters = 4096;
@@ -114,4 +117,56 @@ __global__ void __launch_bounds__(kPeakThreads, 2) peak_mix_kernel(float* out, f
     if (s == 12345.678f) out[0] = s;
 }
 
-}  // namespace lsp
+}  // namespace
+
+/*
+ * Runs a register-only loop of one instruction class on every SM and returns the measured thread-level operations per second.
+ *   which: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2, counted as 2 FMA per lane), 2 = DFMA, 3 = MUFU.SIN+MUFU.COS (counted
+ *          as 2 ops), 4 = FFMA2 with one LDS.128 per 8 (the factored kernel's inner-loop mix)
+ * Returns 0 on success (a cudaError_t otherwise) and writes *ops_per_s and *elapsed_ms (HOST, the latter may be NULL).
+ */
+extern "C" int bench_pipe_peak(int32_t device, int32_t which, double* ops_per_s, double* elapsed_ms)
+{
+    if (!ops_per_s || which < 0 || which > 4) return (int)cudaErrorInvalidValue;
+#define BP_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return (int)e_; } while (0)
+    BP_CUDA(cudaSetDevice(device));
+    cudaDeviceProp prop;
+    BP_CUDA(cudaGetDeviceProperties(&prop, device));
+    void* out = nullptr;
+    BP_CUDA(cudaMalloc(&out, 64));
+    cudaEvent_t e0, e1;
+    BP_CUDA(cudaEventCreate(&e0));
+    BP_CUDA(cudaEventCreate(&e1));
+    const int ctas_per_sm = (which == 4) ? 2 : 4;
+    const unsigned grid = (unsigned)(prop.multiProcessorCount * ctas_per_sm * 4);    // 4 full waves
+    double ops_per_thread = 0.0;
+    float best_ms = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {                      // rep 0 is the warm-up
+        BP_CUDA(cudaEventRecord(e0, 0));
+        switch (which) {
+            case 0: peak_ffma_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
+                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
+            case 1: peak_ffma2_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
+                    ops_per_thread = 2.0 * kPeakIters * kPeakIlp; break;
+            case 2: peak_dfma_kernel<<<grid, kPeakThreads>>>((double*)out, 1.0000001, 1e-9);
+                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
+            case 3: peak_mufu_kernel<<<grid, kPeakThreads>>>((float*)out, 0.001f);
+                    ops_per_thread = 2.0 * (kPeakIters / 4) * kPeakIlp; break;
+            default: peak_mix_kernel<<<grid, kPeakThreads>>>((float*)out, 0.5f);
+                    ops_per_thread = 2.0 * 32.0 * 16.0 * (kPeakIters / 16); break;
+        }
+        BP_CUDA(cudaGetLastError());
+        BP_CUDA(cudaEventRecord(e1, 0));
+        BP_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        BP_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0) best_ms = std::min(best_ms, ms);
+    }
+#undef BP_CUDA
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    *ops_per_s = ops_per_thread * (double)grid * kPeakThreads / (best_ms * 1e-3);
+    if (elapsed_ms) *elapsed_ms = best_ms;
+    return 0;
+}

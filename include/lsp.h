@@ -72,15 +72,25 @@ typedef struct lsp_config {
     int64_t max_objects;    /* scratch sizing hints; 0 = size on first use (scratch grows when needed)     */
     int64_t max_total_obs;
     int32_t kernel;         /* lsp_kernel                                                                  */
-    int32_t reserved;       /* must be 0                                                                   */
+    int32_t flags;          /* bit set of LSP_FLAG_*; unknown bits are rejected                            */
+    int64_t table_budget_bytes; /* tensor path: cap on the per-launch B-operand table; larger batches run in
+                                   object ranges (same results); 0 = library default (12 GiB)              */
+    int32_t tensor_roles;   /* tensor path warp-role shape: 0 = chosen by item length, 1 = short-item shape
+                                   (8 epilogue warps), 2 = long-item shape (4 epilogue warps)               */
+    int32_t tensor_b_stages;/* tensor path: depth of the B-operand (TMA) ring, 2..8; 0 = library default    */
 } lsp_config;
+
+/* lsp_config.flags */
+#define LSP_FLAG_PAGEABLE_STAGED 1 /* host output into PAGEABLE memory goes through a plan-owned pinned staging ring and
+                                      host-side copies on the copy streams' callback threads (the paper's scheme,
+                                      PAPER.md:L117) instead of plain cudaMemcpyAsync into the pageable buffer      */
 
 /*
  * Create a plan: validates cfg, selects the device, creates the D2H copy streams and events and
  * allocates scratch (argmax partials, split-N_t partial sums, the device chunk ring for host output).
  * The plan owns all of that; the caller owns every buffer passed to the calls below.
  * Errors: LSP_ERR_INVALID_ARG (f_min <= 0, f_max <= f_min, n_freq < 1, fast_math with FP64, unknown
- * enum, reserved != 0), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
+ * enum or flag bit, tensor_roles / tensor_b_stages out of range), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
  * failure.  A plan is not thread-safe; distinct plans are independent.
  */
 lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan /* HOST */);
@@ -97,7 +107,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan
  *                a DEVICE pointer when out_is_host == 0, else a HOST pointer filled through the plan's chunk ring and copy
  *                streams: a pinned (or registered) buffer is written directly by the async copies and overlaps with compute;
  *                a pageable one is handed to cudaMemcpyAsync as it is (works, does not overlap), or, with
- *                LSP_PAGEABLE=staged in the environment at plan creation, goes through a plan-owned pinned staging ring and
+ *                LSP_FLAG_PAGEABLE_STAGED in cfg.flags, goes through a plan-owned pinned staging ring and
  *                per-chunk host-side copies run by the copy streams' callback threads (PAPER.md:L117's scheme)
  *   d_best_*     DEVICE, optional (all three NULL or all three non-NULL): per object best period
  *                (cfg.dtype), its power (cfg.dtype) and grid index (int64; -1 and NaN period when N_t = 0)
@@ -168,6 +178,22 @@ lsp_status lsp_periodogram_batched_host(lsp_plan* plan, int64_t n_obj,
                                         void* h_best_period, void* h_best_power, int64_t* h_best_index,
                                         void* cuda_stream);
 
+/*
+ * Best period over FREQUENCY SHARDS (a single huge object, or any batch, whose grid was cut into contiguous index ranges that
+ * ran as separate plans, possibly on different GPUs).  `plan` is a plan for the GLOBAL grid (its f_min,
+ * f_max, n_freq and dtype are used; no periodogram is computed).  For every object the candidates of the n_parts shards are
+ * merged with the library's own rule (reading a7: largest power, lowest grid index on exact ties, NaN or
+ * index -1 never wins) and period = 1/f_k on the global grid.
+ *   d_part_power   DEVICE, [n_parts][n_obj] of cfg.dtype: each shard's best power per object
+ *   d_part_index   DEVICE, int64 [n_parts][n_obj]: each shard's best GLOBAL grid index per object, or -1
+ *   d_best_*       DEVICE, n_obj elements each (index -1, power 0, period NaN when no shard had a candidate)
+ * Asynchronous on cuda_stream.  Errors: LSP_ERR_INVALID_ARG, LSP_ERR_CUDA.
+ */
+lsp_status lsp_best_merge(lsp_plan* plan, int64_t n_obj, int32_t n_parts,
+                          const void* d_part_power, const int64_t* d_part_index,
+                          void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                          void* cuda_stream);
+
 /* Frees the plan and everything it owns (synchronises its streams first).  NULL is a no-op. */
 void lsp_destroy(lsp_plan* plan);
 
@@ -175,11 +201,12 @@ void lsp_destroy(lsp_plan* plan);
  * plan == NULL, the message of the last failed lsp_plan_create on this thread.  Never NULL. */
 const char* lsp_last_error(const lsp_plan* plan);
 
-/* Bookkeeping of the LAST call on the plan, for benchmarks: how many of the library's kernels it launched,
- * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), and --
- * host-output calls only -- chunks copied.  Any pointer may be NULL. */
+/* Bookkeeping of the LAST call on the plan, for benchmarks and tests: how many of the library's kernels it launched,
+ * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), -- host-output
+ * calls only -- chunks copied, and the tensor kernel's warp-role shape (0 = tensor kernel not used, 1 = short-item
+ * shape, 2 = long-item shape; see lsp_config.tensor_roles).  Any pointer may be NULL. */
 void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used,
-                        int32_t* n_split, int64_t* n_chunks);
+                        int32_t* n_split, int64_t* n_chunks, int32_t* tensor_shape);
 
 /*
  * Device time of the periodogram kernel(s) of the LAST call, in milliseconds, measured with CUDA events
@@ -188,15 +215,6 @@ void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pa
  */
 void  lsp_set_timing(lsp_plan* plan, int32_t on);
 float lsp_last_kernel_ms(lsp_plan* plan);
-
-/*
- * Pipe-peak microbenchmark used for the roofline denominators: runs a register-only
- * loop of one instruction class on every SM and returns the measured thread-level operations per second.
- *   which: 0 = FFMA, 1 = FFMA2 (fma.rn.f32x2, counted as 2 FMA per lane), 2 = DFMA, 3 = MUFU.SIN+MUFU.COS (counted
- *          as 2 ops), 4 = FFMA2 with one LDS.128 per 8 (the factored kernel's inner-loop mix)
- * Returns LSP_OK and writes *ops_per_s (HOST) and *sm_mhz_est (HOST, may be NULL): ops / (SMs * lanes) is left to the caller.
- */
-lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, double* elapsed_ms);
 
 /* Library version / build string (static). */
 const char* lsp_version(void);

@@ -6,15 +6,16 @@ its thin Python binding.  There is no CPU fallback: the calls fail loudly withou
 from .binding import (  # noqa: F401
     EXPORTS,
     LspConfig,
+    LSP_FLAG_PAGEABLE_STAGED,
     LspError,
     Plan,
     load_library,
+    lsp_best_merge,
     lsp_best_period,
     lsp_destroy,
     lsp_periodogram_batched,
     lsp_periodogram_batched_host,
     lsp_periodogram_generalized,
-    lsp_pipe_peak,
     lsp_plan_create,
     lsp_version,
 )

@@ -8,7 +8,6 @@ be built, importing this module raises: there is no CPU fallback.
 from __future__ import annotations
 
 import ctypes
-import os
 from typing import Optional
 
 import torch
@@ -24,9 +23,10 @@ _KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LS
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
 EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host",
-           "lsp_periodogram_generalized", "lsp_destroy",
+           "lsp_periodogram_generalized", "lsp_best_merge", "lsp_destroy",
            "lsp_last_error",
-           "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_pipe_peak", "lsp_version")
+           "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_version")
+LSP_FLAG_PAGEABLE_STAGED = 1
 
 
 class LspConfig(ctypes.Structure):
@@ -36,7 +36,8 @@ class LspConfig(ctypes.Structure):
         ("dtype", ctypes.c_int32), ("fast_math", ctypes.c_int32), ("normalize", ctypes.c_int32),
         ("center", ctypes.c_int32), ("device", ctypes.c_int32), ("n_copy_streams", ctypes.c_int32),
         ("chunk_bytes", ctypes.c_int64), ("max_objects", ctypes.c_int64), ("max_total_obs", ctypes.c_int64),
-        ("kernel", ctypes.c_int32), ("reserved", ctypes.c_int32),
+        ("kernel", ctypes.c_int32), ("flags", ctypes.c_int32),
+        ("table_budget_bytes", ctypes.c_int64), ("tensor_roles", ctypes.c_int32), ("tensor_b_stages", ctypes.c_int32),
     ]
 
 
@@ -54,8 +55,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     global _lib
     if _lib is not None and path is None:
         return _lib
-    # LSP_B200_LIB names a prebuilt library to use instead of the in-tree build (kernel A/B experiments)
-    lib = ctypes.CDLL(path or os.environ.get("LSP_B200_LIB") or _build.build())
+    lib = ctypes.CDLL(path or _build.build())
     vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
     lib.lsp_plan_create.argtypes = [ctypes.POINTER(LspConfig), ctypes.POINTER(vp)]
     lib.lsp_plan_create.restype = ctypes.c_int
@@ -67,19 +67,19 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_periodogram_batched_host.restype = ctypes.c_int
     lib.lsp_periodogram_generalized.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsp_periodogram_generalized.restype = ctypes.c_int
+    lib.lsp_best_merge.argtypes = [vp, i64, i32, vp, vp, vp, vp, vp, vp]
+    lib.lsp_best_merge.restype = ctypes.c_int
     lib.lsp_destroy.argtypes = [vp]
     lib.lsp_destroy.restype = None
     lib.lsp_last_error.argtypes = [vp]
     lib.lsp_last_error.restype = ctypes.c_char_p
     lib.lsp_last_call_info.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i32),
-                                       ctypes.POINTER(i32), ctypes.POINTER(i64)]
+                                       ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32)]
     lib.lsp_last_call_info.restype = None
     lib.lsp_set_timing.argtypes = [vp, i32]
     lib.lsp_set_timing.restype = None
     lib.lsp_last_kernel_ms.argtypes = [vp]
     lib.lsp_last_kernel_ms.restype = ctypes.c_float
-    lib.lsp_pipe_peak.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
-    lib.lsp_pipe_peak.restype = ctypes.c_int
     lib.lsp_version.argtypes = []
     lib.lsp_version.restype = ctypes.c_char_p
     if path is None:
@@ -143,15 +143,16 @@ def lsp_periodogram_generalized(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y
                                                       _dptr(d_best_power), _dptr(d_best_index), _stream_ptr(stream)), plan)
 
 
+def lsp_best_merge(plan, n_obj: int, n_parts: int, d_part_power, d_part_index, d_best_period, d_best_power, d_best_index,
+                   stream=None) -> None:
+    """Merge the fused-argmax results of n_parts frequency shards (include/lsp.h): device tensors, asynchronous."""
+    _check(load_library().lsp_best_merge(plan, int(n_obj), int(n_parts), _dptr(d_part_power), _dptr(d_part_index),
+                                         _dptr(d_best_period), _dptr(d_best_power), _dptr(d_best_index),
+                                         _stream_ptr(stream)), plan)
+
+
 def lsp_destroy(plan) -> None:
     load_library().lsp_destroy(plan)
-
-
-def lsp_pipe_peak(which: int, device: int = 0):
-    """(ops_per_s, elapsed_ms) of the pipe microbenchmark `which` (see include/lsp.h)."""
-    ops, ms = ctypes.c_double(), ctypes.c_double()
-    _check(load_library().lsp_pipe_peak(int(device), int(which), ctypes.byref(ops), ctypes.byref(ms)))
-    return ops.value, ms.value
 
 
 def lsp_version() -> str:
@@ -164,12 +165,16 @@ class Plan:
 
     def __init__(self, f_min: float, f_max: float, n_freq: int, dtype: str = "f32", *, fast_math: bool = False,
                  normalize: bool = False, center: bool = False, device: int = 0, n_copy_streams: int = 0,
-                 chunk_bytes: int = 0, kernel: str = "auto", max_objects: int = 0, max_total_obs: int = 0):
+                 chunk_bytes: int = 0, kernel: str = "auto", max_objects: int = 0, max_total_obs: int = 0,
+                 pageable_staged: bool = False, table_budget_bytes: int = 0, tensor_roles: int = 0,
+                 tensor_b_stages: int = 0):
         if dtype not in ("f32", "f64"):
             raise ValueError("dtype must be 'f32' or 'f64'")
         self.cfg = LspConfig(float(f_min), float(f_max), int(n_freq), LSP_F32 if dtype == "f32" else LSP_F64,
                              int(fast_math), int(normalize), int(center), int(device), int(n_copy_streams),
-                             int(chunk_bytes), int(max_objects), int(max_total_obs), _KERNELS[kernel], 0)
+                             int(chunk_bytes), int(max_objects), int(max_total_obs), _KERNELS[kernel],
+                             LSP_FLAG_PAGEABLE_STAGED if pageable_staged else 0, int(table_budget_bytes),
+                             int(tensor_roles), int(tensor_b_stages))
         self.dtype = dtype
         self.torch_dtype = torch.float32 if dtype == "f32" else torch.float64
         self.n_freq = int(n_freq)
@@ -195,13 +200,24 @@ class Plan:
         self.destroy()
 
     # -- helpers
-    def _check_inputs(self, offsets, t, y):
-        if offsets.dtype != torch.int64 or not offsets.is_cuda:
-            raise TypeError("offsets must be a CUDA int64 tensor")
+    def _check_inputs(self, offsets, t, y, h_offsets=None):
+        """The C side receives raw pointers and cannot check any of this: a mismatched CSR must become a TypeError here,
+        not an out-of-bounds device read there."""
+        if offsets.dtype != torch.int64 or not offsets.is_cuda or not offsets.is_contiguous() or offsets.numel() < 1:
+            raise TypeError("offsets must be a contiguous CUDA int64 tensor of n_obj + 1 elements")
         for x in (t, y):
             if x.dtype != self.torch_dtype or not x.is_cuda or not x.is_contiguous():
                 raise TypeError(f"t and y must be contiguous CUDA tensors of {self.torch_dtype}")
-        return int(offsets.numel() - 1)
+        if t.numel() != y.numel():
+            raise TypeError("t and y must have the same number of elements")
+        n_obj = int(offsets.numel() - 1)
+        if h_offsets is not None:
+            if h_offsets.is_cuda or h_offsets.dtype != torch.int64 or not h_offsets.is_contiguous() \
+                    or h_offsets.numel() != n_obj + 1:
+                raise TypeError("h_offsets must be a contiguous host int64 tensor of n_obj + 1 elements")
+            if int(h_offsets[-1]) > t.numel():
+                raise TypeError("offsets[n_obj] exceeds the length of t / y")
+        return n_obj
 
     def set_timing(self, on: bool):
         load_library().lsp_set_timing(self._plan, int(on))
@@ -211,18 +227,18 @@ class Plan:
 
     def last_call_info(self) -> dict:
         nl, npairs, nch = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
-        ku, ns = ctypes.c_int32(), ctypes.c_int32()
+        ku, ns, ts = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
         load_library().lsp_last_call_info(self._plan, ctypes.byref(nl), ctypes.byref(npairs), ctypes.byref(ku),
-                                          ctypes.byref(ns), ctypes.byref(nch))
+                                          ctypes.byref(ns), ctypes.byref(nch), ctypes.byref(ts))
         return {"launches": nl.value, "pairs": npairs.value, "kernel": _KERNEL_NAMES.get(ku.value, ku.value),
-                "n_split": ns.value, "chunks": nch.value}
+                "n_split": ns.value, "chunks": nch.value, "tensor_shape": ts.value}
 
     # -- the two calls
     def periodogram_batched(self, offsets, t, y, *, out=None, host_out=None, best: bool = False, h_offsets=None,
                             stream=None):
         """Full periodogram.  Returns (power, best) where power is `out` (device), `host_out` (host) or a new
         device tensor [n_obj, n_freq], and best is None or (period, power, index) device tensors."""
-        n_obj = self._check_inputs(offsets, t, y)
+        n_obj = self._check_inputs(offsets, t, y, h_offsets)
         if host_out is not None:
             if host_out.is_cuda or host_out.dtype != self.torch_dtype or host_out.numel() != n_obj * self.n_freq \
                     or not host_out.is_contiguous():
@@ -246,12 +262,14 @@ class Plan:
         """End-to-end call on HOST tensors (pinned for overlap): fills `host_out` [n_obj, n_freq] (or skips the
         periodogram when None) and `best_out` = (period, power, index) host tensors (optional unless host_out
         is None).  Returns after all results are on the host."""
-        if h_offsets.is_cuda or h_offsets.dtype != torch.int64:
-            raise TypeError("h_offsets must be a host int64 tensor")
+        if h_offsets.is_cuda or h_offsets.dtype != torch.int64 or not h_offsets.is_contiguous() or h_offsets.numel() < 1:
+            raise TypeError("h_offsets must be a contiguous host int64 tensor of n_obj + 1 elements")
         n_obj = int(h_offsets.numel() - 1)
         for x in (h_t, h_y):
             if x.is_cuda or x.dtype != self.torch_dtype or not x.is_contiguous():
                 raise TypeError(f"h_t and h_y must be contiguous host tensors of {self.torch_dtype}")
+        if h_t.numel() != h_y.numel() or int(h_offsets[-1]) > h_t.numel():
+            raise TypeError("h_t and h_y must have the same length, at least offsets[n_obj]")
         if host_out is not None and (host_out.is_cuda or host_out.dtype != self.torch_dtype or not host_out.is_contiguous()
                                      or host_out.numel() != n_obj * self.n_freq):
             raise TypeError("host_out must be a contiguous host tensor [n_obj, n_freq] of the plan dtype")
@@ -267,7 +285,7 @@ class Plan:
     def periodogram_generalized(self, offsets, t, y, sigma, *, out=None, best: bool = False, want_power: bool = True,
                                 h_offsets=None, stream=None):
         """Generalised LSP: (power [n_obj, n_freq] or None, best = (period, power, index) or None), device tensors."""
-        n_obj = self._check_inputs(offsets, t, y)
+        n_obj = self._check_inputs(offsets, t, y, h_offsets)
         if sigma.dtype != self.torch_dtype or not sigma.is_cuda or not sigma.is_contiguous() or sigma.numel() != y.numel():
             raise TypeError("sigma must be a contiguous CUDA tensor like y")
         power = None
@@ -283,9 +301,23 @@ class Plan:
         lsp_periodogram_generalized(self._plan, n_obj, offsets, h_offsets, t, y, sigma, power, bp, bw, bi, stream)
         return power, ((bp, bw, bi) if best else None)
 
+    def best_merge(self, part_power, part_index, *, stream=None):
+        """Merge per-shard (power, GLOBAL index) candidates, tensors [n_parts, n_obj] on this plan's device, into
+        (period, power, index) on this plan's (global) grid.  The tie rule and period = 1/f_k live in the library."""
+        if part_power.dim() != 2 or part_power.shape != part_index.shape or part_power.dtype != self.torch_dtype \
+                or part_index.dtype != torch.int64 or not part_power.is_cuda or not part_index.is_cuda \
+                or not part_power.is_contiguous() or not part_index.is_contiguous():
+            raise TypeError("part_power [n_parts, n_obj] (plan dtype) and part_index [n_parts, n_obj] (int64): contiguous CUDA tensors")
+        n_parts, n_obj = part_power.shape
+        out = (torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),
+               torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),
+               torch.empty(n_obj, dtype=torch.int64, device=self.device))
+        lsp_best_merge(self._plan, n_obj, n_parts, part_power, part_index, out[0], out[1], out[2], stream)
+        return out
+
     def best_period(self, offsets, t, y, *, out=None, h_offsets=None, stream=None):
         """Fused best period: (period, power, index) device tensors; the periodogram is never materialised."""
-        n_obj = self._check_inputs(offsets, t, y)
+        n_obj = self._check_inputs(offsets, t, y, h_offsets)
         if out is None:
             out = (torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),
                    torch.empty(n_obj, dtype=self.torch_dtype, device=self.device),

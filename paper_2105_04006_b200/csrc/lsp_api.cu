@@ -13,13 +13,13 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
 #include <type_traits>
 #include <vector>
 
 #include "lsp_factored_ws.cuh"
 #include "lsp_tensor.cuh"
 #include "lsp_gls.cuh"
-#include "lsp_peak.cuh"
 
 using namespace lsp;
 
@@ -49,7 +49,7 @@ struct lsp_plan {
     struct HostCopy { void* dst; const void* src; size_t bytes; };
     std::vector<HostCopy> host_copies;           // arguments of the per-chunk host memcpy callbacks (stable during a call)
     int pageable_mode = 1;        // 1 = plain cudaMemcpyAsync to a pageable destination (default: faster on the measured host),
-                                  // 0 = staged (pinned ring + host-side copies; LSP_PAGEABLE=staged)
+                                  // 0 = staged (pinned ring + host-side copies; LSP_FLAG_PAGEABLE_STAGED)
     DeviceBuffer partials;        // Best[n_obj * n_parts]
     DeviceBuffer sums;            // Vec4<T>[n_split * n_obj_launch * n_freq]
     DeviceBuffer stats;           // ObjStats[n_obj]
@@ -59,17 +59,20 @@ struct lsp_plan {
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     int tc_stages_b = 3;          // B-operand ring depth of the tensor kernel
-    int tc_roles = 0;             // 0 = by item length, 1 = force (8 epilogue warps, 2 generator groups), 2 = force (4, 3); LSP_TC_ROLES
+    int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
-    bool use_ws = true;           // persistent warp-specialised factored kernel (LSP_FACTORED_IMPL=classic disables)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
     DeviceBuffer gls_x, gls_yy, gls_sums;        // generalised mode: x_A / x_B arrays, chi0^2 per object, 3 passes of partial sums
     int64_t* h_offsets_pinned = nullptr;
     size_t   h_offsets_cap = 0;
+    // Dynamic shared memory opted in per kernel function on THIS plan's device (the attribute is per device, and a plan is
+    // bound to one device): (function, bytes) pairs.
+    std::vector<std::pair<const void*, size_t>> smem_optins;
 
     // last-call bookkeeping
     int64_t n_launches = 0, n_pairs = 0, n_chunks = 0;
     int32_t kernel_used = 0, n_split = 1;
+    int32_t tensor_shape = 0;     // role shape of the last tensor-kernel launch: 0 = none, 1 = short-item, 2 = long-item
     bool timing = false;
     std::vector<cudaEvent_t> t_start, t_stop;
     size_t t_used = 0;
@@ -111,6 +114,31 @@ lsp_status ensure(lsp_plan* p, DeviceBuffer& b, size_t bytes)
 
 size_t elem_size(const lsp_config& c) { return c.dtype == LSP_F32 ? 4 : 8; }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute: remembered per plan (one device), never per process.
+template <typename K>
+cudaError_t optin_smem(lsp_plan* p, K kern, size_t bytes)
+{
+    const void* key = reinterpret_cast<const void*>(kern);
+    for (auto& e : p->smem_optins)
+        if (e.first == key) {
+            if (e.second >= bytes) return cudaSuccess;
+            const cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+            if (err == cudaSuccess) e.second = bytes;
+            return err;
+        }
+    const cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (err == cudaSuccess) p->smem_optins.emplace_back(key, bytes);
+    return err;
+}
+
+// The grid and per-object conventions one launch sequence runs with.  The standard calls use the plan's own; the generalised
+// mode passes derived ones (doubled grid, no centring) BY VALUE -- the plan's public configuration is never scratch space.
+struct GridSpec {
+    double f_min, f_max;
+    int center, normalize;
+};
+GridSpec plan_grid(const lsp_config& c) { return GridSpec{c.f_min, c.f_max, c.center, c.normalize}; }
+
 // ---- step 1: scheduling ------------------------------------------------------------------------------------
 struct Schedule {
     int kernel;      // LSP_KERNEL_DIRECT / LSP_KERNEL_FACTORED
@@ -121,11 +149,11 @@ struct Schedule {
     TensorParams tp;   // tensor path only
 };
 
-Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
+Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int kernel_override = -1)
 {
     const lsp_config& c = p->cfg;
     Schedule s{};
-    int k = c.kernel;
+    int k = kernel_override >= 0 ? kernel_override : c.kernel;
     if (k == LSP_KERNEL_AUTO)
         k = (c.n_freq < 1024) ? LSP_KERNEL_DIRECT : (c.dtype == LSP_F32 ? LSP_KERNEL_TENSOR : LSP_KERNEL_FACTORED);
     s.kernel = k;
@@ -149,8 +177,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs)
     } else if (k == LSP_KERNEL_FACTORED) {
         s.tile = c.dtype == LSP_F32 ? fac_tile<float>() : fac_tile<double>();
         s.direct_r = 0;
-        slots = p->use_ws ? (int64_t)p->sm_count                  // one persistent CTA per SM
-                          : (int64_t)p->sm_count * 2;             // __launch_bounds__(256, 2)
+        slots = (int64_t)p->sm_count;                             // one persistent CTA per SM
     } else {
         const int64_t tiles4 = (c.n_freq + 4 * kDirectThreads - 1) / (4 * kDirectThreads);
         s.direct_r = (n_obj * tiles4 >= (int64_t)p->sm_count * 8) ? 4 : 1;
@@ -201,33 +228,26 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
         if constexpr (std::is_same<T, float>::value) {
             const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.stages_b, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
             const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
-            auto go = [&](auto kern, int threads, size_t& attr_smem) -> cudaError_t {
-                if (smem > attr_smem) {
-                    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-                    if (e != cudaSuccess) return e;
-                    attr_smem = smem;
-                }
+            auto go = [&](auto kern, int threads) -> cudaError_t {
+                const cudaError_t ea = optin_smem(p, kern, smem);
+                if (ea != cudaSuccess) return ea;
                 kern<<<ctas, threads, smem, st>>>(gp, s.tp, d_off, (const float*)d_t, (const float*)d_y,
                                                   (const TensorObj*)p->tc_objs.ptr, (const __half*)p->tc_table.ptr, (float*)out,
                                                   partials, (float4*)sums, n_obj_launch, (long long)grid);
                 return cudaSuccess;
             };
-            static size_t attr_short = 0, attr_long = 0;       // per FAST instantiation
-            cudaError_t e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 3>, TcRoles<4, 3>::kThreads, attr_long)
-                                            : go(lsp_tensor_kernel<float, FAST, 8, 2>, TcRoles<8, 2>::kThreads, attr_short);
+            p->tensor_shape = s.tp.long_items ? 2 : 1;
+            cudaError_t e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 3>, TcRoles<4, 3>::kThreads)
+                                            : go(lsp_tensor_kernel<float, FAST, 8, 2>, TcRoles<8, 2>::kThreads);
             if (e != cudaSuccess) return e;
         } else {
             return cudaErrorInvalidValue;      // rejected at plan creation
         }
-    } else if (s.kernel == LSP_KERNEL_FACTORED && p->use_ws) {
+    } else if (s.kernel == LSP_KERNEL_FACTORED) {
         auto kern = lsp_factored_ws_kernel<T, FAST>;
-        static bool attr_done = false;     // per instantiation
-        if (!attr_done) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ws_smem_bytes<T>());
-            if (e != cudaSuccess) return e;
-            attr_done = true;
-        }
-        cudaError_t e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
+        cudaError_t e = optin_smem(p, kern, ws_smem_bytes<T>());
+        if (e != cudaSuccess) return e;
+        e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return e;
         const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
         using V2 = typename FactoredCfg<T>::V2;
@@ -238,16 +258,6 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
         kern<<<ctas, kWsThreads, ws_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
                                                           (V4*)sums, n_obj_launch, (long long)grid,
                                                           (unsigned long long*)p->counter.ptr, tabV, tabB1, tabB2);
-    } else if (s.kernel == LSP_KERNEL_FACTORED) {
-        auto kern = lsp_factored_kernel<T, FAST>;
-        static bool attr_done = false;     // per instantiation
-        if (!attr_done) {
-            cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fac_smem_bytes<T>());
-            if (e != cudaSuccess) return e;
-            attr_done = true;
-        }
-        kern<<<(unsigned)grid, kFacThreads, fac_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats,
-                                                                     (T*)out, partials, (V4*)sums, n_obj_launch);
     } else if (s.direct_r == 4) {
         lsp_direct_kernel<T, FAST, 4><<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y,
                                                                                  stats, (T*)out, partials, (V4*)sums, n_obj_launch);
@@ -260,7 +270,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 
 // Launches steps 2-6' for objects [obj_base, obj_base + n_obj_launch) on `st`.
 // `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed globally.
-lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
+lsp_status run_range(lsp_plan* p, const Schedule& s, const GridSpec& g, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
                      const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
                      cudaStream_t st, void* ext_sums = nullptr)      // ext_sums: write partial sums there and stop (generalised mode)
 {
@@ -273,13 +283,13 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
         if (e != LSP_OK) return e;
         if ((e = ensure(p, p->tc_table, std::max<size_t>(256, (size_t)kb_bound * (size_t)s.tp.b_stage_bytes))) != LSP_OK) return e;
         GridParams gq{};
-        gq.f_min = c.f_min;
-        gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
+        gq.f_min = g.f_min;
+        gq.df = (g.f_max - g.f_min) / (double)c.n_freq;
         gq.n_freq = (int)c.n_freq;
         gq.obj_base = (int)obj_base;
         const int stats_threads = n_obj_launch < 64 ? 1024 : 128;     // a lone long object gets a full CTA
         lsp_tensor_stats_kernel<float><<<(unsigned)n_obj_launch, stats_threads, 0, st>>>(d_off, (const float*)d_y, (TensorObj*)p->tc_objs.ptr,
-                                                                            (int)obj_base, c.center, c.normalize);
+                                                                            (int)obj_base, g.center, g.normalize);
         lsp_tensor_scan_kernel<<<1, 1024, 0, st>>>(d_off, (TensorObj*)p->tc_objs.ptr, (int)obj_base, (int)n_obj_launch);
         if (kb_bound > 0) {
             if (c.fast_math)
@@ -293,13 +303,13 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, int64_t obj_base, int64_t n
         p->n_launches += 3;
     }
     GridParams gp;
-    gp.f_min = c.f_min;
-    gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gp.f_min = g.f_min;
+    gp.df = (g.f_max - g.f_min) / (double)c.n_freq;
     gp.n_freq = (int)c.n_freq;
     gp.n_tiles = s.n_tiles;
     gp.n_split = s.n_split;
     gp.obj_base = (int)obj_base;
-    const ObjStats* stats = (c.center || c.normalize) ? (const ObjStats*)p->stats.ptr : nullptr;
+    const ObjStats* stats = (g.center || g.normalize) ? (const ObjStats*)p->stats.ptr : nullptr;
     void* sums = nullptr;
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
     if (ext_sums) {
@@ -383,15 +393,15 @@ lsp_status run_finalize(lsp_plan* p, int64_t obj_base, int64_t n_obj_launch, int
     return LSP_OK;
 }
 
-// Pre-pass of the factored WS path: tile-independent phasors of every observation on the plan's CURRENT grid, once per call
+// Pre-pass of the factored WS path: tile-independent phasors of every observation on grid `g`, once per call
 // (per pass in the generalised mode).
-lsp_status build_ws_table(lsp_plan* p, const Schedule& s, const void* d_t, int64_t total_obs, cudaStream_t st)
+lsp_status build_ws_table(lsp_plan* p, const Schedule& s, const GridSpec& g, const void* d_t, int64_t total_obs, cudaStream_t st)
 {
     const lsp_config& c = p->cfg;
-    if (!(s.kernel == LSP_KERNEL_FACTORED && p->use_ws)) return LSP_OK;
+    if (s.kernel != LSP_KERNEL_FACTORED) return LSP_OK;
     GridParams gq{};
-    gq.f_min = c.f_min;
-    gq.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gq.f_min = g.f_min;
+    gq.df = (g.f_max - g.f_min) / (double)c.n_freq;
     gq.n_freq = (int)c.n_freq;
     p->ws_table_obs = total_obs;
     const size_t bytes = c.dtype == LSP_F32 ? ws_table_bytes<float>(total_obs) : ws_table_bytes<double>(total_obs);
@@ -422,6 +432,7 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     const lsp_config& c = p->cfg;
     p->n_launches = p->n_pairs = p->n_chunks = 0;
     p->t_used = 0;
+    p->tensor_shape = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
     const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
@@ -464,12 +475,12 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         ++p->n_launches;
     }
 
+    const GridSpec g = plan_grid(c);
     {
-        lsp_status e = build_ws_table(p, s, d_t, total_obs, st);
+        lsp_status e = build_ws_table(p, s, g, d_t, total_obs, st);
         if (e != LSP_OK) return e;
     }
 
-    int n_parts = 0;
     const size_t es = elem_size(c);
     const size_t row_bytes = (size_t)c.n_freq * es;
     // Host copy of the offsets, fetched only when an object range has to be cut by observation count.
@@ -486,38 +497,41 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         }
         return off_cache.data();
     };
-    if (!out_power || !out_is_host) {
-        // steps 2-6': asynchronous on the caller's stream.  One launch over the whole batch, except on the tensor path
-        // when the B-operand table of the whole batch would exceed its memory budget: then objects go in ranges.
+    // Steps 2-6' for objects [o0, o0 + no) holding `obs` observations, asynchronous on the caller's stream: `out` (device, may be
+    // NULL) receives rows relative to o0.  One launch sequence, except on the tensor path when the B-operand table of the range
+    // would exceed its memory budget: then the objects go in sub-ranges (same results: an object's sums never span launches).
+    auto run_objs = [&](int64_t o0, int64_t no, int64_t obs, void* out) -> lsp_status {
+        int n_parts = 0;
+        const Schedule sc = make_schedule(p, no, obs, s.kernel);
         const bool cut = s.kernel == LSP_KERNEL_TENSOR &&
-                         (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget;
+                         (size_t)(obs / kTcKB + no) * (size_t)sc.tp.b_stage_bytes > p->tc_table_budget;
         if (!cut) {
-            lsp_status e = run_range(p, s, 0, n_obj, total_obs, d_off, d_t, d_y, out_power, want_best, &n_parts, st);
+            lsp_status e = run_range(p, sc, g, o0, no, obs, d_off, d_t, d_y, out, want_best, &n_parts, st);
             if (e != LSP_OK) return e;
-            if (want_best) return run_finalize(p, 0, n_obj, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
-            return LSP_OK;
+            return want_best ? run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st) : LSP_OK;
         }
         const int64_t* ho = host_offsets();
         if (!ho) return fail(p, LSP_ERR_CUDA, "reading offsets back failed");
-        const int64_t kb_cap = (int64_t)(p->tc_table_budget / (size_t)s.tp.b_stage_bytes);
-        for (int64_t o0 = 0; o0 < n_obj;) {
-            int64_t no = 0, kbs = 0;
-            while (o0 + no < n_obj) {
-                const int64_t k = tc_n_kb(ho[o0 + no + 1] - ho[o0 + no]);
-                if (no > 0 && kbs + k > kb_cap) break;
+        const int64_t kb_cap = (int64_t)(p->tc_table_budget / (size_t)sc.tp.b_stage_bytes);
+        for (int64_t a0 = o0; a0 < o0 + no;) {
+            int64_t na = 0, kbs = 0;
+            while (a0 + na < o0 + no) {
+                const int64_t k = tc_n_kb(ho[a0 + na + 1] - ho[a0 + na]) + 1;      // + 1: the table's per-object slack block
+                if (na > 0 && kbs + k > kb_cap) break;
                 kbs += k;
-                ++no;
+                ++na;
             }
-            Schedule sc = make_schedule(p, no, ho[o0 + no] - ho[o0]);
-            sc.kernel = s.kernel;
-            lsp_status e = run_range(p, sc, o0, no, ho[o0 + no] - ho[o0], d_off, d_t, d_y,
-                                     out_power ? (char*)out_power + (size_t)o0 * row_bytes : nullptr, want_best, &n_parts, st);
+            const int64_t obs_a = ho[a0 + na] - ho[a0];
+            const Schedule sa = make_schedule(p, na, obs_a, s.kernel);
+            lsp_status e = run_range(p, sa, g, a0, na, obs_a, d_off, d_t, d_y,
+                                     out ? (char*)out + (size_t)(a0 - o0) * row_bytes : nullptr, want_best, &n_parts, st);
             if (e != LSP_OK) return e;
-            if (want_best && (e = run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
-            o0 += no;
+            if (want_best && (e = run_finalize(p, a0, na, n_parts, d_off, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+            a0 += na;
         }
         return LSP_OK;
-    }
+    };
+    if (!out_power || !out_is_host) return run_objs(0, n_obj, total_obs, out_power);
 
     // ---- step 7: chunked compute -> event -> copy streams -> (pinned) host -------------------
     const size_t chunk_bytes = c.chunk_bytes > 0 ? (size_t)c.chunk_bytes : ((size_t)64 << 20);
@@ -552,22 +566,18 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         p->host_copies.assign((size_t)((n_obj + objs_per_chunk - 1) / objs_per_chunk), lsp_plan::HostCopy{});
     }
     std::fill(p->slot_used.begin(), p->slot_used.end(), 0);
-    // a chunk's schedule is made for the chunk's own object count, so small chunks still split observations
+    // a chunk's schedule is made for the chunk's own object and observation counts (so small chunks still split observations
+    // and the tensor path's operand table is sized for the chunk, not the batch): the offsets are needed on the host
+    const int64_t* ho = (n_obj > objs_per_chunk) ? host_offsets() : nullptr;
+    if (n_obj > objs_per_chunk && !ho) return fail(p, LSP_ERR_CUDA, "reading offsets back failed");
     int64_t chunk = 0;
     for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_chunk, ++chunk) {
         const int64_t no = std::min(objs_per_chunk, n_obj - o0);
         const int slot = (int)(chunk % n_slots);
         char* dslot = (char*)p->ring.ptr + (size_t)slot * slot_bytes;
         if (p->slot_used[slot]) LSP_CUDA(p, cudaStreamWaitEvent(st, p->slot_free[slot], 0));
-        const int64_t obs_est = h_off ? (h_off[o0 + no] - h_off[o0]) : total_obs / n_obj * no;
-        Schedule sc = make_schedule(p, no, obs_est);
-        sc.kernel = s.kernel;
-        lsp_status e = run_range(p, sc, o0, no, h_off ? obs_est : total_obs, d_off, d_t, d_y, dslot, want_best, &n_parts, st);
+        lsp_status e = run_objs(o0, no, ho ? ho[o0 + no] - ho[o0] : total_obs, dslot);
         if (e != LSP_OK) return e;
-        if (want_best) {
-            e = run_finalize(p, o0, no, n_parts, d_off, d_best_period, d_best_power, d_best_index, st);
-            if (e != LSP_OK) return e;
-        }
         LSP_CUDA(p, cudaEventRecord(p->slot_ready[slot], st));
         cudaStream_t cs = p->copy_streams[chunk % p->copy_streams.size()];
         LSP_CUDA(p, cudaStreamWaitEvent(cs, p->slot_ready[slot], 0));
@@ -613,7 +623,11 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     if (cfg->kernel < LSP_KERNEL_AUTO || cfg->kernel > LSP_KERNEL_TENSOR) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown kernel");
     if (cfg->kernel == LSP_KERNEL_TENSOR && cfg->dtype != LSP_F32)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "the tensor-core kernel is FP32-mode only (FP16-split operands, FP32 accumulation)");
-    if (cfg->reserved != 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "reserved must be 0");
+    if (cfg->flags & ~LSP_FLAG_PAGEABLE_STAGED) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown bit in flags");
+    if (cfg->table_budget_bytes < 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "table_budget_bytes < 0");
+    if (cfg->tensor_roles < 0 || cfg->tensor_roles > 2) return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_roles must be 0, 1 or 2");
+    if (cfg->tensor_b_stages != 0 && (cfg->tensor_b_stages < 2 || cfg->tensor_b_stages > 8))
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_b_stages must be 0 or 2..8");
     if (cfg->n_copy_streams < 0 || cfg->n_copy_streams > 16 || cfg->chunk_bytes < 0 || cfg->max_objects < 0 || cfg->max_total_obs < 0)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "negative / oversized sizing field");
     int n_dev = 0;
@@ -648,10 +662,10 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     }
     p->sm_count = prop.multiProcessorCount;
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
-    if (const char* b = getenv("LSP_TABLE_BUDGET_MB")) p->tc_table_budget = (size_t)std::max(1L, atol(b)) << 20;
-    if (const char* b = getenv("LSP_PAGEABLE")) p->pageable_mode = strcmp(b, "staged") == 0 ? 0 : 1;
-    if (const char* b = getenv("LSP_TC_ROLES")) p->tc_roles = (int)std::min(2L, std::max(0L, atol(b)));
-    if (const char* b = getenv("LSP_TC_SB")) p->tc_stages_b = (int)std::min(6L, std::max(2L, atol(b)));
+    if (cfg->table_budget_bytes > 0) p->tc_table_budget = (size_t)cfg->table_budget_bytes;
+    p->pageable_mode = (cfg->flags & LSP_FLAG_PAGEABLE_STAGED) ? 0 : 1;
+    p->tc_roles = cfg->tensor_roles;
+    if (cfg->tensor_b_stages > 0) p->tc_stages_b = cfg->tensor_b_stages;
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
         cudaStream_t s;
@@ -667,7 +681,6 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     }
     p->slot_used.assign(n_slots, 0);
     if (ensure(p, p->counter, 64) != LSP_OK) return bail(LSP_ERR_OOM);
-    if (const char* impl = getenv("LSP_FACTORED_IMPL")) p->use_ws = strcmp(impl, "classic") != 0;
     if (cfg->max_objects > 0) {
         const int tile = cfg->dtype == LSP_F32 ? fac_tile<float>() : fac_tile<double>();
         const size_t parts = (size_t)std::max<int64_t>((cfg->n_freq + tile - 1) / tile,
@@ -710,6 +723,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     if (!p) return LSP_ERR_INVALID_ARG;
     p->n_launches = p->n_pairs = p->n_chunks = 0;
     p->t_used = 0;
+    p->tensor_shape = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
     const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
@@ -736,10 +750,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     if (total_obs > 0 && (!d_t || !d_y || !d_sigma)) return fail(p, LSP_ERR_INVALID_ARG, "d_t / d_y / d_sigma is NULL");
 
     // The three passes run the standard kernels on derived inputs: y is already weighted and centred (center / normalize off),
-    // pass C runs on the doubled grid.  The configuration is restored before returning.
-    const lsp_config saved = p->cfg;
-    struct Restore { lsp_plan* p; lsp_config c; ~Restore() { p->cfg = c; } } restore{p, saved};
-    p->cfg.center = p->cfg.normalize = 0;
+    // pass C runs on the doubled grid.  Each pass gets its grid by value; the plan's configuration is never modified.
     const lsp_config& c = p->cfg;
     const size_t es = elem_size(c);
     lsp_status e;
@@ -758,10 +769,9 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     if (s.kernel == LSP_KERNEL_TENSOR &&
         (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget) {
         // the tensor path's operand table of the whole batch does not fit: AUTO falls back to the FMA-pipe kernel
-        if (saved.kernel != LSP_KERNEL_AUTO)
+        if (c.kernel != LSP_KERNEL_AUTO)
             return fail(p, LSP_ERR_UNSUPPORTED, "generalised mode on the tensor path: batch too large for the operand table (use kernel = factored)");
-        p->cfg.kernel = LSP_KERNEL_FACTORED;
-        s = make_schedule(p, n_obj, total_obs);
+        s = make_schedule(p, n_obj, total_obs, LSP_KERNEL_FACTORED);
     }
     p->kernel_used = s.kernel;
     p->n_split = s.n_split;
@@ -777,15 +787,13 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
         if ((e = ensure(p, p->gls_sums, 3 * pass_bytes)) != LSP_OK) return e;
         int n_parts = 0;
         for (int pass = 0; pass < 3; ++pass) {
-            p->cfg.f_min = saved.f_min * (pass == 2 ? 2.0 : 1.0);
-            p->cfg.f_max = saved.f_max * (pass == 2 ? 2.0 : 1.0);
-            if ((e = build_ws_table(p, s, d_t, total_obs, st)) != LSP_OK) return e;
-            e = run_range(p, s, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st,
+            const double fs = pass == 2 ? 2.0 : 1.0;
+            const GridSpec g{c.f_min * fs, c.f_max * fs, 0, 0};
+            if ((e = build_ws_table(p, s, g, d_t, total_obs, st)) != LSP_OK) return e;
+            e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st,
                           (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes);
             if (e != LSP_OK) return e;
         }
-        p->cfg.f_min = saved.f_min;
-        p->cfg.f_max = saved.f_max;
         GridParams gp;
         gp.f_min = c.f_min;
         gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
@@ -865,6 +873,35 @@ lsp_status lsp_periodogram_batched_host(lsp_plan* plan, int64_t n_obj, const int
     return LSP_OK;
 }
 
+lsp_status lsp_best_merge(lsp_plan* plan, int64_t n_obj, int32_t n_parts, const void* d_part_power,
+                          const int64_t* d_part_index, void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                          void* cuda_stream)
+{
+    lsp_plan* p = plan;
+    if (!p) return LSP_ERR_INVALID_ARG;
+    if (n_obj < 0 || n_parts < 1) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0 or n_parts < 1");
+    if (n_obj == 0) return LSP_OK;
+    if (!d_part_power || !d_part_index || !d_best_period || !d_best_power || !d_best_index)
+        return fail(p, LSP_ERR_INVALID_ARG, "lsp_best_merge: NULL argument");
+    const lsp_config& c = p->cfg;
+    LSP_CUDA(p, cudaSetDevice(c.device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GridParams gp{};
+    gp.f_min = c.f_min;
+    gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gp.n_freq = (int)c.n_freq;
+    const unsigned grid = (unsigned)((n_obj + 127) / 128);
+    if (c.dtype == LSP_F32)
+        lsp_merge_best_kernel<float><<<grid, 128, 0, st>>>(gp, (const float*)d_part_power, d_part_index, n_parts, n_obj,
+                                                          (float*)d_best_period, (float*)d_best_power, d_best_index);
+    else
+        lsp_merge_best_kernel<double><<<grid, 128, 0, st>>>(gp, (const double*)d_part_power, d_part_index, n_parts, n_obj,
+                                                           (double*)d_best_period, (double*)d_best_power, d_best_index);
+    LSP_CUDA(p, cudaGetLastError());
+    p->n_launches = 1;
+    return LSP_OK;
+}
+
 void lsp_destroy(lsp_plan* p)
 {
     if (!p) return;
@@ -891,9 +928,10 @@ const char* lsp_last_error(const lsp_plan* plan)
 }
 
 void lsp_last_call_info(const lsp_plan* p, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used, int32_t* n_split,
-                        int64_t* n_chunks)
+                        int64_t* n_chunks, int32_t* tensor_shape)
 {
     if (!p) return;
+    if (tensor_shape) *tensor_shape = p->tensor_shape;
     if (n_launches) *n_launches = p->n_launches;
     if (n_pairs) *n_pairs = p->n_pairs;
     if (kernel_used) *kernel_used = p->kernel_used;
@@ -917,51 +955,6 @@ float lsp_last_kernel_ms(lsp_plan* p)
         total += ms;
     }
     return total;
-}
-
-lsp_status lsp_pipe_peak(int32_t device, int32_t which, double* ops_per_s, double* elapsed_ms)
-{
-    if (!ops_per_s || which < 0 || which > 4) return fail(nullptr, LSP_ERR_INVALID_ARG, "lsp_pipe_peak: bad argument");
-    lsp_plan* p = nullptr;
-    LSP_CUDA(p, cudaSetDevice(device));
-    cudaDeviceProp prop;
-    LSP_CUDA(p, cudaGetDeviceProperties(&prop, device));
-    void* out = nullptr;
-    LSP_CUDA(p, cudaMalloc(&out, 64));
-    cudaEvent_t e0, e1;
-    LSP_CUDA(p, cudaEventCreate(&e0));
-    LSP_CUDA(p, cudaEventCreate(&e1));
-    const int ctas_per_sm = (which == 4) ? 2 : 4;
-    const unsigned grid = (unsigned)(prop.multiProcessorCount * ctas_per_sm * 4);    // 4 full waves
-    double ops_per_thread = 0.0;
-    float best_ms = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {                      // rep 0 is the warm-up
-        LSP_CUDA(p, cudaEventRecord(e0, 0));
-        switch (which) {
-            case 0: peak_ffma_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
-                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
-            case 1: peak_ffma2_kernel<<<grid, kPeakThreads>>>((float*)out, 1.0000001f, 1e-9f);
-                    ops_per_thread = 2.0 * kPeakIters * kPeakIlp; break;
-            case 2: peak_dfma_kernel<<<grid, kPeakThreads>>>((double*)out, 1.0000001, 1e-9);
-                    ops_per_thread = (double)kPeakIters * kPeakIlp; break;
-            case 3: peak_mufu_kernel<<<grid, kPeakThreads>>>((float*)out, 0.001f);
-                    ops_per_thread = 2.0 * (kPeakIters / 4) * kPeakIlp; break;
-            default: peak_mix_kernel<<<grid, kPeakThreads>>>((float*)out, 0.5f);
-                    ops_per_thread = 2.0 * 32.0 * 16.0 * (kPeakIters / 16); break;
-        }
-        LSP_CUDA(p, cudaGetLastError());
-        LSP_CUDA(p, cudaEventRecord(e1, 0));
-        LSP_CUDA(p, cudaEventSynchronize(e1));
-        float ms = 0.f;
-        LSP_CUDA(p, cudaEventElapsedTime(&ms, e0, e1));
-        if (rep > 0) best_ms = std::min(best_ms, ms);
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(out);
-    *ops_per_s = ops_per_thread * (double)grid * kPeakThreads / (best_ms * 1e-3);
-    if (elapsed_ms) *elapsed_ms = best_ms;
-    return LSP_OK;
 }
 
 const char* lsp_version(void)

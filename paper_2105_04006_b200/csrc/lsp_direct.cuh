@@ -217,6 +217,34 @@ __global__ void lsp_finalize_best_kernel(GridParams gp, const int64_t* __restric
     }
 }
 
+// Step 6' across frequency shards: merges, per object, the fused-argmax results of n_parts runs that each
+// covered a contiguous slice of ONE global grid.  part_index holds GLOBAL grid indices (-1 = the slice had no valid frequency).
+// Same rule as everywhere: largest power, lowest index on exact ties, NaN / -1 never win; period = 1/f_k on the global grid.
+template <typename T>
+__global__ void lsp_merge_best_kernel(GridParams gp, const T* __restrict__ part_power, const int64_t* __restrict__ part_index,
+                                      int n_parts, int64_t n_obj, T* __restrict__ best_period, T* __restrict__ best_power,
+                                      int64_t* __restrict__ best_index)
+{
+    const int64_t obj = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (obj >= n_obj) return;
+    Best v;
+    v.p = -2.0;
+    v.k = INT64_MAX;
+    for (int i = 0; i < n_parts; ++i) {
+        const T pw = part_power[(int64_t)i * n_obj + obj];
+        const int64_t k = part_index[(int64_t)i * n_obj + obj];
+        if (k < 0 || k >= gp.n_freq || !(pw == pw)) continue;
+        Best b;
+        b.p = (double)pw;
+        b.k = k;
+        v = best_of(v, b);
+    }
+    const bool empty = v.k == INT64_MAX;
+    best_index[obj] = empty ? -1 : v.k;
+    best_power[obj] = empty ? T(0) : (T)v.p;
+    best_period[obj] = empty ? (T)NAN : (T)(1.0 / (gp.f_min + (double)v.k * gp.df));
+}
+
 // Step 1 pre-pass (only when center=1 or normalize=1): per-object mean and 1/(0.5 sum (y-mean)^2).
 template <typename T>
 __global__ void lsp_object_stats_kernel(const int64_t* __restrict__ offsets, const T* __restrict__ y,

@@ -5,11 +5,12 @@ Every (object, frequency) power is independent, so the path
 * a batch is cut into contiguous object ranges balanced by sum N_t (`partition_objects`); each rank runs the
   library on its own CSR slice (`slice_csr`) and owns those rows / best periods: no data-path collective;
 * a single huge object is cut by frequency range (`partition_frequencies`); the full periodogram needs nothing,
-  the best period needs one max-reduce of (power, index) per object (`reduce_best`: an all-gather of 16 bytes per
-  object per rank, lowest index wins exact ties, NaN never wins -- the library's own rule, DESIGN.md a7).
+  the best period needs one max-reduce of (power, index) per object: `gather_best` all-gathers 16 bytes per object per
+  rank and the library's `lsp_best_merge` (include/lsp.h) picks the winner with its own rule (DESIGN.md a7).
 
-This module holds plumbing only (integer partitioning and one argmax over ranks); it never evaluates a periodogram
-and works with any torch.distributed backend (nccl on GPUs; gloo in the CPU tests).
+This module holds plumbing only (integer partitioning, CSR slicing, all-gathers); it never evaluates a periodogram, an
+argmax or a period -- those live behind the C ABI -- and works with any torch.distributed backend (nccl on GPUs; gloo in
+the CPU tests).
 """
 from __future__ import annotations
 
@@ -66,31 +67,36 @@ def partition_frequencies(f_min: float, f_max: float, n_freq: int, world: int):
     return out
 
 
-def reduce_best(power: torch.Tensor, index: torch.Tensor, k_offset: int, f_min: float, f_max: float, n_freq: int,
-                group=None):
-    """Best period over frequency-sharded ranks.  `power[n_obj]` / `index[n_obj]` are this rank's fused-argmax results
-    on its own grid slice (index -1 = no valid frequency); `k_offset` is the slice's first global frequency number.
-    Returns (period, power, global index) on every rank.  One all-gather of (power, index) per object; the winner is
-    the largest power, lowest global index on exact ties, NaN / -1 entries never win."""
+def gather_best(power: torch.Tensor, index: torch.Tensor, k_offset: int, group=None):
+    """Frequency-sharded best period, plumbing half: every rank contributes its fused-argmax results on its own grid
+    slice (`power[n_obj]`, `index[n_obj]` with -1 = no valid frequency; `k_offset` = the slice's first GLOBAL frequency
+    number) and receives the candidates of all ranks as (part_power [world, n_obj], part_index [world, n_obj], GLOBAL
+    indices, -1 kept).  One all-gather of 16 bytes per object per rank; no arithmetic on the powers happens here -- the
+    winner is picked by the library (`Plan.best_merge` = lsp_best_merge of include/lsp.h: largest power, lowest index on
+    exact ties, NaN / -1 never win, period = 1/f_k on the global grid)."""
     import torch.distributed as dist
     world = dist.get_world_size(group)
     gidx = torch.where(index >= 0, index + int(k_offset), torch.full_like(index, -1))
-    p64 = power.to(torch.float64)
-    p64 = torch.where(torch.isnan(p64) | (gidx < 0), torch.full_like(p64, -float("inf")), p64)
-    ps = [torch.empty_like(p64) for _ in range(world)]
+    ps = [torch.empty_like(power) for _ in range(world)]
     ks = [torch.empty_like(gidx) for _ in range(world)]
-    dist.all_gather(ps, p64, group=group)
+    dist.all_gather(ps, power.contiguous(), group=group)
     dist.all_gather(ks, gidx, group=group)
-    P = torch.stack(ps)                          # [world, n_obj]
-    K = torch.stack(ks)
-    pmax = P.max(dim=0).values
-    big = torch.iinfo(torch.int64).max
-    cand = torch.where((P == pmax.unsqueeze(0)) & (K >= 0), K, torch.full_like(K, big))
-    kbest = cand.min(dim=0).values
-    none = kbest == big
-    kbest = torch.where(none, torch.full_like(kbest, -1), kbest)
-    df = (f_max - f_min) / n_freq
-    period = 1.0 / (f_min + kbest.to(torch.float64) * df)
-    period = torch.where(none, torch.full_like(period, float("nan")), period)
-    pw = torch.where(none, torch.zeros_like(pmax), pmax)
-    return period.to(power.dtype), pw.to(power.dtype), kbest
+    return torch.stack(ps), torch.stack(ks)
+
+
+def gather_objects(best, counts: List[int], group=None):
+    """Object-sharded batch, plumbing half: rank r holds (period, power, index) tensors of its own counts[r] objects;
+    returns the three arrays of the whole batch, in object order, on every rank (ranges from `partition_objects` are
+    contiguous and ordered, so concatenation by rank is the batch order).  No arithmetic."""
+    import torch.distributed as dist
+    world = dist.get_world_size(group)
+    assert len(counts) == world
+    n_max = max(counts) if counts else 0
+    out = []
+    for x in best:
+        pad = torch.zeros(n_max, dtype=x.dtype, device=x.device)
+        pad[:x.numel()] = x
+        parts = [torch.empty_like(pad) for _ in range(world)]
+        dist.all_gather(parts, pad, group=group)
+        out.append(torch.cat([parts[r][:counts[r]] for r in range(world)]))
+    return tuple(out)

@@ -1,7 +1,9 @@
 """Host-side sharding plumbing (paper_2105_04006_b200/sharding.py), covered on CPU with
-world_size-2 gloo: object partition of a batch (no collective on the data path) and the (power, index) max-reduce that a
-frequency-sharded single object needs for its best period.  The per-rank "periodograms" here come from the CPU oracle
-(test infrastructure): what is under test is the partitioning and the reduce, not a kernel.
+world_size-2 gloo: object partition of a batch (no collective on the data path), the gather of per-rank best periods,
+and the (power, GLOBAL index) all-gather that a frequency-sharded object needs before the library's lsp_best_merge picks
+the winner.  The per-rank "periodograms" here come from the CPU oracle and the merge rule is restated in this file
+(test infrastructure): what is under test is the partitioning and the gathers, not a kernel.  The CUDA library on
+shards -- including lsp_best_merge itself -- is covered by tests/test_gpu_parity.py (-m gpu).
 """
 import os
 import socket
@@ -83,7 +85,10 @@ def _worker(rank: int, world: int, port: int, mode: str, q):
             o0, o1 = sharding.partition_objects(w.offsets, world)[rank]
             off, t, y = sharding.slice_csr(w.offsets, w.t, w.y, o0, o1)
             P = oracle.periodogram(off, t, y, w.f_min, w.f_max, w.n_freq)
-            q.put((rank, o0, o1, P))
+            idx, pw, per = oracle.best(off, P, w.f_min, w.f_max, w.n_freq)
+            counts = [b - a for a, b in sharding.partition_objects(w.offsets, world)]
+            allb = sharding.gather_objects((torch.from_numpy(per), torch.from_numpy(pw), torch.from_numpy(idx)), counts)
+            q.put((rank, o0, o1, P, tuple(x.numpy() for x in allb)))
         else:
             # one object sharded by frequency range + the best-period max-reduce, with a planted exact tie across ranks
             w = make_config(1)
@@ -92,11 +97,25 @@ def _worker(rank: int, world: int, port: int, mode: str, q):
             idx, pw, _ = oracle.best(w.offsets, P, fa, fb, k1 - k0)
             power = torch.tensor([pw[0], 7.0, float("nan") if rank == 0 else 1.0, 0.0], dtype=torch.float64)
             index = torch.tensor([idx[0], 5, 3, -1], dtype=torch.int64)
-            per, bp, bk = sharding.reduce_best(power, index, k0, w.f_min, w.f_max, w.n_freq)
-            q.put((rank, k0, P, per.numpy(), bp.numpy(), bk.numpy()))
+            pp, pk = sharding.gather_best(power, index, k0)
+            per, bp, bk = _merge_rule_a7(pp.numpy(), pk.numpy(), w.f_min, w.f_max, w.n_freq)
+            q.put((rank, k0, P, per, bp, bk))
         dist.barrier()
     finally:
         dist.destroy_process_group()
+
+
+def _merge_rule_a7(part_power, part_index, f_min, f_max, n_freq):
+    """DESIGN.md reading a7 written out for the test: largest power wins, lowest GLOBAL index on exact ties, NaN / -1 never."""
+    n_obj = part_power.shape[1]
+    per, bp, bk = np.full(n_obj, np.nan), np.zeros(n_obj), np.full(n_obj, -1, dtype=np.int64)
+    for o in range(n_obj):
+        cands = [(part_power[r, o], part_index[r, o]) for r in range(part_power.shape[0])
+                 if part_index[r, o] >= 0 and not np.isnan(part_power[r, o])]
+        if cands:
+            p, k = sorted(cands, key=lambda c: (-c[0], c[1]))[0]
+            per[o], bp[o], bk[o] = 1.0 / (f_min + k * (f_max - f_min) / n_freq), p, k
+    return per, bp, bk
 
 
 def _run(mode: str, world: int = 2):
@@ -117,10 +136,13 @@ def _run(mode: str, world: int = 2):
 def test_object_sharded_batch_gloo_world2(oracle):
     w = make_config(3, n_obj=12, n_freq=300)
     P_all = oracle.periodogram(w.offsets, w.t, w.y, w.f_min, w.f_max, w.n_freq)
+    ridx, rpw, rper = oracle.best(w.offsets, P_all, w.f_min, w.f_max, w.n_freq)
     rows = 0
-    for rank, o0, o1, P in _run("objects"):
+    for rank, o0, o1, P, allb in _run("objects"):
         assert np.array_equal(P, P_all[o0:o1])          # same arithmetic on the same rows: bit-identical
         rows += o1 - o0
+        # every rank ends with the whole batch's best periods, in object order
+        assert np.array_equal(allb[2], ridx) and np.array_equal(allb[1], rpw) and np.array_equal(allb[0], rper)
     assert rows == w.n_obj
 
 
