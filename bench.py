@@ -1,25 +1,34 @@
 #!/usr/bin/env python
 """bench.py -- (t,f) pair-evaluations/s of the batched Lomb-Scargle hot path on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4] [--dtype f32|f64] [--fast-math]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4|c5] [--dtype f32|f64] [--fast-math] [--variants]
     python bench.py --impl reference ...          # the CPU oracle, as it stands, on the box's host cores
 
 A "step" is one pass of the whole hot path (SURVEY.md section 8(a) steps 1-6/6', and 7 for host output) over one
 batch of seeded synthetic input.  Default workload: BASELINE.json configs[1] (single object, N_t = 10,000,
-N_f = 1,000,000, full periodogram), in FP32 (primary line) and FP64 (the "fp64" object of the same line).
+N_f = 1,000,000, full periodogram) in FP32 (the primary keys).  The same line then carries, as short objects,
+  fp64           the same workload in FP64 (value, e2e, roofline)
+  fp32_fma_pipe  the all-FP32 FFMA2 contraction on the FMA pipe (north_star's "FP32 issue-bound roofline")
+  c3, c4         BASELINE.json configs[2] (batch, fused best period) and configs[3] (4 GB of periodograms to pinned host
+                 through the copy streams: T_compute, T_d2h, T_pipelined)
+and, with --variants, the comparison legs (fast_math, the paper-shaped direct kernels, the generalised mode).
   value       device-resident: inputs and output in HBM, CUDA events around each step on the launching stream
   e2e         the same pass through lsp_periodogram_batched_host: pinned HOST inputs, H2D + kernels + D2H inside
               the timed region
-  roofline    the dominant kernel against the FMA-pipe (FP32) / FP64-pipe peak: "bound": "alu"
+  roofline    the dominant kernel: tensor peak for the tcgen05 kernel, FMA / FP64 pipe peak for the FMA-pipe kernels
   cpu_baseline  the oracle timed on a bounded sample of the same workload (rank 0, N = 1 only)
-Multi-GPU (torchrun, one rank per GPU): every rank runs its own object of the same shape (seed + rank), no data-path
-collective ("scaling": "weak"); times are device times, max over ranks.
+Multi-GPU (torchrun, one rank per GPU): c2 -- every rank runs its own object of the same shape (seed + rank), "scaling":
+"weak"; c3 -- ONE batch is cut by `sharding.partition_objects` (balanced by sum N_t), every rank runs the library on its
+own CSR slice and the best periods are gathered, "scaling": "strong".  No data-path collective; device times, max over ranks.
 """
 from __future__ import annotations
 
 import argparse
+import ctypes
+import csv
 import json
 import os
+import subprocess
 import sys
 import threading
 import time
@@ -43,9 +52,62 @@ TENSOR_PRODUCTS = {False: 3, True: 1}
 TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 burst; fp16 : bf16 nominal ratio is 1)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel on config 2, from the committed
-# `ncu --set full` captures (profiles/r01_ncu_full_*.csv; commands in profiles/r01_README.md).  Other workloads: null.
-NCU_TRAFFIC_C2 = {("tensor", False): 20.83e6 + 58.40e6, ("factored", "f32"): 5.94e6 + 0.37e6, ("factored", "f64"): 6.65e6 + 42.69e6}
+# roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, READ at run time from the
+# committed `ncu --set full` summary of the same workload and kernel (profiles/*.csv; the commands are in the README beside
+# them).  No capture for this (workload, kernel) -> null.  Newest round first.
+NCU_SUMMARIES = {
+    ("c2", "tensor", "f32"): ("profiles/r02_ncu_full_tensor_f32_c2.csv", "profiles/r01_ncu_full_tensor_f32_c2.csv"),
+    ("c3", "tensor", "f32"): ("profiles/r02_ncu_full_tensor_f32_c3.csv", "profiles/r01_ncu_full_tensor_f32_c3.csv"),
+    ("c2", "factored", "f32"): ("profiles/r02_ncu_full_factored_ws_f32.csv", "profiles/r01_ncu_full_factored_ws_f32.csv"),
+    ("c2", "factored", "f64"): ("profiles/r02_ncu_full_factored_ws_f64.csv", "profiles/r01_ncu_full_factored_ws_f64.csv"),
+}
+
+
+def ncu_traffic(workload: str, kernel: str, dtype: str):
+    """(bytes per launch, file) from the newest committed ncu summary of this workload / kernel, or (None, None)."""
+    for rel in NCU_SUMMARIES.get((workload, kernel, dtype), ()):
+        path = os.path.join(ROOT, rel)
+        if not os.path.exists(path):
+            continue
+        tot = {}
+        with open(path, newline="") as fh:
+            for row in csv.DictReader(fh):
+                if row.get("metric") in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+                    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(row.get("unit", ""), None)
+                    if scale is not None:
+                        tot[row["metric"]] = float(row["value"]) * scale
+        if len(tot) == 2:
+            return sum(tot.values()), rel
+    return None, None
+
+
+_PEAK_LIB = None
+
+
+def pipe_peak(which: int, device: int):
+    """(ops_per_s, elapsed_ms) of the register-only pipe microbenchmark `which` (bench_peak.cu: 1 = FFMA2, 2 = DFMA, ...).
+    A bench-only helper library built beside this file; it is not part of liblsp_b200.so."""
+    global _PEAK_LIB
+    if _PEAK_LIB is None:
+        _PEAK_LIB = ctypes.CDLL(build_peak_lib())
+        _PEAK_LIB.bench_pipe_peak.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+        _PEAK_LIB.bench_pipe_peak.restype = ctypes.c_int
+    ops, ms = ctypes.c_double(), ctypes.c_double()
+    rc = _PEAK_LIB.bench_pipe_peak(int(device), int(which), ctypes.byref(ops), ctypes.byref(ms))
+    if rc != 0:
+        raise RuntimeError(f"bench_pipe_peak failed with cudaError {rc}")
+    return ops.value, ms.value
+
+
+def build_peak_lib(force: bool = False) -> str:
+    """nvcc -> libbench_peak.so beside bench.py (sm_100a; cross-compiles without a GPU)."""
+    src, lib = os.path.join(ROOT, "bench_peak.cu"), os.path.join(ROOT, "libbench_peak.so")
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        nvcc = os.environ.get("NVCC") or "/usr/local/cuda/bin/nvcc"
+        subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
+                        "-shared", "-o", lib + ".tmp", src], check=True)
+        os.replace(lib + ".tmp", lib)
+    return lib
 
 
 def measured_tensor_peak():
@@ -61,14 +123,13 @@ def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pip
     """Roofline object of the dominant kernel: achieved = algorithmic flop per launch
     (8 flop per (t,f) pair x pairs) / mean launch duration measured with CUDA events on the launching stream."""
     achieved = pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
-    traffic = None
-    if workload == "c2":
-        traffic = NCU_TRAFFIC_C2.get((kernel, bool(fast)) if kernel == "tensor" else (kernel, dtype))
+    traffic, traffic_from = (None, None) if fast else ncu_traffic(workload, kernel, dtype)
     if kernel == "tensor":
         peak, prov = measured_tensor_peak()
         prod = TENSOR_PRODUCTS[bool(fast)]
         return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
+                "traffic": traffic, "traffic_from": traffic_from,
+                "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
                 "peak_is": prov,
                 "executed_flop_per_pair": FLOP_PER_PAIR * prod,
                 "executed_tflops": achieved * prod, "frac_executed": achieved * prod / peak,
@@ -91,7 +152,7 @@ def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pip
                 "kernel": "lsp_direct_kernel", "ops_per_pair": ops,
                 "peak_is": "derived: 148 SMs x %d lanes/clk/SM x 1965 MHz, %s" % (lanes_, what)}
     return {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
-            "kernel": "lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double"),
+            "traffic_from": traffic_from, "kernel": "lsp_factored_ws_kernel<%s>" % ("float" if dtype == "f32" else "double"),
             "flop_per_pair": FLOP_PER_PAIR,
             "peak_is": "derived: 148 SMs x %d %s FMA lanes/clk/SM x 2 flop x 1965 MHz (clocks.max.sm)" % (lanes, "FP32" if dtype == "f32" else "FP64"),
             "pipe_peak_measured": pipe_ops * 2 / 1e12, "frac_of_measured_pipe": achieved / (pipe_ops * 2 / 1e12)}
@@ -108,16 +169,26 @@ def parse_args():
     ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
     ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored", "tensor"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-secondary", action="store_true", help="skip the other-precision leg")
+    ap.add_argument("--no-secondary", action="store_true", help="primary leg only (no fp64 / fp32_fma_pipe / c3 / c4 objects)")
+    ap.add_argument("--variants", action="store_true", help="add the comparison legs: fast_math, direct kernels, generalised mode")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
     return ap.parse_args()
 
 
-def workload_for(name: str, dtype: str, rank: int):
-    from workloads import make_config
+def workload_for(name: str, dtype: str, rank: int, world: int = 1):
+    """This rank's input.  c2 / c4 / c5: weak scaling, rank r draws its own object(s) from the same generator with sweep-point
+    index r.  c3 with world > 1: ONE batch (the config's own seed), cut into contiguous object ranges balanced by sum N_t
+    (sharding.partition_objects); rank r gets its CSR slice -- strong scaling, no data-path collective."""
+    from workloads import make_config, Workload
     from workloads.configs import config_seed  # noqa: F401  (seed recipe: DESIGN.md "Input recipe")
     cfg = {"c2": 2, "c3": 3, "c4": 4, "c5": 5}[name]
-    # weak scaling: rank r draws its own object(s) from the same generator with sweep-point index r
+    if name == "c3" and world > 1:
+        from paper_2105_04006_b200 import sharding
+        w = make_config(cfg, dtype=dtype)
+        o0, o1 = sharding.partition_objects(w.offsets, world)[rank]
+        off, t, y = sharding.slice_csr(w.offsets, w.t, w.y, o0, o1)
+        return Workload(w.name, off.copy(), t, y, w.f_min, w.f_max, w.n_freq, dtype,
+                        meta={"shard": [int(o0), int(o1)], "n_obj_total": int(w.n_obj), "n_obs_total": int(w.n_obs)})
     return make_config(cfg, dtype=dtype, point=rank)
 
 
@@ -250,7 +321,8 @@ def describe_workload(name: str, w) -> str:
         return (f"BASELINE.json configs[1]: single object, N_t={w.n_obs}, N_f={w.n_freq}, f in [{w.f_min},{w.f_max}) c/d, "
                 f"full periodogram")
     if name == "c3":
-        return (f"BASELINE.json configs[2]: {w.n_obj} objects, N_t in [50,500] (sum {w.n_obs}), N_f={w.n_freq}, "
+        n_obj, n_obs = w.meta.get("n_obj_total", w.n_obj), w.meta.get("n_obs_total", w.n_obs)
+        return (f"BASELINE.json configs[2]: {n_obj} objects, N_t in [50,500] (sum {n_obs}), N_f={w.n_freq}, "
                 f"best period only")
     return (f"BASELINE.json configs[3]: {w.n_obj} objects (sum N_t {w.n_obs}), N_f={w.n_freq}, full periodogram to "
             f"pinned host over copy streams")
@@ -350,12 +422,22 @@ def timed_loop(torch, dist, world, leg, step, steps: int, warmup: int, flush):
     return total_ms, info
 
 
+ARITHMETIC = {
+    ("tensor", False): "fp16 hi+lo split operands (22-bit), 3 tcgen05 products per MAC, fp32 accumulate in TMEM; phases two-float fp32",
+    ("tensor", True): "fp16 operands, 1 tcgen05 product per MAC, fp32 accumulate; MUFU sincos (fast_math)",
+    ("factored", False): "all-fp32 FFMA2 contraction (fp64: DFMA)", ("factored", True): "all-fp32 FFMA2 contraction, MUFU sincos",
+    ("direct", False): "one accurate sincos per pair", ("direct", True): "one MUFU sincos per pair",
+}
+
+
 def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_clocks: bool, kernel=None, fast=None,
-            with_e2e: bool = True):
-    w = workload_for(args.workload, dtype, rank)
+            with_e2e: bool = True, workload=None, steps=None):
+    name = args.workload if workload is None else workload
+    steps = args.steps if steps is None else steps
+    w = workload_for(name, dtype, rank, world)
     kernel = args.kernel if kernel is None else kernel
     fast = bool(args.fast_math if fast is None else fast) and dtype == "f32"
-    leg = Leg(pkg, torch, w, args.workload, dtype, fast, kernel, device)
+    leg = Leg(pkg, torch, w, name, dtype, fast, kernel, device)
     pairs_step = w.pairs
     pairs_all = pairs_step
     if world > 1:
@@ -365,27 +447,49 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     sampler = ClockSampler(device) if with_clocks else None
     if sampler:
         sampler.__enter__()
-    total_ms, info = timed_loop(torch, dist, world, leg, leg.step_device, args.steps, args.warmup, flush)
+    total_ms, info = timed_loop(torch, dist, world, leg, leg.step_device, steps, args.warmup, flush)
     dev_launches, kernel_ms = leg.launches, list(leg.kernel_ms)
     leg.launches, leg.kernel_ms = 0, []
-    ms_step = total_ms / args.steps
+    ms_step = total_ms / steps
     k_ms = sum(kernel_ms) / len(kernel_ms)
-    # measured pipe peak with the same clocks the kernels see (register-only FFMA2 / DFMA loops, lsp_pipe_peak)
-    pipe_ops, _ = pkg.lsp_pipe_peak(1 if dtype == "f32" else 2, device)
+    # measured pipe peak with the same clocks the kernels see (register-only FFMA2 / DFMA loops, bench_peak.cu)
+    pipe_ops = 0.0
+    if info["kernel"] == "factored":
+        pipe_ops, _ = pipe_peak(1 if dtype == "f32" else 2, device)
+    rf = roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, name)
+    es = 4 if dtype == "f32" else 8
+    in_bytes = w.n_obs * 2 * es + (w.n_obj + 1) * 8
+    out_bytes = w.n_obj * (2 * es + 8) if leg.best_only else w.n_obj * w.n_freq * es
+    rf["algorithmic_bytes"] = int(in_bytes + out_bytes)
+    if not leg.best_only and not leg.host_mode:
+        # achieved HBM write rate of the full-periodogram stores (north_star): N_o x N_f powers per launch of the
+        # kernel that writes them
+        rf["hbm_write_gbs"] = out_bytes / (k_ms * 1e-3) / 1e9
     out = {
         "dtype": dtype,
-        "value": pairs_all * args.steps / (total_ms * 1e-3),
+        "value": pairs_all * steps / (total_ms * 1e-3),
         "ms_per_step": ms_step,
-        "kernel": info["kernel"], "n_split": info["n_split"], "fast_math": fast,
+        "kernel": info["kernel"], "n_split": info["n_split"], "fast_math": fast, "tensor_shape": info.get("tensor_shape", 0),
         "kernel_ms_per_step": k_ms,
         "gpu_launches": dev_launches,
-        "roofline": roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, args.workload),
+        "roofline": rf,
+        "arithmetic": ARITHMETIC.get((info["kernel"], fast), ""),
     }
+    if world > 1 and name == "c3":
+        obs = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(world)]
+        dist.all_gather(obs, torch.tensor([int(w.n_obs)], dtype=torch.int64, device="cuda"))
+        out["rank_sum_nt"] = [int(x.item()) for x in obs]
+        # the best periods of the whole batch, gathered on every rank (outside the timed region: 24 bytes per object)
+        from paper_2105_04006_b200 import sharding
+        counts = [b - a for a, b in sharding.partition_objects(
+            __import__("workloads").make_config(3, dtype=dtype).offsets, world)]
+        allb = sharding.gather_objects(leg.d_best, counts)
+        out["gathered_best_periods"] = int(allb[0].numel())
     if with_e2e:
-        e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, args.steps, args.warmup, flush)
+        e2e_ms, _ = timed_loop(torch, dist, world, leg, leg.step_e2e, steps, args.warmup, flush)
         h2d, d2h = leg.e2e_bytes()
-        out["e2e"] = {"value": pairs_all * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                      "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / args.steps}
+        out["e2e"] = {"value": pairs_all * steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                      "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms / steps}
     if sampler:
         sampler.__exit__()
     if sampler:
@@ -394,7 +498,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     return out, w
 
 
-def c4_overlap(args, pkg, torch, device, flush):
+def c4_overlap(args, pkg, torch, device, flush, with_pageable: bool = True):
     """SURVEY.md 8(d) "C4 overlap": T_c = compute only (periodograms to a device buffer), T_d = D2H only of the resident
     N_o x N_f buffer with the library's chunking (chunk_bytes pieces round-robin over n_copy_streams streams into the
     pinned destination), T = the pipelined call.  hidden = (T_c + T_d - T) / min(T_c, T_d); "fully overlapped" means
@@ -447,22 +551,24 @@ def c4_overlap(args, pkg, torch, device, flush):
     plan.destroy()
     # pageable destination (Fig. 8): pinned staging ring + host-side copies on the copy
     # streams' callback threads, against plain cudaMemcpyAsync into the pageable buffer
-    h_page = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32)
-    h_page.fill_(0.0)                                  # touch the pages once, outside the timed region
+    h_page = None
+    if with_pageable:
+        h_page = torch.empty((w.n_obj, w.n_freq), dtype=torch.float32)
+        h_page.fill_(0.0)                              # touch the pages once, outside the timed region
     pageable = {}
-    for mode in ("staged", "plain"):
-        os.environ["LSP_PAGEABLE"] = mode
+    for mode in (("staged", "plain") if with_pageable else ()):
         pl = pkg.Plan(w.f_min, w.f_max, w.n_freq, "f32", kernel=args.kernel, device=device, n_copy_streams=n_streams,
-                      chunk_bytes=chunk_bytes)
+                      chunk_bytes=chunk_bytes, pageable_staged=(mode == "staged"))
         pageable[mode] = timeit(lambda: pl.periodogram_batched(d_off, d_t, d_y, host_out=h_page, h_offsets=h_off), reps=2)
         pl.destroy()
-    os.environ.pop("LSP_PAGEABLE", None)
     gb = w.n_obj * row / 1e9
-    return {"T_compute_ms": tc, "T_d2h_ms": td, "T_pipelined_ms": tp, "d2h_GBps": gb / (td * 1e-3),
-            "T_pageable_staged_ms": pageable["staged"], "T_pageable_plain_ms": pageable["plain"],
-            "hidden_fraction": (tc + td - tp) / min(tc, td), "T_over_max": tp / max(tc, td),
-            "fully_overlapped": bool(tp <= 1.05 * max(tc, td) + td / max(1, -(-w.n_obj // objs_per_chunk))),
-            "chunk_bytes": chunk_bytes, "n_copy_streams": n_streams, "bytes": w.n_obj * row}
+    out = {"T_compute_ms": tc, "T_d2h_ms": td, "T_pipelined_ms": tp, "d2h_GBps": gb / (td * 1e-3),
+           "hidden_fraction": (tc + td - tp) / min(tc, td), "T_over_max": tp / max(tc, td),
+           "fully_overlapped": bool(tp <= 1.05 * max(tc, td) + td / max(1, -(-w.n_obj // objs_per_chunk))),
+           "value": w.pairs / (tp * 1e-3), "chunk_bytes": chunk_bytes, "n_copy_streams": n_streams, "bytes": w.n_obj * row}
+    if with_pageable:
+        out["T_pageable_staged_ms"], out["T_pageable_plain_ms"] = pageable["staged"], pageable["plain"]
+    return out
 
 
 def run_c5(args, pkg, torch, device, flush):
@@ -472,7 +578,7 @@ def run_c5(args, pkg, torch, device, flush):
     dev = torch.device("cuda", device)
     rows = []
     for dtype in ("f32", "f64"):
-        pipe_ops, _ = pkg.lsp_pipe_peak(1 if dtype == "f32" else 2, device)
+        pipe_ops, _ = pipe_peak(1 if dtype == "f32" else 2, device)
         tdt = torch.float32 if dtype == "f32" else torch.float64
         for i, nt in enumerate(C5_NT):
             for j, nf in enumerate(C5_NF):
@@ -504,6 +610,11 @@ def run_c5(args, pkg, torch, device, flush):
                              "pairs_per_s": w.pairs * steps / (tot * 1e-3), "bound": rf["bound"], "roofline_frac": rf["frac"],
                              "frac_executed": rf.get("frac_executed")})
                 plan.destroy()
+    # FP64 / FP32 time ratio per point (the paper's Table 4 analogue)
+    f32 = {(r["n_t"], r["n_freq"]): r["ms_per_step"] for r in rows if r["dtype"] == "f32"}
+    for r in rows:
+        if r["dtype"] == "f64":
+            r["time_vs_f32"] = r["ms_per_step"] / f32[(r["n_t"], r["n_freq"])]
     return rows
 
 
@@ -574,31 +685,32 @@ def run_b200(args, rank: int, world: int, local_rank: int):
                               "sweep": rows}), flush=True)
         return
     primary, w = run_leg(args, pkg, torch, dist, rank, world, local_rank, args.dtype, flush, True)
-    other = None
+    solo = rank == 0 and world == 1
+    secondary = not args.no_secondary and args.workload == "c2" and args.kernel == "auto" and not args.fast_math
+    other = fma = c3 = c4 = None
     variants = {}
-    if not args.no_secondary and args.workload == "c2":
+    if secondary:
         other_dtype = "f64" if args.dtype == "f32" else "f32"
         other, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, other_dtype, flush, False)
-        if args.kernel == "auto" and not args.fast_math:
-            # the other FP32 formulations on the same workload (device-resident only): the FFMA2 contraction on the
-            # FMA pipe (north_star's "FP32 issue-bound roofline") and the fast_math tensor mode
-            variants["fp32_fma_pipe"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
-                                                   kernel="factored", fast=False, with_e2e=False)
-            variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
-                                                    kernel="auto", fast=True, with_e2e=False)
-            # the paper-shaped kernel (thread = frequency, one sincos per pair): __sincosf-class vs accurate sincos
-            # (PAPER.md:L423-433), the comparison north_star asks for
-            saved_steps = args.steps
-            args.steps = max(3, min(args.steps, 5))
-            variants["direct_fp32_sincosf"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
-                                                         kernel="direct", fast=True, with_e2e=False)
-            variants["direct_fp32_accurate"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
-                                                          kernel="direct", fast=False, with_e2e=False)
-            variants["direct_fp64"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f64", flush, False,
-                                                 kernel="direct", fast=False, with_e2e=False)
-            args.steps = saved_steps
+        # the all-FP32 FFMA2 contraction on the FMA pipe: north_star's "FP32 issue-bound roofline" is answered by this kernel
+        fma, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, kernel="factored", fast=False,
+                         with_e2e=False)
+        if solo:
+            # BASELINE.json configs[2] and configs[3], short: the driver's record then carries them too
+            c3, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, workload="c3",
+                            steps=max(3, min(args.steps, 10)))
+            c4 = c4_overlap(args, pkg, torch, local_rank, flush, with_pageable=False)
+    if args.variants and args.workload == "c2":
+        # fast_math tensor mode and the paper-shaped kernel (thread = frequency, one sincos per pair): __sincosf-class vs
+        # accurate sincos, the comparison north_star asks for
+        variants["fp32_fast_math"], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False,
+                                                kernel="auto", fast=True, with_e2e=False)
+        few = max(3, min(args.steps, 5))
+        for key, dt, fast in (("direct_fp32_sincosf", "f32", True), ("direct_fp32_accurate", "f32", False), ("direct_fp64", "f64", False)):
+            variants[key], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, dt, flush, False, kernel="direct",
+                                       fast=fast, with_e2e=False, steps=few)
     gls = None
-    if not args.no_secondary and args.workload in ("c2", "c3") and rank == 0 and world == 1:
+    if args.variants and args.workload in ("c2", "c3") and solo:
         gls = {}
         for dt in (("f32", "f64") if args.workload == "c2" else ("f32",)):
             g = run_generalized(args, pkg, torch, local_rank, flush, dt)
@@ -606,36 +718,66 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             g["time_vs_standard_same_dtype"] = (g["ms_per_step"] / std_ms) if std_ms else None
             gls[dt] = g
     overlap = None
-    if args.workload == "c4" and rank == 0 and world == 1:
+    if args.workload == "c4" and solo:
         overlap = c4_overlap(args, pkg, torch, local_rank, flush)
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if solo and not args.no_cpu_baseline:
         cpu = cpu_baseline(w, args.cpu_seconds)
     if rank == 0:
+        sharded = world > 1 and args.workload == "c3"
+        rf_keys = ("bound", "achieved", "peak", "unit", "frac", "traffic", "traffic_from", "algorithmic_bytes", "hbm_write_gbs",
+                   "kernel", "peak_is", "executed_flop_per_pair", "frac_executed", "frac_of_measured_pipe")
+
+        def short_rf(rf):
+            return {k: rf[k] for k in rf_keys if k in rf}
+
+        def short_leg(v, with_e2e=True):
+            o = {"value": v["value"], "ms_per_step": v["ms_per_step"], "kernel_ms_per_step": v["kernel_ms_per_step"],
+                 "kernel": v["kernel"], "gpu_launches": v["gpu_launches"], "roofline": short_rf(v["roofline"])}
+            if with_e2e and "e2e" in v:
+                o["e2e"] = v["e2e"]
+            return o
+
+        # the contract's keys first, so that a cut tail cannot lose them
         line = {
             "metric": METRIC, "value": primary["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": primary["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": primary["ms_per_step"], "higher_is_better": True,
+            "scaling": "strong" if sharded else "weak",
             "vs_baseline": None, "dtype": primary["dtype"], "data": "synthetic",
             "config": {"workload": describe_workload(args.workload, w), "kernel": primary["kernel"],
+                       "arithmetic": primary["arithmetic"],
                        "fast_math": bool(args.fast_math and args.dtype == "f32"), "n_split": primary["n_split"],
+                       "tensor_shape": primary["tensor_shape"],
                        "l2": "flushed between steps (256 MiB fill, outside the event pairs)",
-                       "parallelism": f"replicas x{world} (one object set per rank, no collective)"},
+                       "parallelism": (f"one batch sharded by object over {world} ranks (balanced by sum N_t), no collective"
+                                       if sharded else f"replicas x{world} (one object set per rank, no collective)")},
             "e2e": primary["e2e"], "gpu_launches": primary["gpu_launches"],
             "kernel_ms_per_step": primary["kernel_ms_per_step"],
-            "roofline": primary["roofline"], "clocks": primary.get("clocks"),
+            "roofline": short_rf(primary["roofline"]), "clocks": primary.get("clocks"),
         }
+        if "rank_sum_nt" in primary:
+            line["rank_sum_nt"] = primary["rank_sum_nt"]
         if other is not None:
-            line[other["dtype"] == "f64" and "fp64" or "fp32"] = {k: other[k] for k in
-                                                                 ("value", "ms_per_step", "kernel_ms_per_step", "e2e", "roofline",
-                                                                  "gpu_launches", "kernel")}
-        for name, v in variants.items():
-            line[name] = {k: v[k] for k in ("value", "ms_per_step", "kernel_ms_per_step", "roofline", "gpu_launches", "kernel")}
-        if gls:
-            line["generalized"] = gls
+            line["fp64" if other["dtype"] == "f64" else "fp32"] = short_leg(other)
+        if fma is not None:
+            line["fp32_fma_pipe"] = {"value": fma["value"], "ms_per_step": fma["ms_per_step"], "frac": fma["roofline"]["frac"],
+                                     "achieved": fma["roofline"]["achieved"], "peak": fma["roofline"]["peak"], "unit": "TFLOP/s",
+                                     "bound": "alu", "kernel": fma["roofline"]["kernel"]}
+        if c3 is not None:
+            line["c3"] = {"value": c3["value"], "ms_per_step": c3["ms_per_step"], "kernel_ms_per_step": c3["kernel_ms_per_step"],
+                          "frac": c3["roofline"]["frac"], "frac_executed": c3["roofline"].get("frac_executed"),
+                          "e2e": c3["e2e"]["value"], "fast_math": c3["fast_math"]}
+        if c4 is not None:
+            line["c4"] = {k: c4[k] for k in ("value", "T_compute_ms", "T_d2h_ms", "T_pipelined_ms", "T_over_max", "d2h_GBps",
+                                             "fully_overlapped")}
         if overlap is not None:
             line["d2h_overlap"] = overlap
         if cpu is not None:
             line["cpu_baseline"] = cpu
+        for name, v in variants.items():
+            line[name] = short_leg(v, with_e2e=False)
+        if gls:
+            line["generalized"] = gls
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.barrier()

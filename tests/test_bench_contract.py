@@ -30,3 +30,22 @@ def test_nonzero_rank_of_reference_arm_exits_quietly():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
                           "--warmup", "0"], capture_output=True, text=True, timeout=120, cwd=ROOT, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_pipe_peak_helper_builds_outside_the_library():
+    """The pipe-peak microbenchmarks are a bench-only helper (bench_peak.cu -> libbench_peak.so), not part of liblsp_b200.so."""
+    import ctypes
+    sys.path.insert(0, ROOT)
+    import bench
+    lib = ctypes.CDLL(bench.build_peak_lib())
+    assert hasattr(lib, "bench_pipe_peak")
+    import paper_2105_04006_b200 as pkg
+    assert not hasattr(pkg.load_library(), "lsp_pipe_peak") and not hasattr(pkg.load_library(), "bench_pipe_peak")
+
+
+def test_roofline_traffic_is_read_from_a_committed_capture():
+    sys.path.insert(0, ROOT)
+    import bench
+    b, src = bench.ncu_traffic("c2", "tensor", "f32")
+    assert src is not None and os.path.exists(os.path.join(ROOT, src)) and b > 1e6
+    assert bench.ncu_traffic("c4", "tensor", "f32") == (None, None)
