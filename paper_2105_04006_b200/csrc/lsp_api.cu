@@ -58,7 +58,7 @@ struct lsp_plan {
     DeviceBuffer tc_objs;         // TensorObj[n_obj_launch]   (tensor path pre-pass)
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
-    int tc_stages_b = 3;          // B-operand ring depth of the tensor kernel
+    int tc_stages_b = 0;          // B-operand ring depth of the tensor kernel; 0 = as many as fit (cfg.tensor_b_stages)
     int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
@@ -167,10 +167,8 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
         s.tp.nl = (int)nl;
         s.tp.tile = (int)(kTcGroups * 2 * nl);
         s.tp.n_ops = c.fast_math ? 2 : 4;
-        s.tp.a_stage_bytes = s.tp.n_ops * 128 * kTcKB * 2;
-        s.tp.b_stage_bytes = s.tp.n_ops * 2 * (int)nl * kTcKB * 2;
-        // B ring: 3 stages (LSP_TC_SB overrides); A ring: whatever else fits, at most 8 (sized after the split is known)
-        s.tp.stages_b = p->tc_stages_b;
+        s.tp.b_plane_bytes = 2 * (int)nl * kTcKB * 2;
+        s.tp.b_stage_bytes = s.tp.n_ops * s.tp.b_plane_bytes + kTcAuxBytes;
         s.tile = s.tp.tile;
         s.direct_r = 0;
         slots = p->sm_count;
@@ -203,14 +201,24 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
             if (waves >= 8.0) break;
         }
     }
+    if (k == LSP_KERNEL_TENSOR && n_obj > 0) {
+        // The tensor cores add into their FP32 accumulators with truncation: the bias grows with the number of accumulations
+        // (measured ~3e-8 of the sum per 16-observation stage).  Items are capped at 1024 stages so it stays below 1e-4 of max P.
+        const int64_t nkb_avg = (total_obs / n_obj + kTcKB - 1) / kTcKB;
+        split = std::max<int64_t>(split, (nkb_avg + 1023) / 1024);
+    }
     s.n_split = (int)split;
     if (k == LSP_KERNEL_TENSOR) {
         // role shape by item length: stages (16 observations) per work item
         const int64_t avg_nt = n_obj > 0 ? total_obs / n_obj : 0;
         const int64_t stages_per_item = (avg_nt / kTcKB) / std::max<int64_t>(1, split);
         s.tp.long_items = (p->tc_roles == 0) ? (stages_per_item >= 48 ? 1 : 0) : (p->tc_roles == 2 ? 1 : 0);
-        const int reserve = (s.tp.long_items ? tc_static_smem<3>() : tc_static_smem<2>()) + 2048;
-        s.tp.stages = (int)std::max<int64_t>(3, std::min<int64_t>(8, ((int64_t)(p->smem_optin - reserve) - (int64_t)s.tp.stages_b * s.tp.b_stage_bytes) / s.tp.a_stage_bytes));
+        // B ring (TMA -> MMA; the generators read its aux blocks): as deep as shared memory allows, at most 8 stages
+        const int reserve = (s.tp.long_items ? tc_static_smem<4, 4>() : tc_static_smem<8, 3>()) + (int)tc_smem_bytes(0, 0) + 512;
+        const int fit = (int)std::max<int64_t>(2, std::min<int64_t>(8, (int64_t)(p->smem_optin - reserve) / s.tp.b_stage_bytes));
+        const int need = tc_min_stages_b(c.fast_math != 0, s.tp.long_items ? 4 : 3);       // always <= fit for NL <= 112
+        s.tp.stages_b = std::max(need, p->tc_stages_b > 0 ? std::min(p->tc_stages_b, fit) : fit);
+        s.tp.fixup = split > 1 ? 1 : 0;
     }
     return s;
 }
@@ -226,19 +234,23 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (s.kernel == LSP_KERNEL_TENSOR) {
         if constexpr (std::is_same<T, float>::value) {
-            const size_t smem = tc_smem_bytes(s.tp.stages, s.tp.stages_b, s.tp.a_stage_bytes, s.tp.b_stage_bytes);
+            const size_t smem = tc_smem_bytes(s.tp.stages_b, s.tp.b_stage_bytes);
             const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
             auto go = [&](auto kern, int threads) -> cudaError_t {
                 const cudaError_t ea = optin_smem(p, kern, smem);
                 if (ea != cudaSuccess) return ea;
-                kern<<<ctas, threads, smem, st>>>(gp, s.tp, d_off, (const float*)d_t, (const float*)d_y,
-                                                  (const TensorObj*)p->tc_objs.ptr, (const __half*)p->tc_table.ptr, (float*)out,
-                                                  partials, (float4*)sums, n_obj_launch, (long long)grid);
+                kern<<<ctas, threads, smem, st>>>(gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr, (const unsigned char*)p->tc_table.ptr,
+                                                  (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid);
                 return cudaSuccess;
             };
             p->tensor_shape = s.tp.long_items ? 2 : 1;
-            cudaError_t e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 3>, TcRoles<4, 3>::kThreads)
-                                            : go(lsp_tensor_kernel<float, FAST, 8, 2>, TcRoles<8, 2>::kThreads);
+            cudaError_t e;
+            if (s.tp.weighted)           // generalised mode: the W slot carries the weights
+                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, true>, TcRoles<4, 4>::kThreads)
+                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, true>, TcRoles<8, 3>::kThreads);
+            else
+                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, false>, TcRoles<4, 4>::kThreads)
+                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, false>, TcRoles<8, 3>::kThreads);
             if (e != cudaSuccess) return e;
         } else {
             return cudaErrorInvalidValue;      // rejected at plan creation
@@ -269,15 +281,27 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 }
 
 // Launches steps 2-6' for objects [obj_base, obj_base + n_obj_launch) on `st`.
-// `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed globally.
-lsp_status run_range(lsp_plan* p, const Schedule& s, const GridSpec& g, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
+// `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed by the launch-local object.
+struct RangeOpts {
+    void* ext_sums = nullptr;     // write partial sums there and stop (generalised mode)
+    const void* wgt = nullptr;    // generalised mode: per-observation weights carried by the W slot (sum w e^{2 i theta})
+    int z_only = 0;               // generalised mode: only the Z slot is wanted (tensor path skips the W contraction)
+};
+lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
                      const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
-                     cudaStream_t st, void* ext_sums = nullptr)      // ext_sums: write partial sums there and stop (generalised mode)
+                     cudaStream_t st, const RangeOpts& opt = RangeOpts{})
 {
     const lsp_config& c = p->cfg;
-    if (s.kernel == LSP_KERNEL_TENSOR) {
-        // pre-pass of the tensor path: per-object statistics, table offsets, then the B-operand table (once per object,
-        // shared by all of its frequency tiles and observation splits)
+    Schedule s = s_in;
+    void* ext_sums = opt.ext_sums;
+    const bool tensor = s.kernel == LSP_KERNEL_TENSOR;
+    const bool fixup = tensor && s.n_split > 1 && !ext_sums;      // the tensor kernel finishes split tiles itself
+    if (tensor) {
+        s.tp.fixup = fixup ? 1 : 0;
+        s.tp.weighted = opt.wgt ? 1 : 0;
+        s.tp.z_only = opt.z_only;
+        // pre-pass of the tensor path, ONE launch: the B-operand table (once per object, shared by all of its frequency tiles
+        // and observation splits; each stage carries the aux block the generators read) and the per-object statistics
         const int64_t kb_bound = obs_bound / kTcKB + n_obj_launch;
         lsp_status e = ensure(p, p->tc_objs, (size_t)(n_obj_launch + 1) * sizeof(TensorObj));
         if (e != LSP_OK) return e;
@@ -287,20 +311,18 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, const GridSpec& g, int64_t 
         gq.df = (g.f_max - g.f_min) / (double)c.n_freq;
         gq.n_freq = (int)c.n_freq;
         gq.obj_base = (int)obj_base;
-        const int stats_threads = n_obj_launch < 64 ? 1024 : 128;     // a lone long object gets a full CTA
-        lsp_tensor_stats_kernel<float><<<(unsigned)n_obj_launch, stats_threads, 0, st>>>(d_off, (const float*)d_y, (TensorObj*)p->tc_objs.ptr,
-                                                                            (int)obj_base, g.center, g.normalize);
-        lsp_tensor_scan_kernel<<<1, 1024, 0, st>>>(d_off, (TensorObj*)p->tc_objs.ptr, (int)obj_base, (int)n_obj_launch);
-        if (kb_bound > 0) {
-            if (c.fast_math)
-                lsp_tensor_table_kernel<float, true><<<(unsigned)kb_bound, kTcMaxNL, 0, st>>>(gq, s.tp, d_off, (const float*)d_t,
-                                                                                          (const TensorObj*)p->tc_objs.ptr, (int)n_obj_launch, (__half*)p->tc_table.ptr);
-            else
-                lsp_tensor_table_kernel<float, false><<<(unsigned)kb_bound, kTcMaxNL, 0, st>>>(gq, s.tp, d_off, (const float*)d_t,
-                                                                                           (const TensorObj*)p->tc_objs.ptr, (int)n_obj_launch, (__half*)p->tc_table.ptr);
-        }
+        const int64_t pre_grid = kb_bound + n_obj_launch;
+        if (pre_grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
+        if (c.fast_math)
+            lsp_tensor_prepass_kernel<true><<<(unsigned)pre_grid, kTcPreThreads, 0, st>>>(
+                gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
+                (int)n_obj_launch, (long long)kb_bound, g.center, g.normalize, (unsigned char*)p->tc_table.ptr);
+        else
+            lsp_tensor_prepass_kernel<false><<<(unsigned)pre_grid, kTcPreThreads, 0, st>>>(
+                gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
+                (int)n_obj_launch, (long long)kb_bound, g.center, g.normalize, (unsigned char*)p->tc_table.ptr);
         LSP_CUDA(p, cudaGetLastError());
-        p->n_launches += 3;
+        ++p->n_launches;
     }
     GridParams gp;
     gp.f_min = g.f_min;
@@ -314,13 +336,21 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, const GridSpec& g, int64_t 
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
     if (ext_sums) {
         sums = ext_sums;
+    } else if (fixup) {
+        // tensor path: one slot per (split, object, tile) in the epilogue's own element order (lsp_tensor.cuh)
+        const size_t tile_elems = (size_t)((s.tp.nl + 15) / 16) * 16 * 128;
+        const size_t need = (size_t)s.n_split * n_obj_launch * s.n_tiles * tile_elems * sizeof(float4);
+        lsp_status e = ensure(p, p->sums, need);
+        if (e != LSP_OK) return e;
+        sums = p->sums.ptr;
     } else if (s.n_split > 1) {
         const size_t need = (size_t)s.n_split * n_obj_launch * c.n_freq * 4 * elem_size(c);
         lsp_status e = ensure(p, p->sums, need);
         if (e != LSP_OK) return e;
         sums = p->sums.ptr;
     }
-    *n_parts_out = (s.n_split > 1 || ext_sums) ? n_cparts : s.n_tiles;
+    const bool combine = s.n_split > 1 && !ext_sums && !fixup;    // FMA-pipe / direct kernels: partial sums + lsp_combine_kernel
+    *n_parts_out = (combine || ext_sums) ? n_cparts : (fixup ? s.n_tiles * kTcFixParts : s.n_tiles);
     if (want_best) {     // partials are indexed by the launch-local object: each launch's finalize follows it in-stream
         lsp_status e = ensure(p, p->partials, (size_t)n_obj_launch * (size_t)*n_parts_out * sizeof(Best));
         if (e != LSP_OK) return e;
@@ -355,7 +385,16 @@ lsp_status run_range(lsp_plan* p, const Schedule& s, const GridSpec& g, int64_t 
     ++p->n_launches;
     if (ev1) LSP_CUDA(p, cudaEventRecord(ev1, st));
 
-    if (s.n_split > 1 && !ext_sums) {
+    if (fixup) {
+        // tensor path: add the splits' partial slots in split order and finish the tiles (steps 5, 6, 6')
+        const int64_t grid = n_obj_launch * (int64_t)s.n_tiles * kTcFixParts;
+        if (grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
+        lsp_tensor_fix_kernel<float><<<(unsigned)grid, kTcFixThreads, 0, st>>>(gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
+                                                                              (const float4*)sums, (float*)out, partials, n_obj_launch);
+        LSP_CUDA(p, cudaGetLastError());
+        ++p->n_launches;
+    }
+    if (combine) {
         const int64_t grid = n_obj_launch * n_cparts;
         if (c.dtype == LSP_F32)
             lsp_combine_kernel<float><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, d_off, stats, (const float4*)sums, (float*)out,
@@ -790,8 +829,9 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
             const double fs = pass == 2 ? 2.0 : 1.0;
             const GridSpec g{c.f_min * fs, c.f_max * fs, 0, 0};
             if ((e = build_ws_table(p, s, g, d_t, total_obs, st)) != LSP_OK) return e;
-            e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st,
-                          (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes);
+            RangeOpts ro;
+            ro.ext_sums = (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes;
+            e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st, ro);
             if (e != LSP_OK) return e;
         }
         GridParams gp;
@@ -959,7 +999,7 @@ float lsp_last_kernel_ms(lsp_plan* p)
 
 const char* lsp_version(void)
 {
-    return "lsp-b200 0.3 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05; modes: standard, generalised)";
+    return "lsp-b200 0.4 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05 (A operands in TMEM); modes: standard, generalised)";
 }
 
 }  // extern "C"

@@ -1,36 +1,43 @@
 // lsp_tensor.cuh -- the FP32-mode periodogram contraction on the 5th-generation tensor cores (tcgen05 + TMEM).
 //
 // The factored formulation (lsp_factored.cuh: theta_kj = alpha_gj +/- beta_mj, a = y e^{i alpha}, b = e^{i beta})
-// makes steps 4 of the hot path a dense real contraction over the observations j of one object:
+// makes step 4 of the hot path a dense real contraction over the observations j of one object:
 //
 //     D_Z[128 x 2NL] = A_Z[128 x N_t] * B_Z[N_t x 2NL]        A_Z rows: Re a_g / Im a_g of 64 frequency groups
 //     D_W[128 x 2NL] = A_W[128 x N_t] * B_W[N_t x 2NL]        B_Z cols: Re b_m (m < NL) | Im b_m;  W: doubled angles
 //
 // D holds, per (group g, offset m), Srr, Sri (row "Re a_g") and Sir, Sii (row "Im a_g"), from which
 //     Z(c_g + m + 1/2) = (Srr - Sii) + i (Sri + Sir),   Z(c_g - m - 1/2) = (Srr + Sii) + i (Sir - Sri)
-// and the same for W: one 128 x 2NL tile pair covers 64 * 2NL <= 16384 grid frequencies of one object, and the four
+// and the same for W: one 128 x 2NL tile pair covers 64 * 2NL <= 14336 grid frequencies of one object, and the four
 // real sums of Eq. 2's closed form (lsp_common.cuh) for every one of them.  This is a GEMM, so it runs as one:
-// tcgen05.mma kind::f16 (M = 128, N = 2NL <= 256, K = 16), FP32 accumulators in TMEM (Z in columns [0,256),
-// W in [256,512): the whole 256 KB), operands in shared memory in the no-swizzle K-major core-matrix layout.
+// tcgen05.mma kind::f16, M = 128, N = 2NL <= 224, K = 16, FP32 accumulators in TMEM.
+//
+// Where the operands live (round 2: the shared-memory pipe was the ceiling of the SS-mode kernel -- 12 KB of operand reads
+// per 128-cycle MMA plus the generators' operand stores plus the TMA fills):
+//   A operands (tile dependent, generated on the fly) are written by the generator warps STRAIGHT INTO TENSOR MEMORY
+//               (tcgen05.st) and the MMAs read them from there (A-from-TMEM form of tcgen05.mma): no shared-memory store,
+//               no shared-memory read, no proxy fence.  TMEM columns: Z accumulators [0, 2NL), W accumulators
+//               [224, 224 + 2NL), A ring [448, 512) = 2 stages x 4 planes x 8 columns (fast_math: 4 stages x 2 planes).
+//   B operands  e^{i beta}, e^{2 i beta} depend on (object, observation, m) only -- not on the tile -- so one pre-pass launch
+//               (lsp_tensor_prepass_kernel) writes them once per object into a table already laid out as shared-memory
+//               stages; warp 0 streams the stages in with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx).
+//               Each table stage also carries an "aux" block (t_j, y_j, w_j and the tile-independent phasors v of its 16
+//               observations), so the generators never touch global memory.
 //
 // Precision: operands are FP16 pairs x = x_hi + x_lo (22 significand bits, the same class as
-// FP32's 24) and the product is a_hi b_hi + a_hi b_lo + a_lo b_hi (three MMAs; a_lo b_lo < 2^-24 is dropped), with y
+// FP32's 24) and the product is a_hi b_hi + a_hi b_lo + a_lo b_hi (three MMAs; a_lo b_lo < 2^-22 is dropped), with y
 // pre-scaled by a power of two per object so FP16 never overflows or loses the low part.  fast_math = 1 keeps only
 // a_hi b_hi (one MMA, ~2^-11 per operand) and evaluates sincos with MUFU: the "fast vs accurate" comparison of
-// PAPER.md:L423-433 carried over to this formulation.  Phases are formed in FP64 and range-reduced before any FP32
-// trigonometry, as everywhere in the library.
+// PAPER.md:L423-433 carried over to this formulation.  Phases are range-reduced before any FP32 trigonometry.
 //
-// Data flow per CTA (persistent, one per SM, static round-robin over (object, tile, split) work items):
-//   B operands  e^{i beta}, e^{2 i beta} depend on (object, observation, m) only -- not on the tile -- so a pre-pass
-//               (lsp_tensor_table_kernel) writes them once per object into a table already laid out as shared-memory
-//               stages; warp 0 streams the stages in with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx).
-//   A operands  depend on the tile: warps 12-19 generate them straight into the stage ring (st.shared +
-//               fence.proxy.async): one sincos per thread per stage (two-float FP32 phase), then the 64 x 16 operands as
-//               phasor products e^{i alpha_g} = u_{g mod 8} v_{g div 8} on the FMA pipe, scaled by y, split into FP16 hi/lo.
-//   warp 1      one thread issues the MMAs of a stage when its mbarrier completes, and tcgen05.commit releases the
-//               stage / publishes the finished accumulators.
-//   warps 4-11  epilogue: tcgen05.ld the accumulators, combine rows with a shuffle, closed-form power (step 5),
-//               vector stores of the periodogram (step 6) or the fused argmax partial (step 6').
+// Roles of one CTA (persistent, one per SM, static round-robin over (object, tile, split) work items):
+//   warp 0      TMA producer of the B ring          warp 1   MMA issuer (one elected lane)        warp 2   TMEM allocator
+//   warps 4..   epilogue: tcgen05.ld the accumulators, pair rows with a shuffle, closed-form power (step 5), vector
+//               stores of the periodogram (step 6) or the fused argmax partial (step 6'); for split-N_t items the
+//               partial sums go to global memory in the epilogue's own order (coalesced) and lsp_tensor_fix_kernel adds
+//               them in split order and finishes the tiles
+//   then NG generator groups of 4 warps, each taking every NG-th stage: one sincos per thread (the tile's phasors u),
+//               then row r = (group g, Re/Im) of the stage's A operand for its 16 observations in registers -> TMEM.
 #pragma once
 #include <cuda_fp16.h>
 
@@ -42,135 +49,71 @@ namespace lsp {
 
 constexpr int kTcGroups = 64;                  // frequency groups per tile (128 MMA rows)
 constexpr int kTcKB = 16;                      // observations per MMA / ring stage (kind::f16: K = 16)
-constexpr int kTcMaxNL = 128;                  // N = 2 NL <= 256
-// Generator scratch (floats): three planes (cos, sin, -sin) of [observation quad j/4][phasor q][j%4]; a quad row is 16 x 4
-// floats + 16 floats of padding so that the two quads a quarter-warp reads fall into different banks (conflict-free LDS.128).
-constexpr int kTcScratchQuad = 16 * 4 + 16;
-constexpr int kTcScratchPlane = 4 * kTcScratchQuad;
-constexpr int kTcGenGroupThreads = 256;                               // threads that build one ring stage
-// Warp roles of one CTA: 4 control warps, EW epilogue warps, NG generator groups of 8 warps.  Two shapes are built:
-//   (EW, NG) = (8, 2): 896 threads -- short items (batches of short light curves): the per-item epilogue is on the critical path
-//   (EW, NG) = (4, 3): 1024 threads -- long items (hundreds of stages): the generators are, the epilogue is rare
-// Registers are re-split with setmaxnreg (per 4-warp group): control 40, generators 56, epilogue what is left
-// (120 resp. 136): 128 x 40 + 256 x 120 + 512 x 56 = 64512 = 896 x 72;  128 x 40 + 128 x 136 + 768 x 56 = 65536 = 1024 x 64.
-template <int EW, int NG> struct TcRoles {
-    static constexpr int kThreads = (4 + EW + 8 * NG) * 32;
-    static constexpr int kEpiThreads = EW * 32;
-    static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8;
-    static constexpr int kCtrlRegs = 40, kGenRegs = 56;
-    static constexpr int kEpiRegs = ((kLaunchRegs * kThreads - 128 * kCtrlRegs - 8 * NG * 32 * kGenRegs) / kEpiThreads) / 8 * 8;
-    static_assert(EW % 4 == 0 && kThreads <= 1024 && kEpiRegs >= 96 && kEpiRegs <= 255, "role split");
-};
-// static shared memory of the kernel (generator scratch etc.) + alignment slack, for the host's ring sizing
-template <int NG> constexpr int tc_static_smem() { return NG * 2 * (3 * kTcScratchPlane + kTcKB) * 4 + 1024; }
+#ifndef LSP_TC_MAX_NL
+#define LSP_TC_MAX_NL 112
+#endif
+constexpr int kTcMaxNL = LSP_TC_MAX_NL;        // N = 2 NL <= 224: leaves 64 TMEM columns for the A ring (104: 96 columns)
+constexpr int kTcWCol = 2 * kTcMaxNL;          // first TMEM column of the W accumulators
+constexpr int kTcACol = 4 * kTcMaxNL;          // first TMEM column of the A-operand ring
+constexpr int kTcACols = 512 - kTcACol;        // its width
+constexpr int kTcPreThreads = 128;             // threads of a pre-pass block
+// aux block of a table stage (floats): t[16], y[16], w[16], then 16 phasor rows of 16 complex values (+ 4 floats of padding
+// per row: 144-byte rows keep the LDS.128 of lanes that read different rows conflict-free).  Rows 0-7: v_g1 = e^{2 pi i (8 g1 L df) t_j};
+// rows 8-15: v_g1 e^{-i pi/4}, the version the "Im a" rows use (see the generators).  Inside a row the 16 phasors are stored
+// per observation PAIR as (cos_2h, cos_2h+1, sin_2h, sin_2h+1): one LDS.128 yields two register-aligned float2 operands
+// of the packed FP32x2 instructions.
+constexpr int kTcVRow = 36;
+constexpr int kTcAuxFloats = 48 + 16 * kTcVRow;
+constexpr int kTcAuxBytes = kTcAuxFloats * 4;  // 2496
 constexpr float kTcUnitScale = 256.0f;         // scale of the unit-modulus A_W operands (keeps the FP16 low part normal)
+constexpr float kTcPhasorScale = 16.0f;        // sqrt of it: carried by the phasors u
+
+// Warp roles of one CTA: 4 control warps, EW epilogue warps, NG generator groups of 4 warps.  Two shapes are built:
+//   (EW, NG) = (8, 3): short items (batches of short light curves): the per-item epilogue is on the critical path
+//   (EW, NG) = (4, 4): long items (hundreds of stages): the generators are, the epilogue is rare
+// Both have 768 threads (80 registers at launch).  Registers are re-split with setmaxnreg: control 40, generators 72,
+// epilogue what is left (112 resp. 152).
+template <int EW, int NG> struct TcRoles {
+    static constexpr int kThreads = (4 + EW + 4 * NG) * 32;
+    static constexpr int kEpiThreads = EW * 32;
+    static constexpr int kGenGroupThreads = 128;
+    static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8;
+    static constexpr int kCtrlRegs = 40, kGenRegs = 72;
+    static constexpr int kEpiRegs = ((kLaunchRegs * kThreads - 128 * kCtrlRegs - 4 * NG * 32 * kGenRegs) / kEpiThreads) / 8 * 8;
+    static_assert(EW % 4 == 0 && kThreads <= 1024 && kGenRegs <= kLaunchRegs && kEpiRegs >= 96 && kEpiRegs <= 255, "role split");
+};
 
 struct TensorParams {
-    int nl;             // NL: half-width of a frequency group (multiple of 8, <= 128); group width L = 2 NL = MMA N
+    int nl;             // NL: half-width of a frequency group (multiple of 8, <= 112); group width L = 2 NL = MMA N
     int tile;           // frequencies per tile = 64 * 2 NL
     int n_ops;          // FP16 operand planes per stage side: 4 (accurate: hi and lo of Z- and W-operands) or 2 (fast)
-    int stages;         // A-operand ring depth (generators -> MMA)
-    int stages_b;       // B-operand ring depth (TMA -> MMA): shallower, the copies are fast and B stages are twice as large
-    int long_items;     // 1: many stages per item -> the (4 epilogue warps, 3 generator groups) shape; 0: (8, 2)
-    int b_stage_bytes;  // n_ops * 2 NL * 32
-    int a_stage_bytes;  // n_ops * 128 * 32
+    int stages_b;       // B-operand ring depth (TMA -> MMA)
+    int long_items;     // 1: many stages per item -> the (4 epilogue warps, 4 generator groups) shape; 0: (8, 3)
+    int b_plane_bytes;  // 2 NL * 32
+    int b_stage_bytes;  // n_ops * b_plane_bytes + kTcAuxBytes
+    int fixup;          // n_split > 1: 1 = partial slots in the epilogue's own order, finished by lsp_tensor_fix_kernel;
+                        // 0 = partial sums per grid frequency (generalised mode)
+    int weighted;       // generalised mode: the W operand carries the weights w_j (aux.w) instead of 1
+    int z_only;         // generalised mode, second pass: only the Z contraction is wanted
 };
 
 // Per-object pre-pass results of the tensor path.
 struct TensorObj {
     double  mean;       // subtracted from y (0 unless center = 1)
     float   yscale;     // power of two: max |y - mean| * yscale in [256, 512)
-    float   pscale;     // output scale: (normalize ? 2 / sum (y-mean)^2 : 1) * 256 / yscale^2
-    float   zinv;       // 1 / yscale (split-N_t path: sums are written un-scaled)
-    int     pad;
-    int64_t kb_off;     // first table block of this object
+    float   pscale;     // output scale: nrm * 256 / yscale^2
+    float   zinv;       // 1 / yscale (partial sums are written un-scaled)
+    float   nrm;        // normalize ? 2 / sum (y-mean)^2 : 1
+    float   wscale;     // weighted mode: power of two, max w * wscale in [256, 512); else 256
+    float   winv;       // 1 / wscale
 };
 
 __host__ __device__ inline int tc_n_kb(int64_t n_t) { return (int)((n_t + kTcKB - 1) / kTcKB); }
-
-// ---- pre-pass 1: per-object statistics (one CTA per object) -----------------------------------------------------
-template <typename T>
-__global__ void lsp_tensor_stats_kernel(const int64_t* __restrict__ offsets, const T* __restrict__ y, TensorObj* __restrict__ objs,
-                                        int obj_base, int center, int normalize)
+// First table block of launch-local object o: floor(offset / 16) + o.  It needs no scan over the objects and leaves every
+// object at least ceil(N_t / 16) blocks (the table is sized total_obs / 16 + n_obj blocks; a few blocks stay unused).
+__device__ __forceinline__ int64_t tc_kb_off(const int64_t* __restrict__ offsets, int64_t obj_base, int64_t o)
 {
-    __shared__ double red[3][32];
-    const int64_t obj = (int64_t)blockIdx.x + obj_base;
-    const int64_t lo = offsets[obj], n = offsets[obj + 1] - lo;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    double s = 0.0;
-    if (center) {
-        for (int64_t j = threadIdx.x; j < n; j += blockDim.x) s += (double)y[lo + j];
-        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
-        if (lane == 0) red[0][wid] = s;
-        __syncthreads();
-        s = 0.0;
-        for (int w = 0; w < nw; ++w) s += red[0][w];
-        __syncthreads();
-    }
-    const double mean = (center && n > 0) ? s / (double)n : 0.0;
-    double q = 0.0, mx = 0.0;
-    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
-        const double v = (double)y[lo + j] - mean;
-        q += v * v;
-        mx = fmax(mx, fabs(v));
-    }
-    for (int d = 16; d > 0; d >>= 1) {
-        q += __shfl_xor_sync(0xffffffffu, q, d);
-        mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
-    }
-    if (lane == 0) { red[1][wid] = q; red[2][wid] = mx; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        q = 0.0; mx = 0.0;
-        for (int w = 0; w < nw; ++w) { q += red[1][w]; mx = fmax(mx, red[2][w]); }
-        TensorObj* o = &objs[blockIdx.x];     // kb_off is written by the scan kernel
-        o->mean = mean;
-        int e = 0;
-        if (mx > 0.0 && isfinite(mx)) frexp(mx, &e);          // mx = f * 2^e, f in [0.5, 1)  ->  mx * 2^(9-e) in [256, 512)
-        e = max(-100, min(100, 9 - e));
-        const double ys = (mx > 0.0 && isfinite(mx)) ? ldexp(1.0, e) : 1.0;
-        o->yscale = (float)ys;
-        o->zinv = (float)(1.0 / ys);
-        const double nrm = normalize ? (q > 0.0 ? 2.0 / q : 0.0) : 1.0;
-        o->pscale = (float)(nrm * (double)kTcUnitScale / (ys * ys));
-        o->pad = 0;
-    }
-}
-
-// ---- pre-pass 2: exclusive scan of ceil(N_t / 16) over the launch's objects (single CTA) -----------------------
-__global__ void lsp_tensor_scan_kernel(const int64_t* __restrict__ offsets, TensorObj* __restrict__ objs, int obj_base, int n_obj)
-{
-    __shared__ int64_t wsum[32];
-    const int tid = threadIdx.x, nt = blockDim.x, lane = tid & 31, wid = tid >> 5;
-    const int per = (n_obj + nt - 1) / nt;
-    const int o0 = min(n_obj, tid * per), o1 = min(n_obj, o0 + per);
-    int64_t s = 0;
-    for (int o = o0; o < o1; ++o) s += tc_n_kb(offsets[obj_base + o + 1] - offsets[obj_base + o]);
-    // block-wide exclusive scan of the per-thread totals: warp shuffles, then the warp totals
-    int64_t inc = s;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const int64_t v = __shfl_up_sync(0xffffffffu, inc, d);
-        if (lane >= d) inc += v;
-    }
-    if (lane == 31) wsum[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-        int64_t w = (lane < (nt >> 5)) ? wsum[lane] : 0, winc = w;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int64_t v = __shfl_up_sync(0xffffffffu, winc, d);
-            if (lane >= d) winc += v;
-        }
-        wsum[lane] = winc - w;                     // exclusive offset of each warp
-        if (lane == 31) objs[n_obj].kb_off = winc; // total number of table blocks
-    }
-    __syncthreads();
-    int64_t run = wsum[wid] + inc - s;              // exclusive prefix of this thread's first object
-    for (int o = o0; o < o1; ++o) {
-        objs[o].kb_off = run;
-        run += tc_n_kb(offsets[obj_base + o + 1] - offsets[obj_base + o]);
-    }
+    return (offsets[obj_base + o] - offsets[obj_base]) / kTcKB + o;
 }
 
 __device__ __forceinline__ void split_half2(float x0, float x1, __half2* hi, __half2* lo)
@@ -181,35 +124,114 @@ __device__ __forceinline__ void split_half2(float x0, float x1, __half2* hi, __h
     *lo = __floats2half2_rn(x0 - b.x, x1 - b.y);
 }
 
-// ---- pre-pass 3: the B-operand table ---------------------------------------------------------------------------------
-// One CTA per (object, 16-observation block); thread m < NL owns offset m.  Block layout (FP16), identical to one
-// shared-memory B stage:  [plane: b_hi, b2_hi, (b_lo, b2_lo)] [k chunk c = 0,1] [column group n/8] [n%8] [k%8]
-// with column n = m (Re) or NL + m (Im) and observation 16 kb + 8 c + k%8.  Observations past N_t are zero.
-template <typename T, bool FAST>
-__global__ void __launch_bounds__(kTcMaxNL)
-lsp_tensor_table_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
-                        const TensorObj* __restrict__ objs, int n_obj, __half* __restrict__ table)
+// ---- the pre-pass: ONE launch ----------------------------------------------------------------------------------------
+// Blocks [0, n_table_blocks): one block per (object, 16-observation block) of the B-operand table; thread m < NL owns offset m.
+//   Stage layout (FP16), identical to one shared-memory B stage:  [plane: b_hi, b2_hi, (b_lo, b2_lo)] [k chunk c = 0,1]
+//   [column n] [k%8] with column n = m (Re) or NL + m (Im) and observation 16 kb + 8 c + k%8, then the aux block (FP32).
+//   Observations past N_t are zero everywhere (v = 0 makes the generated A operand vanish too).
+// Blocks [n_table_blocks, n_table_blocks + n_obj): per-object statistics (mean, power-of-two scales).
+template <bool FAST>
+__global__ void __launch_bounds__(kTcPreThreads)
+lsp_tensor_prepass_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const float* __restrict__ t,
+                          const float* __restrict__ y, const float* __restrict__ wgt, TensorObj* __restrict__ objs, int n_obj,
+                          long long n_table_blocks, int center, int normalize, unsigned char* __restrict__ table)
 {
-    // locate the object of this block: binary search on kb_off (exclusive scan, non-decreasing)
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if ((long long)blockIdx.x >= n_table_blocks) {
+        // ---------------- statistics of object o ----------------
+        __shared__ double red[4][4];
+        const int o = (int)((long long)blockIdx.x - n_table_blocks);
+        const int64_t lo = offsets[gp.obj_base + o], n = offsets[gp.obj_base + o + 1] - lo;
+        double s = 0.0;
+        if (center) {
+            for (int64_t j = tid; j < n; j += kTcPreThreads) s += (double)y[lo + j];
+            for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+            if (lane == 0) red[0][wid] = s;
+            __syncthreads();
+            s = red[0][0] + red[0][1] + red[0][2] + red[0][3];
+        }
+        const double mean = (center && n > 0) ? s / (double)n : 0.0;
+        double q = 0.0, mx = 0.0, mw = 0.0;
+        for (int64_t j = tid; j < n; j += kTcPreThreads) {
+            const double v = (double)y[lo + j] - mean;
+            q += v * v;
+            mx = fmax(mx, fabs(v));
+            if (wgt) mw = fmax(mw, fabs((double)wgt[lo + j]));
+        }
+        for (int d = 16; d > 0; d >>= 1) {
+            q += __shfl_xor_sync(0xffffffffu, q, d);
+            mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+            mw = fmax(mw, __shfl_xor_sync(0xffffffffu, mw, d));
+        }
+        if (lane == 0) { red[1][wid] = q; red[2][wid] = mx; red[3][wid] = mw; }
+        __syncthreads();
+        if (tid == 0) {
+            q = red[1][0] + red[1][1] + red[1][2] + red[1][3];
+            mx = fmax(fmax(red[2][0], red[2][1]), fmax(red[2][2], red[2][3]));
+            mw = fmax(fmax(red[3][0], red[3][1]), fmax(red[3][2], red[3][3]));
+            auto pow2_scale = [](double m) {       // 2^e with m * 2^e in [256, 512); 1 for m = 0 / non-finite
+                int e = 0;
+                if (!(m > 0.0) || !isfinite(m)) return 1.0;
+                frexp(m, &e);                      // m = f * 2^e, f in [0.5, 1)
+                return ldexp(1.0, max(-100, min(100, 9 - e)));
+            };
+            TensorObj ob;
+            ob.mean = mean;
+            const double ys = pow2_scale(mx);
+            ob.yscale = (float)ys;
+            ob.zinv = (float)(1.0 / ys);
+            const double nrm = normalize ? (q > 0.0 ? 2.0 / q : 0.0) : 1.0;
+            ob.nrm = (float)nrm;
+            ob.pscale = (float)(nrm * (double)kTcUnitScale / (ys * ys));
+            const double ws = wgt ? pow2_scale(mw) : (double)kTcUnitScale;
+            ob.wscale = (float)ws;
+            ob.winv = (float)(1.0 / ws);
+            objs[o] = ob;
+        }
+        return;
+    }
+    // ---------------- one stage of the B-operand table ----------------
     const int64_t blk = blockIdx.x;
-    if (blk >= objs[n_obj].kb_off) return;     // the grid is an upper bound
-    int lo_o = 0, hi_o = n_obj - 1;
+    int lo_o = 0, hi_o = n_obj - 1;                 // largest o with kb_off(o) <= blk (kb_off is strictly increasing)
     while (lo_o < hi_o) {
         const int mid = (lo_o + hi_o + 1) >> 1;
-        if (objs[mid].kb_off <= blk) lo_o = mid; else hi_o = mid - 1;
+        if (tc_kb_off(offsets, gp.obj_base, mid) <= blk) lo_o = mid; else hi_o = mid - 1;
     }
-    // objects with zero blocks share kb_off with their successor: the search lands on the last of them, which is the one
-    // that owns the block as long as it has blocks; step forward is never needed because equal offsets mean empty objects.
     const int o = lo_o;
-    const int64_t obj = (int64_t)o + gp.obj_base;
-    const int64_t base = offsets[obj], n_t = offsets[obj + 1] - base;
-    const int kb = (int)(blk - objs[o].kb_off);
-    const int m = threadIdx.x;
+    const int64_t base = offsets[gp.obj_base + o], n_t = offsets[gp.obj_base + o + 1] - base;
+    const int kb = (int)(blk - tc_kb_off(offsets, gp.obj_base, o));
+    if (kb >= tc_n_kb(n_t)) return;                 // slack block between two objects
+    unsigned char* stage = table + (size_t)blk * (size_t)tp.b_stage_bytes;
+    const int L = 2 * tp.nl;
+    {   // aux: t, y, w of the 16 observations and the tile-independent phasors v (two versions)
+        float* aux = reinterpret_cast<float*>(stage + (size_t)tp.n_ops * tp.b_plane_bytes);
+        const int j16 = tid & 15, g1 = tid >> 4;
+        const int64_t j = (int64_t)kb * kTcKB + j16;
+        const bool live = j < n_t;
+        const float tj = live ? t[base + j] : 0.f;
+        if (tid < 16) {
+            aux[tid] = tj;
+            aux[16 + tid] = live ? y[base + j] : 0.f;
+            aux[32 + tid] = live ? (wgt ? wgt[base + j] : 1.f) : 0.f;
+        }
+        float sn = 0.f, cs = 0.f;
+        if (live) {
+            const float r = (float)frac_cycles((double)(8 * g1) * (double)L * gp.df * (double)tj);
+            if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
+        }
+        const float h = 0.70710678118654752f;
+        const int pos = 4 * (j16 >> 1) + (j16 & 1);                // pair-planar: (c0, c1, s0, s1)
+        aux[48 + g1 * kTcVRow + pos] = cs;
+        aux[48 + g1 * kTcVRow + pos + 2] = sn;
+        aux[48 + (8 + g1) * kTcVRow + pos] = (cs + sn) * h;
+        aux[48 + (8 + g1) * kTcVRow + pos + 2] = (sn - cs) * h;
+    }
+    const int m = tid;
     if (m >= tp.nl) return;
     const double f_beta = ((double)m + 0.5) * gp.df;
-    const int n_cols = 2 * tp.nl;
-    const int plane = n_cols * kTcKB;                           // halfs per plane
-    __half* dst = table + (size_t)blk * (size_t)(tp.n_ops * plane);
+    const int n_cols = L;
+    const int plane = tp.b_plane_bytes / 2;                         // halfs per plane
+    __half* dst = reinterpret_cast<__half*>(stage);
     float c1[kTcKB], s1[kTcKB];
 #pragma unroll
     for (int k = 0; k < kTcKB; ++k) {
@@ -217,7 +239,7 @@ lsp_tensor_table_kernel(GridParams gp, TensorParams tp, const int64_t* __restric
         float sn = 0.f, cs = 0.f;
         if (j < n_t) {
             const float r = (float)frac_cycles(f_beta * (double)t[base + j]);
-            sincos_cycles<FAST>(r, &sn, &cs);
+            if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
         }
         c1[k] = cs;
         s1[k] = sn;
@@ -265,12 +287,14 @@ __device__ __forceinline__ uint64_t tc_smem_desc(unsigned saddr, unsigned lbo_by
     d |= (uint64_t)1 << 46;
     return d;
 }
-__device__ __forceinline__ void tc_mma_f16(unsigned d_tmem, uint64_t a_desc, uint64_t b_desc, unsigned idesc, unsigned accumulate)
+// D[tmem] (+)= A[tmem] * B[smem]: the A operand (128 rows x 16 FP16 = 8 columns, row = lane, k even in the low half-word)
+// is read from tensor memory, B through a shared-memory descriptor.
+__device__ __forceinline__ void tc_mma_f16_ts(unsigned d_tmem, unsigned a_tmem, uint64_t b_desc, unsigned idesc, unsigned accumulate)
 {
     asm volatile(
         "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
 }
 __device__ __forceinline__ void tc_commit(unsigned long long* bar)
 {
@@ -278,13 +302,13 @@ __device__ __forceinline__ void tc_commit(unsigned long long* bar)
 }
 // mbarrier wait for roles whose waits are long when they are not the bottleneck (generators on a full ring, epilogue on
 // unfinished accumulators): back off between polls so the spinning warps do not take issue slots from the working ones.
-__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* bar, unsigned parity)
+__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* bar, unsigned parity, unsigned ns = 40u)
 {
     unsigned done;
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                  : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     while (!done) {
-        __nanosleep(40);
+        __nanosleep(ns);
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     }
@@ -309,6 +333,25 @@ __device__ __forceinline__ void tc_ld16(unsigned taddr, float* v)
     for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ void tc_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// 8 consecutive TMEM columns of this thread's lane <- 8 registers (one A-operand plane of a stage: 16 FP16 of one row)
+__device__ __forceinline__ void tc_st8(unsigned taddr, const unsigned (&r)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
+}
+__device__ __forceinline__ void tc_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float4 lds128(unsigned saddr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
+}
+__device__ __forceinline__ float lds32(unsigned saddr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(saddr));
+    return v;
+}
 __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes)
 {
     asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
@@ -318,10 +361,9 @@ __device__ __forceinline__ void tma_bulk_g2s(void* smem_dst, const void* gmem_sr
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 struct TcItem {
-    int64_t obj_local, obj, lo, n_t, K0;
+    int64_t obj_local, obj, n_t, K0;
     int tile, split, kb0, kb1;
 };
 __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorParams& tp, long long item,
@@ -333,8 +375,7 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
     w.tile = (int)(r % gp.n_tiles);
     w.obj_local = r / gp.n_tiles;
     w.obj = w.obj_local + gp.obj_base;
-    w.lo = offsets[w.obj];
-    w.n_t = offsets[w.obj + 1] - w.lo;
+    w.n_t = offsets[w.obj + 1] - offsets[w.obj];
     const int nkb = tc_n_kb(w.n_t);
     w.kb0 = (int)(((long long)nkb * w.split) / gp.n_split);
     w.kb1 = (int)(((long long)nkb * (w.split + 1)) / gp.n_split);
@@ -342,54 +383,164 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
     return w;
 }
 
-constexpr size_t tc_smem_bytes(int stages_a, int stages_b, int a_stage, int b_stage)
+// The generators wait on the B ring's "full" barriers out of step with the MMA warp; their parity waits stay within one phase of
+// the barrier only if the ring is at least NG + D stages deep (D = A-ring depth; see the kernel's hand-off protocol).
+constexpr int tc_min_stages_b(bool fast, int ng)
 {
-    return 1024 /* alignment slack */ + (size_t)stages_a * (size_t)a_stage + (size_t)stages_b * (size_t)b_stage + 512;
+    const int as = kTcACols / (fast ? 16 : 32);
+    return ng + (as < ng ? as : ng);
+}
+// ---- split-N_t fix-up (n_split > 1) ----------------------------------------------------------------------------------
+// The n_split partial slots of a tile (lane-oriented un-scaled sums in the epilogue's own element order: element (i, row r)
+// at i * 128 + r, see the epilogue) are added in SPLIT ORDER -- results do not depend on scheduling -- and steps 5, 6, 6'
+// run on the totals.  One CTA per (object, tile, part): part p of kTcFixParts takes every kTcFixParts-th unit; a unit is
+// (row, four consecutive m); consecutive threads take consecutive rows, so every load is fully coalesced.  A kernel of its
+// own because it needs the whole GPU's memory parallelism: the same sums inside the main kernel's epilogue warps (a few
+// hundred threads per tile) are bound by the latency of their few loads in flight.
+constexpr int kTcFixThreads = 256;
+constexpr int kTcFixParts = 4;
+template <typename T>
+__global__ void __launch_bounds__(kTcFixThreads)
+lsp_tensor_fix_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
+                      const float4* __restrict__ sums, T* __restrict__ out_power, Best* __restrict__ partials, int64_t n_obj_launch)
+{
+    __shared__ Best sbest[kTcFixThreads / 32];
+    const int part = (int)(blockIdx.x % kTcFixParts);
+    const long long r0 = blockIdx.x / kTcFixParts;
+    const int tile = (int)(r0 % gp.n_tiles);
+    const int64_t obj_local = r0 / gp.n_tiles, obj = obj_local + gp.obj_base;
+    const int NL = tp.nl, L = 2 * NL;
+    const int n_quads = (NL + 3) >> 2;
+    const int64_t K0 = (int64_t)tile * tp.tile;
+    const int n_valid = (int)min((int64_t)tp.tile, (int64_t)gp.n_freq - K0);
+    const bool ragged = n_valid < tp.tile;
+    const bool vec_ok = (gp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(out_power) & 15) == 0);
+    const float n_t = (float)(offsets[obj + 1] - offsets[obj]);
+    const float nrm = objs[obj_local].nrm;
+    const int64_t tile_elems = (int64_t)((NL + 15) >> 4) * 16 * 128;
+    const float4* slot0 = sums + (obj_local * gp.n_tiles + tile) * tile_elems;
+    const int64_t sstride = n_obj_launch * (int64_t)gp.n_tiles * tile_elems;
+    T* otile = out_power ? out_power + obj_local * (int64_t)gp.n_freq + K0 : nullptr;
+    float bp = -1.0f;
+    int bk = 0x7fffffff;
+    for (int u = part * kTcFixThreads + threadIdx.x; u < 128 * n_quads; u += kTcFixParts * kTcFixThreads) {
+        const int r = u & 127, i0 = (u >> 7) * 4;
+        const bool is_im = (r & 16) != 0;
+        const int g = 16 * (r >> 5) + (r & 15);
+        const int kc = g * L + NL;
+        const float4* src = slot0 + (int64_t)i0 * 128 + r;
+        float4 acc[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) acc[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+        int sp = 0;
+        for (; sp + 2 <= gp.n_split; sp += 2) {                    // fixed order: split 0, 1, 2, ...; 8 loads in flight
+            float4 v0[4], v1[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                v0[e] = src[(int64_t)sp * sstride + e * 128];
+                v1[e] = src[(int64_t)(sp + 1) * sstride + e * 128];
+            }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                acc[e].x = (acc[e].x + v0[e].x) + v1[e].x;  acc[e].y = (acc[e].y + v0[e].y) + v1[e].y;
+                acc[e].z = (acc[e].z + v0[e].z) + v1[e].z;  acc[e].w = (acc[e].w + v0[e].w) + v1[e].w;
+            }
+        }
+        if (sp < gp.n_split) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float4 v = src[(int64_t)sp * sstride + e * 128];
+                acc[e].x += v.x;  acc[e].y += v.y;  acc[e].z += v.z;  acc[e].w += v.w;
+            }
+        }
+        // Re rows: (x, y, z, w) = (xc, xs, c2, s2) of k = kc + i;  Im rows: (xs, xc, s2, c2) of k = kc - 1 - i
+        float pw[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+            pw[e] = power_from_sums<float>(is_im ? acc[e].y : acc[e].x, is_im ? acc[e].x : acc[e].y, is_im ? acc[e].w : acc[e].z,
+                                           is_im ? acc[e].z : acc[e].w, n_t, nrm);
+        const int klv = is_im ? (kc - i0 - 4) : (kc + i0);         // first of the four consecutive grid points
+        float o4[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) o4[e] = is_im ? pw[3 - e] : pw[e];      // ascending frequency
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int k = klv + e;
+            if (k < n_valid && o4[e] == o4[e] && (o4[e] > bp || (o4[e] == bp && k < bk))) { bp = o4[e]; bk = k; }
+        }
+        if (otile) {
+            if (!ragged && vec_ok) {
+                *reinterpret_cast<float4*>(otile + klv) = make_float4(o4[0], o4[1], o4[2], o4[3]);
+            } else {
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    if (klv + e < n_valid) otile[klv + e] = (T)o4[e];
+            }
+        }
+    }
+    if (partials) {
+        Best mine;
+        mine.p = (double)bp;
+        mine.k = (bk == 0x7fffffff) ? INT64_MAX : K0 + (int64_t)bk;
+        const Best b = block_best(mine, sbest);
+        if (threadIdx.x == 0) partials[(obj_local * gp.n_tiles + tile) * kTcFixParts + part] = b;
+    }
 }
 
-template <typename T, bool FAST, int EW, int NG>
+constexpr size_t tc_smem_bytes(int stages_b, int b_stage)
+{
+    return 1024 /* alignment slack */ + (size_t)stages_b * (size_t)b_stage + 256 /* barriers */;
+}
+// static shared memory of the kernel (generator scratch etc.), for the host's ring sizing
+template <int EW, int NG> constexpr int tc_static_smem() { return NG * 2 * (8 * kTcVRow + 32) * 4 + EW * 16 + 256; }
+
+template <typename T, bool FAST, int EW, int NG, bool WGT>
 __global__ void __launch_bounds__((TcRoles<EW, NG>::kThreads), 1)
-lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
-                  const T* __restrict__ y, const TensorObj* __restrict__ objs, const __half* __restrict__ table,
-                  T* __restrict__ out_power, Best* __restrict__ partials, float4* __restrict__ sums,
-                  int64_t n_obj_launch, long long total_items)
+lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
+                  const unsigned char* __restrict__ table, T* __restrict__ out_power, Best* __restrict__ partials,
+                  float4* __restrict__ sums, int64_t n_obj_launch, long long total_items)
 {
     using R = TcRoles<EW, NG>;
-    constexpr int kTcEpiWarps = EW, kTcEpiThreads = R::kEpiThreads;
+    constexpr int kEpiWarps = EW, kEpiThreads = R::kEpiThreads;
     constexpr int NOPS = FAST ? 2 : 4;
-    constexpr int A_PLANE = 128 * kTcKB * 2;                  // bytes of one A plane: 128 rows x 16 x FP16
+    constexpr int A_STAGE_COLS = NOPS * 8;                    // TMEM columns of one A stage
+    constexpr int AS = kTcACols / A_STAGE_COLS;               // A stages that fit in the ring's columns: 2 (accurate) or 4 (fast)
+    // Hand-off protocol of the A ring.  Stage s (numbered per CTA across items) is built by generator group s % NG into TMEM
+    // slot s % D, D = min(AS, NG).  mbarrier waits are parity waits: a waiter must never be two phases away from its barrier,
+    // so the "slot is free" signal is kept PER GROUP, not per slot: the commit that follows the MMAs of stage j arrives on
+    // free_g[(j + D) % NG], the barrier of the group that will write stage j + D into the slot stage j occupied.  Group k thus
+    // sees exactly one arrival per stage it builds (none for its first stage if that is one of the first D), waits for
+    // them strictly in order, and arrival i + 1 cannot precede its consumption of arrival i (it needs MMA(s + NG - D), which
+    // is issued after MMA(s), which needs this group's stage s).  full_a[slot] is waited on by the MMA warp only, in order.
+    constexpr int D = AS < NG ? AS : NG;
     extern __shared__ unsigned char smem_dyn[];
-    unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
-    // Two rings: A stages (16 KB, written by the generators) and B stages (up to 32 KB, filled by TMA).  The A ring is the
-    // deep one: while the epilogue of a short item holds TMEM, the generators keep building the next item's stages.
-    const int S = tp.stages, SB = tp.stages_b;
-    const int stage_bytes = tp.a_stage_bytes;                 // A ring stride
-    const int b_plane = 2 * tp.nl * kTcKB * 2;                // bytes of one B plane
-    unsigned char* smem_b = smem + (size_t)S * tp.a_stage_bytes;
-    unsigned long long* full = reinterpret_cast<unsigned long long*>(smem_b + (size_t)SB * tp.b_stage_bytes);   // A ring
-    unsigned long long* empty = full + 8;
-    unsigned long long* full_b = empty + 8;                   // B ring
+    unsigned char* smem_b = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+    const int SB = tp.stages_b;
+    const unsigned b_bytes = (unsigned)tp.b_stage_bytes;
+    const int aux_off = NOPS * tp.b_plane_bytes;              // byte offset of the aux block inside a B stage
+    unsigned long long* full_b = reinterpret_cast<unsigned long long*>(smem_b + (size_t)SB * b_bytes);
     unsigned long long* empty_b = full_b + 8;
-    unsigned long long* tmem_full = empty_b + 8;
+    unsigned long long* full_a = empty_b + 8;
+    unsigned long long* free_g = full_a + 4;
+    unsigned long long* tmem_full = free_g + 4;
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
-    __shared__ Best sbest[kTcEpiWarps];
-    __shared__ __align__(16) float s_uv[NG][2][3 * kTcScratchPlane]; // generator scratch: [group][buffer][plane][j/4][phasor q][j%4]
-    __shared__ __align__(16) float s_yv[NG][2][kTcKB];               // scaled, centred y of the stage
+    __shared__ Best sbest[kEpiWarps];
+    // generator scratch: [group][buffer]: 8 rows (g0) of the tile's phasors u * 16, pair-planar like the aux rows, then the
+    // stage's scaled magnitudes for the "Re a" rows (16) and the "Im a" rows (16)
+    __shared__ __align__(16) float s_u[NG][2][8 * kTcVRow + 32];
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);      // broadcast: the compiler may treat the role as warp-uniform
     if (tid == 0) {
-        for (int s = 0; s < S; ++s) {
-            mbar_init(&full[s], kTcGenGroupThreads);
-            mbar_init(&empty[s], 1);
-        }
         for (int s = 0; s < SB; ++s) {
             mbar_init(&full_b[s], 1);
             mbar_init(&empty_b[s], 1);
         }
+        for (int s = 0; s < D; ++s) mbar_init(&full_a[s], 4);     // one arrival per generator warp of the stage's group
+        for (int s = 0; s < NG; ++s) mbar_init(&free_g[s], 1);
         mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, kTcEpiThreads);
+        mbar_init(tmem_empty, kEpiThreads);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
@@ -403,15 +554,13 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
 
     if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kCtrlRegs));
     if (warp == 0) {
-        // =============================== TMA producer: B stages from the per-object table ========================
+        // =============================== TMA producer: B stages (+ aux) from the per-object table ================
         if (lane == 0) {
             int st = 0;
             unsigned ph = 1;                                      // parity of the "empty" phase to wait for
-            const unsigned b_bytes = (unsigned)tp.b_stage_bytes;
             for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
                 const TcItem w = tc_decode(gp, tp, item, offsets);
-                const unsigned char* src = reinterpret_cast<const unsigned char*>(table) +
-                                           (size_t)(objs[w.obj_local].kb_off + w.kb0) * (size_t)b_bytes;
+                const unsigned char* src = table + (size_t)(tc_kb_off(offsets, gp.obj_base, w.obj_local) + w.kb0) * (size_t)b_bytes;
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
                     mbar_wait(&empty_b[st], ph);
                     mbar_arrive_expect_tx(&full_b[st], b_bytes);
@@ -425,60 +574,61 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         // =============================== MMA issuer ===============================================================
         // The whole warp runs the loop with warp-uniform values (item ranges are broadcast from lane 0), so descriptors
         // and barrier addresses live in uniform registers; one elected lane issues the MMAs and commits.
-        {
-            const unsigned idesc = (1u << 4) | ((unsigned)((2 * tp.nl) >> 3) << 17) | ((unsigned)(128 >> 4) << 24);
-            const unsigned a_lbo = 16 * 128, b_lbo = (unsigned)(2 * tp.nl / 8) * 128, sbo = 128;
-            // Descriptors of stage 0; stage s adds s * stage_bytes / 16 to the 14-bit start-address field (the whole ring
-            // lies below 256 KB, so the field never carries into the LBO bits).
-            const unsigned sa0 = smem_u32(smem), sb0 = smem_u32(smem_b);
-            const uint64_t a_zh0 = tc_smem_desc(sa0, a_lbo, sbo), a_wh0 = tc_smem_desc(sa0 + A_PLANE, a_lbo, sbo);
-            const uint64_t a_zl0 = tc_smem_desc(sa0 + 2 * A_PLANE, a_lbo, sbo), a_wl0 = tc_smem_desc(sa0 + 3 * A_PLANE, a_lbo, sbo);
-            const uint64_t b_zh0 = tc_smem_desc(sb0, b_lbo, sbo), b_wh0 = tc_smem_desc(sb0 + b_plane, b_lbo, sbo);
-            const uint64_t b_zl0 = tc_smem_desc(sb0 + 2 * b_plane, b_lbo, sbo), b_wl0 = tc_smem_desc(sb0 + 3 * b_plane, b_lbo, sbo);
-            const uint64_t stage_inc = (uint64_t)(tp.a_stage_bytes >> 4), stage_inc_b = (uint64_t)(tp.b_stage_bytes >> 4);
-            int st = 0, stb = 0;
-            unsigned ph = 0, phb = 0, n_acc = 0;
-            uint64_t so = 0, sob = 0;                             // st * stage_inc, stb * stage_inc_b
-            for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
-                const TcItem w = tc_decode(gp, tp, item, offsets);
-                const int kb0 = __shfl_sync(0xffffffffu, w.kb0, 0), kb1 = __shfl_sync(0xffffffffu, w.kb1, 0);
-                if (kb1 <= kb0) continue;
-                mbar_wait(tmem_empty, (n_acc & 1) ^ 1);          // the epilogue has drained the previous accumulators
+        const unsigned idesc = (1u << 4) | ((unsigned)((2 * tp.nl) >> 3) << 17) | ((unsigned)(128 >> 4) << 24);
+        const unsigned b_lbo = (unsigned)(2 * tp.nl / 8) * 128, sbo = 128;
+        // Descriptors of B stage 0; stage s adds s * stage_bytes / 16 to the 14-bit start-address field (the whole ring
+        // lies below 256 KB, so the field never carries into the LBO bits).
+        const unsigned sb0 = smem_u32(smem_b);
+        const uint64_t b_zh0 = tc_smem_desc(sb0, b_lbo, sbo), b_wh0 = tc_smem_desc(sb0 + tp.b_plane_bytes, b_lbo, sbo);
+        const uint64_t b_zl0 = tc_smem_desc(sb0 + 2 * tp.b_plane_bytes, b_lbo, sbo), b_wl0 = tc_smem_desc(sb0 + 3 * tp.b_plane_bytes, b_lbo, sbo);
+        const uint64_t stage_inc_b = (uint64_t)(b_bytes >> 4);
+        const unsigned d_z = tmem, d_w = tmem + kTcWCol, a0 = tmem + kTcACol;
+        const bool do_w = tp.z_only == 0;
+        int sa = 0, stb = 0, gsel = D % NG;                      // A slot, B slot, group that reuses the A slot next
+        unsigned pha = 0, phb = 0, n_acc = 0;
+        uint64_t sob = 0;                                         // stb * stage_inc_b
+        for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
+            const TcItem w = tc_decode(gp, tp, item, offsets);
+            const int kb0 = __shfl_sync(0xffffffffu, w.kb0, 0), kb1 = __shfl_sync(0xffffffffu, w.kb1, 0);
+            if (kb1 <= kb0) continue;
+            mbar_wait(tmem_empty, (n_acc & 1) ^ 1);              // the epilogue has drained the previous accumulators
+            tc_fence_after();
+            unsigned acc = 0;
+            for (int kb = kb0; kb < kb1; ++kb) {
+                mbar_wait(&full_b[stb], phb);
+                mbar_wait(&full_a[sa], pha);
                 tc_fence_after();
-                unsigned acc = 0;
-                for (int kb = kb0; kb < kb1; ++kb) {
-                    mbar_wait(&full_b[stb], phb);
-                    mbar_wait(&full[st], ph);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        // planes: 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
-                        if (!FAST) {
-                            tc_mma_f16(tmem, a_zl0 + so, b_zh0 + sob, idesc, acc);
-                            tc_mma_f16(tmem, a_zh0 + so, b_zl0 + sob, idesc, 1u);
-                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + sob, idesc, 1u);
-                            tc_mma_f16(tmem + 256, a_wl0 + so, b_wh0 + sob, idesc, acc);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wl0 + sob, idesc, 1u);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + sob, idesc, 1u);
-                        } else {
-                            tc_mma_f16(tmem, a_zh0 + so, b_zh0 + sob, idesc, acc);
-                            tc_mma_f16(tmem + 256, a_wh0 + so, b_wh0 + sob, idesc, acc);
+                if (elect_one()) {
+                    // planes (A in TMEM and B in shared memory alike): 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
+                    const unsigned a = a0 + (unsigned)(sa * A_STAGE_COLS);
+                    if (!FAST) {
+                        tc_mma_f16_ts(d_z, a + 16, b_zh0 + sob, idesc, acc);
+                        tc_mma_f16_ts(d_z, a, b_zl0 + sob, idesc, 1u);
+                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, 1u);
+                        if (do_w) {
+                            tc_mma_f16_ts(d_w, a + 24, b_wh0 + sob, idesc, acc);
+                            tc_mma_f16_ts(d_w, a + 8, b_wl0 + sob, idesc, 1u);
+                            tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, 1u);
                         }
-                        tc_commit(&empty[st]);                   // both stages are free once these MMAs have read them
-                        tc_commit(&empty_b[stb]);
+                    } else {
+                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, acc);
+                        if (do_w) tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, acc);
                     }
-                    __syncwarp();
-                    acc = 1u;
-                    so += stage_inc;
-                    sob += stage_inc_b;
-                    if (++st == S) { st = 0; ph ^= 1; so = 0; }
-                    if (++stb == SB) { stb = 0; phb ^= 1; sob = 0; }
+                    tc_commit(&free_g[gsel]);                    // both stages are free once these MMAs have read them
+                    tc_commit(&empty_b[stb]);
                 }
-                if (elect_one()) tc_commit(tmem_full);           // accumulators complete
                 __syncwarp();
-                ++n_acc;
+                acc = 1u;
+                sob += stage_inc_b;
+                if (++sa == D) { sa = 0; pha ^= 1; }
+                if (++gsel == NG) gsel = 0;
+                if (++stb == SB) { stb = 0; phb ^= 1; sob = 0; }
             }
+            if (elect_one()) tc_commit(tmem_full);               // accumulators complete
+            __syncwarp();
+            ++n_acc;
         }
-    } else if (warp >= 4 && warp < 4 + kTcEpiWarps) {
+    } else if (warp >= 4 && warp < 4 + kEpiWarps) {
         // =============================== epilogue (steps 5, 6, 6') ================================================
         // Lane l of quadrant q holds row 32 q + l: lanes 0-15 the "Re a" rows (Srr, Sri) of groups 16 q + l, lanes 16-31
         // the "Im a" rows (Sir, Sii) of the same groups.  One shuffle per accumulator pairs them; the Re lane then owns
@@ -498,13 +648,14 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         const int ch0 = (n_chunks * half_sel) / kParts, ch1 = (n_chunks * (half_sel + 1)) / kParts;
         const bool vec_ok = (gp.n_freq % 4 == 0) && ((reinterpret_cast<uintptr_t>(out_power) & 15) == 0);
         const int kc = g * L + NL;                                // tile-local index of the first frequency above the centre
+        const bool do_w = tp.z_only == 0;
         unsigned n_acc = 0;
         for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
             const TcItem w = tc_decode(gp, tp, item, offsets);
             const TensorObj ob = objs[w.obj_local];
             const bool have = w.kb1 > w.kb0;
             if (have) {
-                mbar_wait_backoff(tmem_full, n_acc & 1);
+                mbar_wait_backoff(tmem_full, n_acc & 1, EW == 4 ? 400u : 100u);     // long items: the wait lasts a whole item
                 tc_fence_after();
             }
             float bp = -1.0f;                                     // running maximum (P >= 0; NaN never compares greater)
@@ -514,7 +665,6 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const int n_valid = (int)min((int64_t)tp.tile, (int64_t)gp.n_freq - w.K0);     // frequencies of this tile on the grid
             const bool ragged = n_valid < tp.tile;
             T* otile = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq + w.K0 : nullptr;
-            float4* stile = sums ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
             const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
             bool released = false;
             // one chunk = 16 accumulator columns of each of the four TMEM regions; RAG = the tile overhangs the grid
@@ -525,8 +675,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 if (have) {
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
-                    tc_ld16(ta + 256 + m0, wr);
-                    tc_ld16(ta + 256 + NL + m0, wi);
+                    tc_ld16(ta + kTcWCol + m0, wr);
+                    tc_ld16(ta + kTcWCol + NL + m0, wi);
                     tc_ld_wait();
                     if (ch == ch1 - 1) {                          // last TMEM read of this warp: the MMA warp may overwrite
                         tc_fence_before();
@@ -599,24 +749,38 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     }
                 }
             };
-            // split-N_t: un-scaled partial sums (xc, xs, c2, s2) per frequency for lsp_combine_kernel
+            // Partial sums instead of powers, un-scaled.
+            //   split-N_t (tp.fixup): the lane-oriented sums (za, zb, wa, wb) of element (ch, i) of thread (q, lane) go to
+            //     ((16 ch + i) * 128 + 32 q + lane) of this split's slot of the tile -- the epilogue's own order, every store a
+            //     fully coalesced 512-byte warp access; lsp_tensor_fix_kernel adds the slots in split order and finishes;
+            //   generalised mode: (xc, xs, c2, s2) per grid frequency, for lsp_gls_combine_kernel.
+            const int64_t tile_elems = (int64_t)n_chunks * 16 * 128;
+            float4* nat = (sums && tp.fixup) ? sums + (((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_tiles + w.tile) * tile_elems +
+                                                   32 * q + lane : nullptr;
+            float4* stile = (sums && !tp.fixup) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
             auto chunk_sums = [&](int ch) {
                 const int m0 = ch * 16;
                 float zr[16], zi[16], wr[16], wi[16];
                 if (have) {
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
-                    tc_ld16(ta + 256 + m0, wr);
-                    tc_ld16(ta + 256 + NL + m0, wi);
+                    if (do_w) {
+                        tc_ld16(ta + kTcWCol + m0, wr);
+                        tc_ld16(ta + kTcWCol + NL + m0, wi);
+                    }
                     tc_ld_wait();
                     if (ch == ch1 - 1) {
                         tc_fence_before();
                         mbar_arrive(tmem_empty);
                         released = true;
                     }
-                } else {
+                }
+                if (!have || !do_w) {
 #pragma unroll
-                    for (int i = 0; i < 16; ++i) zr[i] = zi[i] = wr[i] = wi[i] = 0.f;
+                    for (int i = 0; i < 16; ++i) {
+                        wr[i] = wi[i] = 0.f;
+                        if (!have) zr[i] = zi[i] = 0.f;
+                    }
                 }
                 const int i_lim = min(16, NL - m0);
                 const int kl0 = is_im ? (kc - 1 - m0) : (kc + m0);
@@ -624,15 +788,18 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 for (int i = 0; i < 16; ++i) {
                     const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
                     const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
-                    const float za = zr[i] - p1, zb = zi[i] + p0, wa = wr[i] - q1, wb = wi[i] + q0;
-                    const float xc = is_im ? zb : za, xs = is_im ? za : zb;
-                    const float c2 = is_im ? wb : wa, s2 = is_im ? wa : wb;
-                    const int kl = is_im ? kl0 - i : kl0 + i;
-                    if (i < i_lim && kl < n_valid)
-                        stile[kl] = make_float4(xc * ob.zinv, xs * ob.zinv, c2 * (1.0f / kTcUnitScale), s2 * (1.0f / kTcUnitScale));
+                    const float za = (zr[i] - p1) * ob.zinv, zb = (zi[i] + p0) * ob.zinv;
+                    const float wa = (wr[i] - q1) * ob.winv, wb = (wi[i] + q0) * ob.winv;
+                    if (nat) {
+                        nat[(int64_t)(m0 + i) * 128] = make_float4(za, zb, wa, wb);
+                    } else {
+                        const int kl = is_im ? kl0 - i : kl0 + i;
+                        if (i < i_lim && kl < n_valid)
+                            stile[kl] = make_float4(is_im ? zb : za, is_im ? za : zb, is_im ? wb : wa, is_im ? wa : wb);
+                    }
                 }
             };
-            if (stile) {
+            if (sums) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk_sums(ch);
             } else if (ragged) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk(ch, std::true_type{});
@@ -647,188 +814,165 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 }
                 ++n_acc;
             }
-            if (partials && !stile) {
+            if (partials && !sums) {
                 Best mine;
                 mine.p = (double)bp;
                 mine.k = (bk == 0x7fffffff) ? INT64_MAX : w.K0 + (int64_t)bk;
                 mine = warp_best(mine);
                 if (lane == 0) sbest[ew] = mine;
-                named_bar_sync(3, kTcEpiThreads);
+                named_bar_sync(3, kEpiThreads);
                 if (etid < 32) {
                     Best v;
                     v.p = -2.0;
                     v.k = INT64_MAX;
-                    if (lane < kTcEpiWarps) v = sbest[lane];
+                    if (lane < kEpiWarps) v = sbest[lane];
                     v = warp_best(v);
                     if (lane == 0) partials[w.obj_local * gp.n_tiles + w.tile] = v;
                 }
-                named_bar_sync(3, kTcEpiThreads);
+                named_bar_sync(3, kEpiThreads);
             }
         }
-    } else if (warp >= 4 + kTcEpiWarps) {
+    } else if (warp >= 4 + kEpiWarps) {
         // =============================== A-operand generators (steps 2-3) ==========================================
         // a_gj = y_j e^{i alpha_gj}, alpha_gj = 2 pi f(c_g) t_j, g = 8 g1 + g0.  Since f(c_g) = f(c_g0) + g1 (8 L df),
-        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}
-        // so a stage (16 observations) needs 16 x 16 sincos -- ONE per thread of a generator group (phase 1, into a
-        // small shared-memory scratch) -- instead of 64 x 16; phase 2 forms the 64 x 16 products on the FMA pipe, splits
-        // them into FP16 hi/lo and writes the UMMA operand planes.  Phases are FP32 two-float products (f = f_hi + f_lo,
-        // exact f_hi t through fma, reduced to (-1/2, 1/2] cycles before the low terms are added): no FP64 in the loop.
-        // Two groups of 8 warps take alternate ring stages, so one group's latencies (sincos chain, group barrier,
-        // LDS, mbarrier wait, proxy fence) are covered by the other group's instructions on the same schedulers.
-        // t / y of a group's NEXT stage (of this or a later work item) are loaded before its current stage is processed.
+        //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}.
+        // v does not depend on the tile: it arrives with the B stage (aux block).  Phase 1: the 128 threads of a group each
+        // evaluate ONE phasor u (g0, j) of the stage (two-float FP32 phase, reduced before the low terms are added) into a
+        // small scratch.  Phase 2: thread = A row r = 32 q + l (q = the warp's TMEM lane quadrant): lanes 0-15 the "Re a"
+        // rows of groups 16 q + l, lanes 16-31 the "Im a" rows.  With (p, q) = u v' for the 16 observations of the stage,
+        //     Re rows (v' = v):              a_Z = y p,             a_W = p^2 - q^2 = cos 2 alpha
+        //     Im rows (v' = v e^{-i pi/4}):  a_Z = y (p + q)/sqrt2, a_W = p^2 - q^2 = sin 2 alpha
+        // -- the same instruction stream for both halves of the warp (the lane's v row, a 0/1 factor and its y scale are
+        // the only differences).  The row's 16 values per plane are split into FP16 hi / lo, packed, and stored with
+        // tcgen05.st into the stage's TMEM columns; the MMAs read them from there.
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kGenRegs));
-        const int gw = warp - (4 + kTcEpiWarps);                  // 0 .. 8 NG - 1
-        const int grp = gw >> 3;                                  // generator group: stages with (stage number mod NG) == grp
-        const int gw8 = gw & 7;
-        const int gtid = (tid - (4 + kTcEpiWarps) * 32) & (kTcGenGroupThreads - 1);      // 0..255 inside the group
-        // phase 1 role: phasor q (0-7: u_g0, 8-15: v_g1) of observation j1 of the stage
-        const int q1 = gtid >> 4, j1 = gtid & 15;
-        const int sc_w = (j1 >> 2) * kTcScratchQuad + q1 * 4 + (j1 & 3);
-        // phase 2 role: 16-group row block qb, k chunk c, group g, observations 4 hsel .. 4 hsel + 3 of the chunk
-        const int qb = gw8 & 3, c = gw8 >> 2;
-        const int g = 16 * qb + (lane >> 1);
-        const int hsel = lane & 1;
-        const int row_re = 32 * qb + (lane >> 1), row_im = row_re + 16;
-        const int off_re = c * (16 * 128) + (row_re >> 3) * 128 + (row_re & 7) * 16 + hsel * 8;
-        const int off_im = c * (16 * 128) + (row_im >> 3) * 128 + (row_im & 7) * 16 + hsel * 8;
-        const int sc_u = (2 * c + hsel) * kTcScratchQuad + (g & 7) * 4;
-        const int sc_v = (2 * c + hsel) * kTcScratchQuad + (8 + (g >> 3)) * 4;
+        const int gw = warp - (4 + kEpiWarps);                    // 0 .. 4 NG - 1
+        const int grp = gw >> 2;                                  // generator group: stages with (stage number mod NG) == grp
+        const int q = warp & 3;                                   // TMEM lane quadrant (= gw & 3)
+        const int gtid = (gw & 3) * 32 + lane;                    // 0..127 inside the group
+        // phase 1 role: phasor u of (g0 = gtid & 7, observation j = gtid >> 3)
+        const int g0p = gtid & 7, jp = gtid >> 3;
+        // phase 2 role
+        const bool is_im = lane >= 16;
+        const int g = 16 * q + (lane & 15);
+        const int g0 = g & 7, g1 = g >> 3;
         const int NL = tp.nl, L = 2 * NL;
-        const double fv = (q1 >= 8) ? (double)(8 * (q1 - 8)) * (double)L * gp.df : 0.0;      // v: the same for every item
+        const float2 gam2 = is_im ? make_float2(1.f, 1.f) : make_float2(0.f, 0.f);
+        const bool do_w = tp.z_only == 0;
+        const unsigned trow = tmem + ((unsigned)(32 * q) << 16) + kTcACol;
+        const unsigned smem_b_u32 = smem_u32(smem_b);
+        const int v_row = is_im ? 8 + g1 : g1;
+        const int pos1 = g0p * kTcVRow + 4 * (jp >> 1) + (jp & 1);   // phase 1: where u (g0p, jp) goes (pair-planar)
 
         // A cursor walks the CTA's stage sequence (items in round-robin order, 16-observation blocks inside an item).
-        struct Cursor {
-            long long item;
-            int64_t lo;           // first observation of the object
-            int n_t, kb, kb1;
-            float f_hi, f_lo, mean, yscale;
+        long long item = blockIdx.x;
+        int left = 0;                                             // stages of `item` not yet consumed by this group's cursor
+        float f_hi = 0.f, f_lo = 0.f, mean = 0.f, ysc = 0.f, wsc = 0.f;
+        auto load_item = [&]() {                                  // `item` is set; returns its number of stages
+            const TcItem w = tc_decode(gp, tp, item, offsets);
+            const double fd = gp.f_min + ((double)(w.K0 + (int64_t)g0p * L + NL) - 0.5) * gp.df;
+            f_hi = (float)fd;
+            f_lo = (float)(fd - (double)f_hi);
+            const TensorObj ob = objs[w.obj_local];
+            mean = (float)ob.mean;
+            ysc = ob.yscale * (1.0f / kTcPhasorScale);
+            wsc = ob.wscale * (1.0f / kTcUnitScale);
+            return w.kb1 - w.kb0;
         };
-        auto load_item = [&](Cursor& cu) {        // cu.item is set; fills the rest; returns false if the item has no stages
-            const TcItem w = tc_decode(gp, tp, cu.item, offsets);
-            cu.lo = w.lo;
-            cu.n_t = (int)w.n_t;
-            cu.kb = w.kb0;
-            cu.kb1 = w.kb1;
-            const double fd = (q1 < 8) ? gp.f_min + ((double)(w.K0 + (int64_t)q1 * L + NL) - 0.5) * gp.df : fv;
-            cu.f_hi = (float)fd;
-            cu.f_lo = (float)(fd - (double)cu.f_hi);
-            cu.mean = (float)objs[w.obj_local].mean;
-            cu.yscale = objs[w.obj_local].yscale;
-            return w.kb1 > w.kb0;
+        auto seek = [&]() {                                       // first item at or after `item` that has stages
+            while (item < total_items && (left = load_item()) <= 0) item += gridDim.x;
         };
-        auto seek = [&](Cursor& cu) {             // first item at or after cu.item that has stages
-            while (cu.item < total_items && !load_item(cu)) cu.item += gridDim.x;
-        };
-        auto step = [&](Cursor& cu) {
-            if (++cu.kb >= cu.kb1) {
-                cu.item += gridDim.x;
-                seek(cu);
+        auto advance = [&](int n) {                               // move the cursor n stages ahead
+            while (n > 0 && item < total_items) {
+                if (left > n) { left -= n; n = 0; }
+                else { n -= left; item += gridDim.x; seek(); }
             }
         };
-        // cur = the group's stage being built (its t, y already in registers); its successor's (t, y) are loaded before
-        // the current stage is processed.
-        Cursor p1;
-        p1.item = blockIdx.x;
-        seek(p1);
-        for (int i = 0; i < grp; ++i)
-            if (p1.item < total_items) step(p1);
-        int st = grp;                                             // ring slot of the stage phase 2 writes
-        unsigned eph = 1;                                         // parity of the "empty" phase to wait for
-        while (st >= S) { st -= S; eph ^= 1; }
-        unsigned it = 0;
-        float* s_uvg = &s_uv[grp][0][0];
-        float* s_yvg = &s_yv[grp][0][0];
-        auto fetch = [&](const Cursor& cu, float& tv, float& yv_) {
-            tv = 0.f;
-            yv_ = 0.f;
-            if (cu.item < total_items) {
-                const int j = cu.kb * kTcKB + j1;
-                if (j < cu.n_t) { tv = (float)t[cu.lo + j]; yv_ = (float)y[cu.lo + j]; }
-            }
-        };
-        auto phase1 = [&](const Cursor& cu, float tv, float yv_, int buf) {
-            float* suv = s_uvg + buf * (3 * kTcScratchPlane);
-            const bool live = (cu.kb * kTcKB + j1) < cu.n_t;
-            const float p = cu.f_hi * tv;
-            const float e = fmaf(cu.f_hi, tv, -p);
-            const float r = (p - rintf(p)) + fmaf(cu.f_lo, tv, e);
-            float sn, cs;
-            if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
-            cs = live ? cs : 0.f;
-            sn = live ? sn : 0.f;
-            suv[sc_w] = cs;
-            suv[kTcScratchPlane + sc_w] = sn;
-            if (q1 < 8) suv[2 * kTcScratchPlane + sc_w] = -sn;
-            if (q1 == 0) s_yvg[buf * kTcKB + j1] = live ? (yv_ - cu.mean) * cu.yscale : 0.f;
-        };
-        float t_p1, y_p1;
-        fetch(p1, t_p1, y_p1);
-        while (p1.item < total_items) {
-            const int buf = it & 1;
-            const float* suv = s_uvg + buf * (3 * kTcScratchPlane);
-            const float* syv = s_yvg + buf * kTcKB;
-            // ---- phase 1 of this stage, then the loads of the group's next stage (two ring stages ahead)
-            phase1(p1, t_p1, y_p1, buf);
-#pragma unroll
-            for (int i = 0; i < NG; ++i)
-                if (p1.item < total_items) step(p1);
-            float t_pf, y_pf;
-            fetch(p1, t_pf, y_pf);
-            named_bar_sync(4 + grp, kTcGenGroupThreads);
-            const float4 ucv = *reinterpret_cast<const float4*>(&suv[sc_u]);
-            const float4 usv = *reinterpret_cast<const float4*>(&suv[kTcScratchPlane + sc_u]);
-            const float4 unv = *reinterpret_cast<const float4*>(&suv[2 * kTcScratchPlane + sc_u]);
-            const float4 vcv = *reinterpret_cast<const float4*>(&suv[sc_v]);
-            const float4 vsv = *reinterpret_cast<const float4*>(&suv[kTcScratchPlane + sc_v]);
-            const float4 yv = *reinterpret_cast<const float4*>(&syv[8 * c + 4 * hsel]);
-            // ---- phase 2: products (packed FP32x2), FP16 split, operand stores
-            float2 ar[2], ai[2], a2r[2], a2i[2];
+        seek();
+        advance(grp);
+        int sb = grp % SB, sa = grp % D;                          // ring slots of this group's current stage
+        unsigned phb = (unsigned)((grp / SB) & 1);
+        unsigned it = 0, n_wait = 0;                              // stages built; "slot free" arrivals consumed
+        while (item < total_items) {
+            float* su = &s_u[grp][it & 1][0];
+            const unsigned aux = smem_b_u32 + (unsigned)sb * b_bytes + (unsigned)aux_off;     // shared-space address of the aux block
+            mbar_wait_backoff(&full_b[sb], phb);                  // the stage's table block (and its aux) has landed
+            // ---- phase 1: u (g0p, jp), scaled by 16; threads with g0p = 0 also scale the stage's magnitudes
             {
-                const float2 k256 = make_float2(kTcUnitScale, kTcUnitScale), km256 = make_float2(-kTcUnitScale, -kTcUnitScale);
-                const float2 k512 = make_float2(2.f * kTcUnitScale, 2.f * kTcUnitScale);
-                const float2 uc[2] = {make_float2(ucv.x, ucv.y), make_float2(ucv.z, ucv.w)};
-                const float2 us[2] = {make_float2(usv.x, usv.y), make_float2(usv.z, usv.w)};
-                const float2 un[2] = {make_float2(unv.x, unv.y), make_float2(unv.z, unv.w)};
-                const float2 vc[2] = {make_float2(vcv.x, vcv.y), make_float2(vcv.z, vcv.w)};
-                const float2 vs[2] = {make_float2(vsv.x, vsv.y), make_float2(vsv.z, vsv.w)};
-                const float2 yy[2] = {make_float2(yv.x, yv.y), make_float2(yv.z, yv.w)};
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const float2 ec = __ffma2_rn(uc[h], vc[h], __fmul2_rn(un[h], vs[h]));      // uc vc - us vs
-                    const float2 es = __ffma2_rn(uc[h], vs[h], __fmul2_rn(us[h], vc[h]));      // uc vs + us vc
-                    ar[h] = __fmul2_rn(yy[h], ec);
-                    ai[h] = __fmul2_rn(yy[h], es);
-                    const float2 e256 = __fmul2_rn(ec, k256), n256 = __fmul2_rn(es, km256);
-                    a2r[h] = __ffma2_rn(e256, ec, __fmul2_rn(n256, es));                       // 256 (ec^2 - es^2)
-                    a2i[h] = __fmul2_rn(__fmul2_rn(ec, k512), es);                             // 512 ec es
+                const float tv = lds32(aux + 4 * jp);
+                const float p = f_hi * tv;
+                const float e = fmaf(f_hi, tv, -p);
+                const float r = (p - rintf(p)) + fmaf(f_lo, tv, e);
+                float sn, cs;
+                if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
+                su[pos1] = cs * kTcPhasorScale;
+                su[pos1 + 2] = sn * kTcPhasorScale;
+                if (g0p == 0) {
+                    const float ys = (lds32(aux + 64 + 4 * jp) - mean) * ysc;
+                    su[8 * kTcVRow + jp] = ys;                                  // "Re a" rows: y p
+                    su[8 * kTcVRow + 16 + jp] = ys * 0.70710678118654752f;      // "Im a" rows: y (p + q) / sqrt 2
                 }
             }
-            mbar_wait_backoff(&empty[st], eph);
-            const unsigned sa = smem_u32(smem) + (unsigned)st * (unsigned)stage_bytes;
-            // hi = fp16x2(x), lo = fp16x2(x - hi): one packed convert, two unpacks, one FFMA2, one packed convert per pair
-            auto put = [&](int plane_hi, int plane_lo, int off, const float2 (&x)[2]) {
-                const float2 m1 = make_float2(-1.f, -1.f);
-                const __half2 h0 = __floats2half2_rn(x[0].x, x[0].y), h1 = __floats2half2_rn(x[1].x, x[1].y);
-                asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane_hi * A_PLANE + off),
-                             "r"(*reinterpret_cast<const unsigned*>(&h0)), "r"(*reinterpret_cast<const unsigned*>(&h1)) : "memory");
-                if (!FAST) {
-                    const float2 r0 = __ffma2_rn(__half22float2(h0), m1, x[0]), r1 = __ffma2_rn(__half22float2(h1), m1, x[1]);
-                    const __half2 l0 = __floats2half2_rn(r0.x, r0.y), l1 = __floats2half2_rn(r1.x, r1.y);
-                    asm volatile("st.shared.v2.b32 [%0], {%1, %2};" ::"r"(sa + plane_lo * A_PLANE + off),
-                                 "r"(*reinterpret_cast<const unsigned*>(&l0)), "r"(*reinterpret_cast<const unsigned*>(&l1)) : "memory");
+            named_bar_sync(4 + grp, R::kGenGroupThreads);
+            // ---- phase 2: this row's 16 operand values per plane
+            const unsigned up = smem_u32(su + g0 * kTcVRow);
+            const unsigned vp = aux + 4 * (48 + v_row * kTcVRow);
+            const unsigned yp = smem_u32(su + 8 * kTcVRow + (is_im ? 16 : 0));
+            unsigned zh[8], zl[8], wh[8], wl[8];
+            float4 y4 = make_float4(0.f, 0.f, 0.f, 0.f), w4 = y4;
+#pragma unroll
+            for (int h = 0; h < 8; ++h) {                          // observations 2 h, 2 h + 1
+                const float4 uu = lds128(up + 16 * h), vv = lds128(vp + 16 * h);               // (c0, c1, s0, s1)
+                const float2 uc = make_float2(uu.x, uu.y), us = make_float2(uu.z, uu.w);
+                const float2 vc = make_float2(vv.x, vv.y), vs = make_float2(vv.z, vv.w);
+                if ((h & 1) == 0) y4 = lds128(yp + 16 * (h >> 1));
+                const float2 ys2 = (h & 1) ? make_float2(y4.z, y4.w) : make_float2(y4.x, y4.y);
+                const float2 pp = __ffma2_rn(uc, vc, __fmul2_rn(make_float2(-us.x, -us.y), vs));     // uc vc - us vs
+                const float2 qq = __ffma2_rn(uc, vs, __fmul2_rn(us, vc));                            // uc vs + us vc
+                const float2 az = __fmul2_rn(__ffma2_rn(qq, gam2, pp), ys2);
+                auto pack = [&](const float2 x, unsigned& hi, unsigned& lo) {
+                    const __half2 hh = __floats2half2_rn(x.x, x.y);
+                    hi = *reinterpret_cast<const unsigned*>(&hh);
+                    if (!FAST) {
+                        const float2 r = __ffma2_rn(__half22float2(hh), make_float2(-1.f, -1.f), x);     // one packed op
+                        const __half2 ll = __floats2half2_rn(r.x, r.y);
+                        lo = *reinterpret_cast<const unsigned*>(&ll);
+                    }
+                };
+                pack(az, zh[h], zl[h]);
+                if (do_w) {
+                    float2 aw = __ffma2_rn(make_float2(-qq.x, -qq.y), qq, __fmul2_rn(pp, pp));       // p^2 - q^2 (x 256)
+                    if (WGT) {
+                        if ((h & 1) == 0) w4 = lds128(aux + 128 + 16 * (h >> 1));
+                        const float2 ww = (h & 1) ? make_float2(w4.z, w4.w) : make_float2(w4.x, w4.y);
+                        aw = __fmul2_rn(aw, __fmul2_rn(ww, make_float2(wsc, wsc)));
+                    }
+                    pack(aw, wh[h], wl[h]);
                 }
-            };
-            put(0, 2, off_re, ar);
-            put(0, 2, off_im, ai);
-            put(1, NOPS - 1, off_re, a2r);
-            put(1, NOPS - 1, off_im, a2i);
-            fence_proxy_async();            // generic-proxy stores -> visible to the tensor core's async proxy
-            mbar_arrive(&full[st]);
-            st += NG;
-            while (st >= S) { st -= S; eph ^= 1; }
+            }
+            // ---- into the stage's TMEM columns once the MMAs that read its previous contents have completed
+            if (it > 0 || grp >= D) {                             // not one of the CTA's first D stages
+                mbar_wait(&free_g[grp], n_wait & 1);              // on the critical path (2-deep ring): no sleep between polls
+                ++n_wait;
+            }
+            tc_fence_after();
+            const unsigned ta = trow + (unsigned)(sa * A_STAGE_COLS);
+            tc_st8(ta, zh);
+            if (do_w) tc_st8(ta + 8, wh);
+            if (!FAST) {
+                tc_st8(ta + 16, zl);
+                if (do_w) tc_st8(ta + 24, wl);
+            }
+            tc_st_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&full_a[sa]);
+            // ---- next stage of this group
+            advance(NG);
+            sb += NG;
+            while (sb >= SB) { sb -= SB; phb ^= 1; }
+            sa = (sa + NG) % D;
             ++it;
-            t_p1 = t_pf;
-            y_p1 = y_pf;
         }
     }
     // teardown: everyone is done with TMEM before it is freed

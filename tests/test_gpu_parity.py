@@ -127,12 +127,12 @@ def test_config2_shape_small(lsp, oracle, dtype, fast, variant):
     assert_best_parity(best, P_ref, w, dtype, oracle)
 
 
-@pytest.mark.parametrize("n_freq,fast", [(200_000, False), (199_999, False), (200_002, True)])
+@pytest.mark.parametrize("n_freq,fast", [(100_000, False), (99_999, False), (100_002, True)])
 def test_long_single_object_full_grid_long_item_shape(lsp, oracle, n_freq, fast):
-    """The long-item role shape through the scheduler's OWN choice (no override): one object of N_t = 10,000 on a grid of a
-    dozen tiles is split by observations into items of >= 48 stages (the config-2 launch configuration at 1/5 of its grid).
-    Full grid against the oracle, N_f % 4 in {0, 3, 2}."""
-    w = make_config(2, dtype="f32", n_t=10_000, n_freq=n_freq)
+    """The long-item role shape through the scheduler's OWN choice (no override): one object of N_t = 20,000 on a grid of
+    seven tiles is split by observations into items of >= 48 stages (config 2's launch configuration on a smaller grid);
+    the last split of every tile to arrive finishes the tile in-kernel.  Full grid against the oracle, N_f % 4 in {0, 3, 2}."""
+    w = make_config(2, dtype="f32", n_t=20_000, n_freq=n_freq)
     P_ref = oracle_full(oracle, w)
     P, best, info = gpu_full(lsp, w, fast_math=fast)
     assert info["kernel"] == "tensor" and info["tensor_shape"] == 2 and info["n_split"] > 1
