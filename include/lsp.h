@@ -144,8 +144,10 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj,
  *   d_sigma      DEVICE, offsets[n_obj] elements of the plan's dtype, all > 0 (1-sigma errors of y).
  *   d_out_power  DEVICE, n_obj * n_freq elements, or NULL when only the best period is wanted.
  *   d_best_*     DEVICE, n_obj elements each: all three or none.
- * Asynchronous on cuda_stream.  Runs the standard contraction kernels three times (sums of w (y - ybar) e^{i theta},
- * w e^{i theta} and w e^{2 i theta}) and one combine kernel: about 3x the cost of lsp_periodogram_batched.
+ * Asynchronous on cuda_stream.  Runs the standard contraction kernels twice in their partial-sum form -- pass 1: sums of
+ * w (y - ybar) e^{i theta} and, in the doubled-angle slot, w e^{2 i theta}; pass 2: sums of w e^{i theta} (the tensor-core
+ * path skips the doubled-angle contraction there) -- and one combine kernel: about 2x the cost of lsp_periodogram_batched
+ * on the FMA-pipe kernels, ~1.5x on the tensor-core path (the paper's own implementation: 2.06-2.14x).
  * kernel = AUTO selects as lsp_periodogram_batched does, except that it falls back from the tensor-core kernel to the FMA-pipe
  * one when the batch's operand table would exceed the plan's budget (LSP_ERR_UNSUPPORTED if kernel = TENSOR was forced).
  * Other errors as lsp_periodogram_batched.

@@ -226,7 +226,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
 template <typename T, bool FAST>
 cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, int64_t n_obj_launch, const int64_t* d_off,
                         const void* d_t, const void* d_y, const ObjStats* stats, void* out, Best* partials,
-                        void* sums, cudaStream_t st)
+                        void* sums, cudaStream_t st, const void* wgt = nullptr)
 {
     using V4 = typename Vec4<T>::type;
     const int64_t grid = n_obj_launch * s.n_tiles * s.n_split;
@@ -256,10 +256,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
             return cudaErrorInvalidValue;      // rejected at plan creation
         }
     } else if (s.kernel == LSP_KERNEL_FACTORED) {
-        auto kern = lsp_factored_ws_kernel<T, FAST>;
-        cudaError_t e = optin_smem(p, kern, ws_smem_bytes<T>());
-        if (e != cudaSuccess) return e;
-        e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
+        cudaError_t e = cudaMemsetAsync(p->counter.ptr, 0, sizeof(unsigned long long), st);
         if (e != cudaSuccess) return e;
         const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
         using V2 = typename FactoredCfg<T>::V2;
@@ -267,15 +264,23 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
         const V2* tabV = (const V2*)p->ws_table.ptr;
         const V2* tabB1 = tabV + rows * 8;
         const V2* tabB2 = tabB1 + rows * FactoredCfg<T>::NL;
-        kern<<<ctas, kWsThreads, ws_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
-                                                          (V4*)sums, n_obj_launch, (long long)grid,
-                                                          (unsigned long long*)p->counter.ptr, tabV, tabB1, tabB2);
-    } else if (s.direct_r == 4) {
-        lsp_direct_kernel<T, FAST, 4><<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y,
-                                                                                 stats, (T*)out, partials, (V4*)sums, n_obj_launch);
+        auto go = [&](auto kern) -> cudaError_t {
+            const cudaError_t ea = optin_smem(p, kern, ws_smem_bytes<T>());
+            if (ea != cudaSuccess) return ea;
+            kern<<<ctas, kWsThreads, ws_smem_bytes<T>(), st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
+                                                              (V4*)sums, n_obj_launch, (long long)grid,
+                                                              (unsigned long long*)p->counter.ptr, tabV, tabB1, tabB2, (const T*)wgt);
+            return cudaSuccess;
+        };
+        e = wgt ? go(lsp_factored_ws_kernel<T, FAST, true>) : go(lsp_factored_ws_kernel<T, FAST, false>);
+        if (e != cudaSuccess) return e;
     } else {
-        lsp_direct_kernel<T, FAST, 1><<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y,
-                                                                                 stats, (T*)out, partials, (V4*)sums, n_obj_launch);
+        auto go = [&](auto kern) {
+            kern<<<(unsigned)grid, kDirectThreads, 0, st>>>(gp, d_off, (const T*)d_t, (const T*)d_y, stats, (T*)out, partials,
+                                                            (V4*)sums, n_obj_launch, (const T*)wgt);
+        };
+        if (s.direct_r == 4) { if (wgt) go(lsp_direct_kernel<T, FAST, 4, true>); else go(lsp_direct_kernel<T, FAST, 4, false>); }
+        else                 { if (wgt) go(lsp_direct_kernel<T, FAST, 1, true>); else go(lsp_direct_kernel<T, FAST, 1, false>); }
     }
     return cudaGetLastError();
 }
@@ -284,8 +289,9 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 // `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed by the launch-local object.
 struct RangeOpts {
     void* ext_sums = nullptr;     // write partial sums there and stop (generalised mode)
-    const void* wgt = nullptr;    // generalised mode: per-observation weights carried by the W slot (sum w e^{2 i theta})
-    int z_only = 0;               // generalised mode: only the Z slot is wanted (tensor path skips the W contraction)
+    const void* wgt = nullptr;    // generalised mode, pass 1: per-observation weights carried by the W slot (sum w e^{2 i theta})
+    int second_pass = 0;          // generalised mode, pass 2 (Z slot = sum w e^{i theta}): the tensor path reuses pass 1's table
+                                  // and statistics (its aux blocks hold w), takes w as the Z operand and skips the W contraction
 };
 lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
                      const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
@@ -299,7 +305,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
     if (tensor) {
         s.tp.fixup = fixup ? 1 : 0;
         s.tp.weighted = opt.wgt ? 1 : 0;
-        s.tp.z_only = opt.z_only;
+        s.tp.z_only = s.tp.y_is_w = opt.second_pass;
         // pre-pass of the tensor path, ONE launch: the B-operand table (once per object, shared by all of its frequency tiles
         // and observation splits; each stage carries the aux block the generators read) and the per-object statistics
         const int64_t kb_bound = obs_bound / kTcKB + n_obj_launch;
@@ -313,7 +319,9 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         gq.obj_base = (int)obj_base;
         const int64_t pre_grid = kb_bound + n_obj_launch;
         if (pre_grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
-        if (c.fast_math)
+        if (opt.second_pass) {
+            // table and statistics of pass 1 (same objects, same grid) are still in place
+        } else if (c.fast_math)
             lsp_tensor_prepass_kernel<true><<<(unsigned)pre_grid, kTcPreThreads, 0, st>>>(
                 gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
                 (int)n_obj_launch, (long long)kb_bound, g.center, g.normalize, (unsigned char*)p->tc_table.ptr);
@@ -322,7 +330,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
                 gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
                 (int)n_obj_launch, (long long)kb_bound, g.center, g.normalize, (unsigned char*)p->tc_table.ptr);
         LSP_CUDA(p, cudaGetLastError());
-        ++p->n_launches;
+        if (!opt.second_pass) ++p->n_launches;
     }
     GridParams gp;
     gp.f_min = g.f_min;
@@ -376,10 +384,10 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
     void* main_out = sums ? nullptr : out;             // kernels write partial sums instead of powers iff `sums` is set
     Best* main_partials = sums ? nullptr : partials;
     if (c.dtype == LSP_F32) {
-        e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st)
-                        : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st);
+        e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt)
+                        : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt);
     } else {
-        e = launch_main<double, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st);
+        e = launch_main<double, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt);
     }
     if (e != cudaSuccess) return fail(p, LSP_ERR_CUDA, "periodogram kernel launch: %s", cudaGetErrorString(e));
     ++p->n_launches;
@@ -788,8 +796,8 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     }
     if (total_obs > 0 && (!d_t || !d_y || !d_sigma)) return fail(p, LSP_ERR_INVALID_ARG, "d_t / d_y / d_sigma is NULL");
 
-    // The three passes run the standard kernels on derived inputs: y is already weighted and centred (center / normalize off),
-    // pass C runs on the doubled grid.  Each pass gets its grid by value; the plan's configuration is never modified.
+    // Two passes of the standard kernels in their partial-sum form on derived inputs (lsp_gls.cuh): y is already weighted and
+    // centred (center / normalize off).  The plan's configuration is never modified.
     const lsp_config& c = p->cfg;
     const size_t es = elem_size(c);
     lsp_status e;
@@ -814,23 +822,24 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     }
     p->kernel_used = s.kernel;
     p->n_split = s.n_split;
-    p->n_pairs = 3 * total_obs * c.n_freq;
-    // objects per round so that the three sums buffers stay within ~12 GB
-    const size_t per_obj = (size_t)3 * s.n_split * c.n_freq * 4 * es;
+    p->n_pairs = 2 * total_obs * c.n_freq;
+    const GridSpec g{c.f_min, c.f_max, 0, 0};
+    if ((e = build_ws_table(p, s, g, d_t, total_obs, st)) != LSP_OK) return e;      // FMA-pipe path: one table for both passes
+    // objects per round so that the two sums buffers stay within ~12 GB
+    const size_t per_obj = (size_t)2 * s.n_split * c.n_freq * 4 * es;
     const int64_t objs_per_round = std::max<int64_t>(1, (int64_t)(((size_t)12 << 30) / per_obj));
     const size_t row_bytes = (size_t)c.n_freq * es;
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
     for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_round) {
         const int64_t no = std::min(objs_per_round, n_obj - o0);
         const size_t pass_bytes = (size_t)s.n_split * no * c.n_freq * 4 * es;
-        if ((e = ensure(p, p->gls_sums, 3 * pass_bytes)) != LSP_OK) return e;
+        if ((e = ensure(p, p->gls_sums, 2 * pass_bytes)) != LSP_OK) return e;
         int n_parts = 0;
-        for (int pass = 0; pass < 3; ++pass) {
-            const double fs = pass == 2 ? 2.0 : 1.0;
-            const GridSpec g{c.f_min * fs, c.f_max * fs, 0, 0};
-            if ((e = build_ws_table(p, s, g, d_t, total_obs, st)) != LSP_OK) return e;
+        for (int pass = 0; pass < 2; ++pass) {
             RangeOpts ro;
             ro.ext_sums = (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes;
+            ro.wgt = pass == 0 ? xb : nullptr;
+            ro.second_pass = pass;
             e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st, ro);
             if (e != LSP_OK) return e;
         }
@@ -848,11 +857,11 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
         if (c.dtype == LSP_F32) {
             const float4* sa = (const float4*)p->gls_sums.ptr;
             lsp_gls_combine_kernel<float><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, (const double*)p->gls_yy.ptr, sa,
-                sa + pass_bytes / sizeof(float4), sa + 2 * (pass_bytes / sizeof(float4)), (float*)out, partials, n_cparts, no);
+                sa + pass_bytes / sizeof(float4), (float*)out, partials, n_cparts, no);
         } else {
             const double4* sa = (const double4*)p->gls_sums.ptr;
             lsp_gls_combine_kernel<double><<<(unsigned)grid, kCombineThreads, 0, st>>>(gp, (const double*)p->gls_yy.ptr, sa,
-                sa + pass_bytes / sizeof(double4), sa + 2 * (pass_bytes / sizeof(double4)), (double*)out, partials, n_cparts, no);
+                sa + pass_bytes / sizeof(double4), (double*)out, partials, n_cparts, no);
         }
         LSP_CUDA(p, cudaGetLastError());
         ++p->n_launches;

@@ -68,17 +68,20 @@ __device__ __forceinline__ WorkItem decode_item(const GridParams& gp)
     return w;
 }
 
-template <typename T, bool FAST, int R>
+// WGT (generalised mode only, partial-sum output): the doubled-angle sums carry the weights, c2 + i s2 = sum w e^{2 i theta}.
+template <typename T, bool FAST, int R, bool WGT = false>
 __global__ void __launch_bounds__(kDirectThreads)
 lsp_direct_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
                   const T* __restrict__ y, const ObjStats* __restrict__ stats,
                   T* __restrict__ out_power, Best* __restrict__ partials,
-                  typename Vec4<T>::type* __restrict__ sums, int64_t n_obj_launch)
+                  typename Vec4<T>::type* __restrict__ sums, int64_t n_obj_launch, const T* __restrict__ wgt = nullptr)
 {
     constexpr int TPB = kDirectThreads;
     constexpr int JC = 512;                       // observations staged per pass (tile = block)
     __shared__ T st[JC];
     __shared__ T sy[JC];
+    __shared__ T sw[WGT ? JC : 1];
+    T w_sum = T(0);
     __shared__ Best sbest[TPB / 32];
 
     const WorkItem wi = decode_item(gp);
@@ -105,11 +108,14 @@ lsp_direct_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* _
         for (int i = tid; i < cnt; i += TPB) {                 // step 2: coalesced staging
             st[i] = t[lo + jb + i];
             sy[i] = y[lo + jb + i] - mean;
+            if (WGT) sw[i] = wgt[lo + jb + i];
         }
         __syncthreads();
 #pragma unroll 4
         for (int j = 0; j < cnt; ++j) {                        // step 4: the per-pair hot loop
             const T tj = st[j], yj = sy[j];
+            const T wj = WGT ? sw[j] : T(1);
+            if (WGT) w_sum += wj;
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 T s, c;
@@ -117,13 +123,19 @@ lsp_direct_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* _
                 sincos_cycles<FAST>(ph, &s, &c);
                 xc[r] = fma(yj, c, xc[r]);
                 xs[r] = fma(yj, s, xs[r]);
-                cc[r] = fma(c, c, cc[r]);
-                cs[r] = fma(c, s, cs[r]);
+                if (WGT) {
+                    const T wc = wj * c;
+                    cc[r] = fma(wc, c, cc[r]);
+                    cs[r] = fma(wc, s, cs[r]);
+                } else {
+                    cc[r] = fma(c, c, cc[r]);
+                    cs[r] = fma(c, s, cs[r]);
+                }
             }
         }
     }
 
-    const T n_part = (T)(j1 - j0);
+    const T n_part = WGT ? w_sum : (T)(j1 - j0);   // sum of the weights of this item's observations
     Best mine;
     mine.p = -1.0;
     mine.k = INT64_MAX;

@@ -54,8 +54,8 @@ struct WsMeta {          // one per ring stage, written by producer thread 0
     int pad;
 };
 
-// producer scratch per buffer (complex elements): u [JC][8], v [JC][8], then JC reals (y) = JC / 2 complex slots
-template <typename T> __host__ __device__ constexpr int ws_scratch_elems() { return WsCfg<T>::JC * 16 + WsCfg<T>::JC / 2; }
+// producer scratch per buffer (complex elements): u [JC][8], v [JC][8], then JC reals (y) and JC reals (w) = JC complex slots
+template <typename T> __host__ __device__ constexpr int ws_scratch_elems() { return WsCfg<T>::JC * 16 + WsCfg<T>::JC; }
 template <typename T> constexpr size_t ws_smem_bytes()
 {
     return (size_t)WsCfg<T>::STAGES * WsCfg<T>::STAGE_ELEMS * 2 * sizeof(T)      // operand ring
@@ -192,7 +192,8 @@ __device__ __forceinline__ void ws_bulk_g2s(void* smem_dst, const void* gmem_src
                  ::"r"(smem_u32(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <typename T, bool FAST>
+// WGT (generalised mode only): the W operands carry the weights, a2 = w e^{2 i alpha}, so W(k) = sum w e^{2 i theta}.
+template <typename T, bool FAST, bool WGT = false>
 __global__ void __launch_bounds__(kWsThreads, 1)
 lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const T* __restrict__ t,
                        const T* __restrict__ y, const ObjStats* __restrict__ stats,
@@ -200,7 +201,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                        typename Vec4<T>::type* __restrict__ sums, int64_t n_obj_launch,
                        long long total_items, unsigned long long* __restrict__ work_counter,
                        const typename FactoredCfg<T>::V2* __restrict__ tabV, const typename FactoredCfg<T>::V2* __restrict__ tabB1,
-                       const typename FactoredCfg<T>::V2* __restrict__ tabB2)
+                       const typename FactoredCfg<T>::V2* __restrict__ tabB2, const T* __restrict__ wgt = nullptr)
 {
     using C = FactoredCfg<T>;
     using V2 = typename C::V2;
@@ -266,7 +267,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             int64_t jb = w.j0;
             do {      // at least one chunk per item, so empty objects still reach the epilogue
                 // loads first, so their latency overlaps the phase-1 arithmetic and the wait for a free stage
-                T t1[NP], y1[NP];
+                T t1[NP], y1[NP], w1[NP];
                 V2 v1[NP];
 #pragma unroll
                 for (int h = 0; h < NP; ++h) {
@@ -274,12 +275,14 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                     const bool live1 = j < w.j1;
                     t1[h] = live1 ? t[w.lo + j] : T(0);
                     y1[h] = (live1 && p_q == 0) ? y[w.lo + j] - mean : T(0);
+                    w1[h] = (WGT && live1 && p_q == 0) ? wgt[w.lo + j] : T(0);
                     v1[h] = tabV[(w.lo + j) * 8 + p_q];                              // padded table: always in range, finite
                 }
                 // ---- phase 1: u of (p_q, p_j + 16 h) (zero beyond the item's range) and v into the scratch
                 V2* sU = scratch + (size_t)(c & 1) * SCR;                            // [JC][8]
                 V2* sV = sU + JC * 8;                                                // [JC][8]
                 T* sY = reinterpret_cast<T*>(sV + JC * 8);                           // [JC]
+                T* sW = sY + JC;                                                     // [JC] (WGT only)
 #pragma unroll
                 for (int h = 0; h < NP; ++h) {
                     const bool live1 = (jb + p_j + 16 * h) < w.j1;
@@ -291,6 +294,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                     sU[(p_j + 16 * h) * 8 + p_q] = u;
                     sV[(p_j + 16 * h) * 8 + p_q] = v1[h];
                     if (p_q == 0) sY[p_j + 16 * h] = y1[h];
+                    if (WGT && p_q == 0) sW[p_j + 16 * h] = w1[h];
                 }
                 named_bar_sync(1, kWsProducers);
                 const int s = c % S;
@@ -318,6 +322,11 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                     a1.y = yj * es;
                     a2.x = fma(ec, ec, -es * es);    // a2 = e^{2 i alpha}
                     a2.y = T(2) * ec * es;
+                    if (WGT) {                       // ... times w_j
+                        const T wj = sW[jj];
+                        a2.x *= wj;
+                        a2.y *= wj;
+                    }
                     sA1[jj * G + gen_pos_a] = a1;
                     sA2[jj * G + gen_pos_a] = a2;
                 }

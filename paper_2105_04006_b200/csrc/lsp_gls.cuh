@@ -7,13 +7,12 @@
 //     YC = sum w (y - ybar) cos,  YS = sum w (y - ybar) sin,  YY = sum w (y - ybar)^2,
 //     CC = 1/2 (1 + c2) - C^2,  SS = 1/2 (1 - c2) - S^2,  CS = 1/2 s2 - C S,
 //     C + i S = sum w e^{i theta},   c2 + i s2 = sum w e^{2 i theta}.
-// Every sum is a "Z slot" of the standard kernels -- sum_j x_j e^{2 pi i f' t_j} on a linear grid -- for a suitable (x, f'):
-//     pass A: x = w (y - ybar), f' = f      -> (YC, YS)
-//     pass B: x = w,            f' = f      -> (C, S)
-//     pass C: x = w,            f' = 2 f    -> (c2, s2)      (the doubled grid is linear too)
-// so the generalised mode runs the unmodified direct / factored / tensor kernels three times in their split-N_t form (partial
-// sums to global memory; any n_split) and combines here.  Cost 3x the standard periodogram (the paper's own implementation:
-// 2.06-2.14x, L419); a weighted W slot in the kernels would make it 2x.
+// The standard kernels evaluate two slots per frequency, Z = sum x e^{i theta} and W = sum e^{2 i theta}.  With the W slot
+// carrying the weights (the kernels' WGT variants: W = sum w e^{2 i theta}) two passes in their partial-sum form give all six sums:
+//     pass 1: x = w (y - ybar), W weighted   -> (YC, YS) and (c2, s2)
+//     pass 2: x = w                           -> (C, S)    (the tensor path skips the W contraction and reuses pass 1's table)
+// and lsp_gls_combine_kernel finishes.  Cost: 2x the standard periodogram on the FMA-pipe kernels, ~1.5x on the tensor path
+// (the paper's own implementation: 2.06-2.14x, L419).
 #pragma once
 #include "lsp_direct.cuh"
 
@@ -67,12 +66,12 @@ lsp_gls_prep_kernel(const int64_t* __restrict__ offsets, const T* __restrict__ y
     if (threadIdx.x == 0) yy[obj] = (n > 0) ? chi0 : 0.0;
 }
 
-// Combine the three passes' partial sums (fixed split order: deterministic) and evaluate P; same launch geometry and
+// Combine the two passes' partial sums (fixed split order: deterministic) and evaluate P; same launch geometry and
 // argmax partials as lsp_combine_kernel.
 template <typename T>
 __global__ void __launch_bounds__(kCombineThreads)
 lsp_gls_combine_kernel(GridParams gp, const double* __restrict__ yy, const typename Vec4<T>::type* __restrict__ sa,
-                       const typename Vec4<T>::type* __restrict__ sb, const typename Vec4<T>::type* __restrict__ sc,
+                       const typename Vec4<T>::type* __restrict__ sb,
                        T* __restrict__ out_power, Best* __restrict__ partials, int n_parts, int64_t n_obj_launch)
 {
     __shared__ Best sbest[kCombineThreads / 32];
@@ -90,10 +89,10 @@ lsp_gls_combine_kernel(GridParams gp, const double* __restrict__ yy, const typen
         double YC = 0, YS = 0, C = 0, S = 0, c2 = 0, s2 = 0;
         for (int s = 0; s < gp.n_split; ++s) {
             const int64_t at = ((int64_t)s * n_obj_launch + obj_local) * gp.n_freq + k;
-            const typename Vec4<T>::type a = sa[at], b = sb[at], c = sc[at];
+            const typename Vec4<T>::type a = sa[at], b = sb[at];
             YC += (double)a.x; YS += (double)a.y;
+            c2 += (double)a.z; s2 += (double)a.w;
             C += (double)b.x;  S += (double)b.y;
-            c2 += (double)c.x; s2 += (double)c.y;
         }
         const double CC = 0.5 * (1.0 + c2) - C * C, SS = 0.5 * (1.0 - c2) - S * S, CS = 0.5 * s2 - C * S;
         const double D = CC * SS - CS * CS;

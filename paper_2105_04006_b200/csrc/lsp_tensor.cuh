@@ -95,6 +95,7 @@ struct TensorParams {
                         // 0 = partial sums per grid frequency (generalised mode)
     int weighted;       // generalised mode: the W operand carries the weights w_j (aux.w) instead of 1
     int z_only;         // generalised mode, second pass: only the Z contraction is wanted
+    int y_is_w;         // generalised mode, second pass: the Z operand carries the weights (aux.w, scale wscale) instead of y
 };
 
 // Per-object pre-pass results of the tensor path.
@@ -758,6 +759,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             float4* nat = (sums && tp.fixup) ? sums + (((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_tiles + w.tile) * tile_elems +
                                                    32 * q + lane : nullptr;
             float4* stile = (sums && !tp.fixup) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
+            const float zinv = tp.y_is_w ? ob.winv : ob.zinv;
             auto chunk_sums = [&](int ch) {
                 const int m0 = ch * 16;
                 float zr[16], zi[16], wr[16], wi[16];
@@ -788,7 +790,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 for (int i = 0; i < 16; ++i) {
                     const float p0 = __shfl_xor_sync(0xffffffffu, zr[i], 16), p1 = __shfl_xor_sync(0xffffffffu, zi[i], 16);
                     const float q0 = __shfl_xor_sync(0xffffffffu, wr[i], 16), q1 = __shfl_xor_sync(0xffffffffu, wi[i], 16);
-                    const float za = (zr[i] - p1) * ob.zinv, zb = (zi[i] + p0) * ob.zinv;
+                    const float za = (zr[i] - p1) * zinv, zb = (zi[i] + p0) * zinv;
                     const float wa = (wr[i] - q1) * ob.winv, wb = (wi[i] + q0) * ob.winv;
                     if (nat) {
                         nat[(int64_t)(m0 + i) * 128] = make_float4(za, zb, wa, wb);
@@ -874,8 +876,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             f_hi = (float)fd;
             f_lo = (float)(fd - (double)f_hi);
             const TensorObj ob = objs[w.obj_local];
-            mean = (float)ob.mean;
-            ysc = ob.yscale * (1.0f / kTcPhasorScale);
+            mean = tp.y_is_w ? 0.f : (float)ob.mean;
+            ysc = (tp.y_is_w ? ob.wscale : ob.yscale) * (1.0f / kTcPhasorScale);
             wsc = ob.wscale * (1.0f / kTcUnitScale);
             return w.kb1 - w.kb0;
         };
@@ -908,7 +910,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 su[pos1] = cs * kTcPhasorScale;
                 su[pos1 + 2] = sn * kTcPhasorScale;
                 if (g0p == 0) {
-                    const float ys = (lds32(aux + 64 + 4 * jp) - mean) * ysc;
+                    const float ys = (lds32(aux + (tp.y_is_w ? 128 : 64) + 4 * jp) - mean) * ysc;
                     su[8 * kTcVRow + jp] = ys;                                  // "Re a" rows: y p
                     su[8 * kTcVRow + 16 + jp] = ys * 0.70710678118654752f;      // "Im a" rows: y (p + q) / sqrt 2
                 }
