@@ -36,16 +36,24 @@ constexpr int kWsThreads = kWsConsumers + kWsProducers;
 #ifndef LSP_WS_STAGES_F64
 #define LSP_WS_STAGES_F64 2
 #endif
+// An a-operand row (one observation, G = 64 groups) is stored in two halves of 32 elements; inside the second half element i
+// sits at i ^ GSKEW (a 64-byte XOR swizzle) so that the producers' stores -- lanes alternate between the halves
+// (operand_pos) -- fall into different banks: without it every quarter-warp store was a 2-way conflict (r01: 87.7 M
+// conflicts per FP64 launch).  No padding: the FP64 ring already fills shared memory.
 template <typename T> struct WsCfg;
 template <> struct WsCfg<float> {
     static constexpr int JC = LSP_WS_JC_F32;         // observations per ring stage
     static constexpr int STAGES = LSP_WS_STAGES_F32;
-    static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<float>::NL);   // complex elements per stage
+    static constexpr int GSKEW = 8;                  // 8 float2 = 64 bytes
+    static constexpr int GP = kFacGroups;            // a-row length
+    static constexpr int STAGE_ELEMS = JC * (2 * GP + 2 * FactoredCfg<float>::NL);   // complex elements per stage
 };
 template <> struct WsCfg<double> {
     static constexpr int JC = LSP_WS_JC_F64;
     static constexpr int STAGES = LSP_WS_STAGES_F64;
-    static constexpr int STAGE_ELEMS = JC * (2 * kFacGroups + 2 * FactoredCfg<double>::NL);
+    static constexpr int GSKEW = 4;                  // 4 double2 = 64 bytes
+    static constexpr int GP = kFacGroups;
+    static constexpr int STAGE_ELEMS = JC * (2 * GP + 2 * FactoredCfg<double>::NL);
 };
 
 struct WsMeta {          // one per ring stage, written by producer thread 0
@@ -206,9 +214,9 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     using C = FactoredCfg<T>;
     using V2 = typename C::V2;
     constexpr int G = kFacGroups, TH = C::TH, TM = C::TM, NL = C::NL, L = 2 * NL, TILE = C::TILE, EPC = C::EPC;
-    constexpr int JC = WsCfg<T>::JC, S = WsCfg<T>::STAGES;
+    constexpr int JC = WsCfg<T>::JC, S = WsCfg<T>::STAGES, GP = WsCfg<T>::GP, GSKEW = WsCfg<T>::GSKEW;
     constexpr int NGI = G / TH, NMI = NL / TM;
-    constexpr int STAGE = WsCfg<T>::STAGE_ELEMS;             // V2 elements per stage: [JC][G] a, [JC][G] a2, [JC][NL] b, [JC][NL] b2
+    constexpr int STAGE = WsCfg<T>::STAGE_ELEMS;             // V2 elements per stage: [JC][GP] a, [JC][GP] a2, [JC][NL] b, [JC][NL] b2
     static_assert(NGI * NMI == kWsConsumers / 2, "Z and W halves each cover the G x NL tile once");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -243,7 +251,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
         // stage are two bulk copies (TMA) from the table straight into the ring, completing on the stage's full barrier.
         const int ptid = tid - kWsConsumers;
         const int gen_g = ptid & (G - 1);
-        const int gen_pos_a = operand_pos<TH, NGI, EPC>(gen_g);
+        const int gen_pos_raw = operand_pos<TH, NGI, EPC>(gen_g);
+        const int gen_pos_a = gen_pos_raw ^ ((gen_pos_raw >> 5) * GSKEW);       // second half of the row: 64-byte XOR swizzle
         const int p_q = ptid & 7, p_j = ptid >> 3;                                 // phase 1: phasor index, observation
         static_assert(JC % 16 == 0 && kWsProducers == 128 && G == 64, "producer work split");
         constexpr int NP = JC / 16;                                                // u phasors per thread per chunk
@@ -300,8 +309,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 const int s = c % S;
                 mbar_wait_sleep(&empty[s], ((c / S) & 1) ^ 1, 100);
                 V2* sA1 = ring + (size_t)s * STAGE;
-                V2* sA2 = sA1 + JC * G;
-                V2* sB1 = sA2 + JC * G;
+                V2* sA2 = sA1 + JC * GP;
+                V2* sB1 = sA2 + JC * GP;
                 V2* sB2 = sB1 + JC * NL;
                 if (ptid == 0) {          // b, b2 rows of observations [jb, jb + JC) of this object: table -> ring (async proxy)
                     ws_mbar_arrive_expect_tx(&full[s], 2 * B_BYTES);
@@ -327,8 +336,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                         a2.x *= wj;
                         a2.y *= wj;
                     }
-                    sA1[jj * G + gen_pos_a] = a1;
-                    sA2[jj * G + gen_pos_a] = a2;
+                    sA1[jj * GP + gen_pos_a] = a1;
+                    sA2[jj * GP + gen_pos_a] = a2;
                 }
                 jb += JC;
                 if (ptid == 0) { meta[s].item = item; meta[s].last = (jb >= w.j1) ? 1 : 0; }
@@ -351,8 +360,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             mi = ((lane >> 1) & 1) | (((lane >> 3) & 1) << 1);
             gi = (lane & 1) | (((lane >> 2) & 1) << 1) | (((lane >> 4) & 1) << 2) | (wq << 3);
         }
-        const int offA = is_w ? JC * G : 0;
-        const int offB = 2 * JC * G + (is_w ? JC * NL : 0);
+        const int offA = is_w ? JC * GP : 0;
+        const int offB = 2 * JC * GP + (is_w ? JC * NL : 0);
 
         V2 acc_r[TH][TM], acc_i[TH][TM];        // (Srr, Sri) and (Sir, Sii) of this thread's (group, m) pairs
 #pragma unroll
@@ -377,7 +386,8 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 if constexpr (EPC == 2) {           // one LDS.128 = two complex operands
 #pragma unroll
                     for (int q = 0; q < TH / 2; ++q) {
-                        const float4 ch = reinterpret_cast<const float4*>(A + jj * G)[q * NGI + gi];
+                        static_assert(TH / 2 * NGI * 2 == G && NGI * 2 == 32, "one float4 index step of NGI = one 32-element half row");
+                        const float4 ch = reinterpret_cast<const float4*>(A + jj * GP)[q * NGI + (gi ^ (q * (GSKEW / 2)))];
                         av[2 * q].x = ch.x; av[2 * q].y = ch.y; av[2 * q + 1].x = ch.z; av[2 * q + 1].y = ch.w;
                     }
 #pragma unroll
@@ -386,8 +396,9 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                         bv[2 * q].x = ch.x; bv[2 * q].y = ch.y; bv[2 * q + 1].x = ch.z; bv[2 * q + 1].y = ch.w;
                     }
                 } else {                            // one LDS.128 = one complex operand
+                    static_assert(EPC == 2 || NGI == 32, "one index step of NGI = one 32-element half row");
 #pragma unroll
-                    for (int a = 0; a < TH; ++a) av[a] = A[jj * G + a * NGI + gi];
+                    for (int a = 0; a < TH; ++a) av[a] = A[jj * GP + a * NGI + (gi ^ (a * GSKEW))];
 #pragma unroll
                     for (int cc = 0; cc < TM; ++cc) bv[cc] = B[jj * NL + cc * NMI + mi];
                 }
