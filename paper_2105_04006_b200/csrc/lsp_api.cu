@@ -131,6 +131,24 @@ cudaError_t optin_smem(lsp_plan* p, K kern, size_t bytes)
     return err;
 }
 
+// Launch with programmatic stream serialisation: the kernel may start while its predecessor on the stream drains; it must
+// execute griddepcontrol.wait (pdl_wait in lsp_tensor.cuh) before reading what the predecessor wrote.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // The grid and per-object conventions one launch sequence runs with.  The standard calls use the plan's own; the generalised
 // mode passes derived ones (doubled grid, no centring) BY VALUE -- the plan's public configuration is never scratch space.
 struct GridSpec {
@@ -239,9 +257,8 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
             auto go = [&](auto kern, int threads) -> cudaError_t {
                 const cudaError_t ea = optin_smem(p, kern, smem);
                 if (ea != cudaSuccess) return ea;
-                kern<<<ctas, threads, smem, st>>>(gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr, (const unsigned char*)p->tc_table.ptr,
-                                                  (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid);
-                return cudaSuccess;
+                return launch_pdl(kern, ctas, (unsigned)threads, smem, st, gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
+                                  (const unsigned char*)p->tc_table.ptr, (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid);
             };
             p->tensor_shape = s.tp.long_items ? 2 : 1;
             cudaError_t e;
@@ -397,8 +414,8 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         // tensor path: add the splits' partial slots in split order and finish the tiles (steps 5, 6, 6')
         const int64_t grid = n_obj_launch * (int64_t)s.n_tiles * kTcFixParts;
         if (grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
-        lsp_tensor_fix_kernel<float><<<(unsigned)grid, kTcFixThreads, 0, st>>>(gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
-                                                                              (const float4*)sums, (float*)out, partials, n_obj_launch);
+        LSP_CUDA(p, launch_pdl(lsp_tensor_fix_kernel<float>, (unsigned)grid, (unsigned)kTcFixThreads, 0, st, gp, s.tp, d_off,
+                               (const TensorObj*)p->tc_objs.ptr, (const float4*)sums, (float*)out, partials, n_obj_launch));
         LSP_CUDA(p, cudaGetLastError());
         ++p->n_launches;
     }

@@ -117,6 +117,13 @@ __device__ __forceinline__ int64_t tc_kb_off(const int64_t* __restrict__ offsets
     return (offsets[obj_base + o] - offsets[obj_base]) / kTcKB + o;
 }
 
+// Programmatic dependent launch (the tensor path's launches are chained: pre-pass -> main -> fix): a kernel lets its dependent
+// start launching early (`pdl_trigger`), the dependent waits for the prerequisite grid to have completed and flushed its
+// memory before touching its results (`pdl_wait`).  Hides the launch latency between the launches; both are no-ops when the
+// kernel was launched without the attribute.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ void split_half2(float x0, float x1, __half2* hi, __half2* lo)
 {
     const __half2 h = __floats2half2_rn(x0, x1);
@@ -138,6 +145,7 @@ lsp_tensor_prepass_kernel(GridParams gp, TensorParams tp, const int64_t* __restr
                           long long n_table_blocks, int center, int normalize, unsigned char* __restrict__ table)
 {
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    pdl_trigger();
     if ((long long)blockIdx.x >= n_table_blocks) {
         // ---------------- statistics of object o ----------------
         __shared__ double red[4][4];
@@ -406,6 +414,7 @@ lsp_tensor_fix_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict_
                       const float4* __restrict__ sums, T* __restrict__ out_power, Best* __restrict__ partials, int64_t n_obj_launch)
 {
     __shared__ Best sbest[kTcFixThreads / 32];
+    pdl_wait();            // the main kernel's partial slots are complete and visible
     const int part = (int)(blockIdx.x % kTcFixParts);
     const long long r0 = blockIdx.x / kTcFixParts;
     const int tile = (int)(r0 % gp.n_tiles);
@@ -552,6 +561,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     __syncthreads();
     tc_fence_after();
     const unsigned tmem = tmem_base_s;
+    pdl_trigger();
+    pdl_wait();            // the pre-pass's table and statistics are complete and visible from here on
 
     if (warp < 4) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kCtrlRegs));
     if (warp == 0) {
