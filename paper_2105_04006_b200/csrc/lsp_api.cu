@@ -244,7 +244,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
 template <typename T, bool FAST>
 cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, int64_t n_obj_launch, const int64_t* d_off,
                         const void* d_t, const void* d_y, const ObjStats* stats, void* out, Best* partials,
-                        void* sums, cudaStream_t st, const void* wgt = nullptr)
+                        void* sums, cudaStream_t st, const void* wgt = nullptr, const double* gls_yy = nullptr)
 {
     using V4 = typename Vec4<T>::type;
     const int64_t grid = n_obj_launch * s.n_tiles * s.n_split;
@@ -258,16 +258,20 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
                 const cudaError_t ea = optin_smem(p, kern, smem);
                 if (ea != cudaSuccess) return ea;
                 return launch_pdl(kern, ctas, (unsigned)threads, smem, st, gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
-                                  (const unsigned char*)p->tc_table.ptr, (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid);
+                                  (const unsigned char*)p->tc_table.ptr, (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid,
+                                  gls_yy);
             };
             p->tensor_shape = s.tp.long_items ? 2 : 1;
             cudaError_t e;
-            if (s.tp.weighted)           // generalised mode: the W slot carries the weights
-                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, true>, TcRoles<4, 4>::kThreads)
-                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, true>, TcRoles<8, 3>::kThreads);
+            if (s.tp.weighted && s.tp.gls == 2)      // generalised mode, weighted W slot + ZK09's epilogue fused
+                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 2>, TcRoles<4, 4>::kThreads)
+                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 2>, TcRoles<8, 3>::kThreads);
+            else if (s.tp.weighted)                  // generalised mode: the W slot carries the weights
+                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 1>, TcRoles<4, 4>::kThreads)
+                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 1>, TcRoles<8, 3>::kThreads);
             else
-                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, false>, TcRoles<4, 4>::kThreads)
-                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, false>, TcRoles<8, 3>::kThreads);
+                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 0>, TcRoles<4, 4>::kThreads)
+                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 0>, TcRoles<8, 3>::kThreads);
             if (e != cudaSuccess) return e;
         } else {
             return cudaErrorInvalidValue;      // rejected at plan creation
@@ -306,9 +310,14 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
 // `out` (device, may be NULL) receives rows relative to obj_base; partials (may be NULL) is indexed by the launch-local object.
 struct RangeOpts {
     void* ext_sums = nullptr;     // write partial sums there and stop (generalised mode)
-    const void* wgt = nullptr;    // generalised mode, pass 1: per-observation weights carried by the W slot (sum w e^{2 i theta})
-    int second_pass = 0;          // generalised mode, pass 2 (Z slot = sum w e^{i theta}): the tensor path reuses pass 1's table
-                                  // and statistics (its aux blocks hold w), takes w as the Z operand and skips the W contraction
+    const void* wgt = nullptr;    // generalised mode: per-observation weights (W slot = sum w e^{2 i theta}; the tensor pre-pass
+                                  // stores them in the table's aux blocks)
+    int w_pass = 0;               // generalised mode, the pass whose Z slot is sum w e^{i theta}: the tensor path takes w from the aux
+                                  // blocks as the Z operand and skips the W contraction
+    int skip_prepass = 0;         // tensor path: table and statistics of the previous launch (same objects, same grid) are reused
+    int gls = 0;                  // tensor path, n_split = 1: 1 = the w pass writes (C, S) per element into ext_sums in the epilogue's
+                                  // own order; 2 = the weighted pass reads them from ext_sums and evaluates ZK09's power in its epilogue
+    const double* gls_yy = nullptr;   // chi0^2 per object (gls = 2)
 };
 lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64_t obj_base, int64_t n_obj_launch, int64_t obs_bound,
                      const int64_t* d_off, const void* d_t, const void* d_y, void* out, bool want_best, int* n_parts_out,
@@ -321,8 +330,9 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
     const bool fixup = tensor && s.n_split > 1 && !ext_sums;      // the tensor kernel finishes split tiles itself
     if (tensor) {
         s.tp.fixup = fixup ? 1 : 0;
-        s.tp.weighted = opt.wgt ? 1 : 0;
-        s.tp.z_only = s.tp.y_is_w = opt.second_pass;
+        s.tp.weighted = (opt.wgt && !opt.w_pass) ? 1 : 0;
+        s.tp.z_only = s.tp.y_is_w = opt.w_pass;
+        s.tp.gls = opt.gls;
         // pre-pass of the tensor path, ONE launch: the B-operand table (once per object, shared by all of its frequency tiles
         // and observation splits; each stage carries the aux block the generators read) and the per-object statistics
         const int64_t kb_bound = obs_bound / kTcKB + n_obj_launch;
@@ -336,8 +346,8 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         gq.obj_base = (int)obj_base;
         const int64_t pre_grid = kb_bound + n_obj_launch;
         if (pre_grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
-        if (opt.second_pass) {
-            // table and statistics of pass 1 (same objects, same grid) are still in place
+        if (opt.skip_prepass) {
+            // table and statistics of the previous launch (same objects, same grid) are still in place
         } else if (c.fast_math)
             lsp_tensor_prepass_kernel<true><<<(unsigned)pre_grid, kTcPreThreads, 0, st>>>(
                 gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
@@ -347,7 +357,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
                 gq, s.tp, d_off, (const float*)d_t, (const float*)d_y, (const float*)opt.wgt, (TensorObj*)p->tc_objs.ptr,
                 (int)n_obj_launch, (long long)kb_bound, g.center, g.normalize, (unsigned char*)p->tc_table.ptr);
         LSP_CUDA(p, cudaGetLastError());
-        if (!opt.second_pass) ++p->n_launches;
+        if (!opt.skip_prepass) ++p->n_launches;
     }
     GridParams gp;
     gp.f_min = g.f_min;
@@ -375,7 +385,8 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         sums = p->sums.ptr;
     }
     const bool combine = s.n_split > 1 && !ext_sums && !fixup;    // FMA-pipe / direct kernels: partial sums + lsp_combine_kernel
-    *n_parts_out = (combine || ext_sums) ? n_cparts : (fixup ? s.n_tiles * kTcFixParts : s.n_tiles);
+    const bool fused_gls = tensor && opt.gls == 2;                // powers and argmax partials come straight from the epilogue
+    *n_parts_out = fused_gls ? s.n_tiles : (combine || ext_sums) ? n_cparts : (fixup ? s.n_tiles * kTcFixParts : s.n_tiles);
     if (want_best) {     // partials are indexed by the launch-local object: each launch's finalize follows it in-stream
         lsp_status e = ensure(p, p->partials, (size_t)n_obj_launch * (size_t)*n_parts_out * sizeof(Best));
         if (e != LSP_OK) return e;
@@ -398,13 +409,15 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         LSP_CUDA(p, cudaEventRecord(ev0, st));
     }
     cudaError_t e;
-    void* main_out = sums ? nullptr : out;             // kernels write partial sums instead of powers iff `sums` is set
-    Best* main_partials = sums ? nullptr : partials;
+    void* main_out = (sums && !fused_gls) ? nullptr : out;       // kernels write partial sums instead of powers iff `sums` is set
+    Best* main_partials = (sums && !fused_gls) ? nullptr : partials;
     if (c.dtype == LSP_F32) {
-        e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt)
-                        : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt);
+        const void* kw = opt.w_pass ? nullptr : opt.wgt;         // the w pass runs the unweighted instantiations
+        e = c.fast_math ? launch_main<float, true>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, kw, opt.gls_yy)
+                        : launch_main<float, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, kw, opt.gls_yy);
     } else {
-        e = launch_main<double, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, opt.wgt);
+        const void* kw = opt.w_pass ? nullptr : opt.wgt;
+        e = launch_main<double, false>(p, s, gp, n_obj_launch, d_off, d_t, d_y, stats, main_out, main_partials, sums, st, kw);
     }
     if (e != cudaSuccess) return fail(p, LSP_ERR_CUDA, "periodogram kernel launch: %s", cudaGetErrorString(e));
     ++p->n_launches;
@@ -843,20 +856,43 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     const GridSpec g{c.f_min, c.f_max, 0, 0};
     if ((e = build_ws_table(p, s, g, d_t, total_obs, st)) != LSP_OK) return e;      // FMA-pipe path: one table for both passes
     // objects per round so that the two sums buffers stay within ~12 GB
-    const size_t per_obj = (size_t)2 * s.n_split * c.n_freq * 4 * es;
+    // Tensor path, n_split = 1: ZK09's epilogue is fused into the kernel's -- the w pass leaves (C, S) per element (8 bytes, in the
+    // epilogue's own order) and the weighted pass reads them back and writes powers / argmax partials itself; nothing else goes
+    // through memory.  Otherwise both passes leave partial sums per grid frequency and lsp_gls_combine_kernel finishes.
+    const bool fused = s.kernel == LSP_KERNEL_TENSOR && s.n_split == 1;
+    const size_t tile_elems = fused ? (size_t)((s.tp.nl + 15) / 16) * 16 * 128 : 0;
+    const size_t per_obj = fused ? (size_t)s.n_tiles * tile_elems * sizeof(float2) : (size_t)2 * s.n_split * c.n_freq * 4 * es;
     const int64_t objs_per_round = std::max<int64_t>(1, (int64_t)(((size_t)12 << 30) / per_obj));
     const size_t row_bytes = (size_t)c.n_freq * es;
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
     for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_round) {
         const int64_t no = std::min(objs_per_round, n_obj - o0);
+        int n_parts = 0;
+        if (fused) {
+            if ((e = ensure(p, p->gls_sums, (size_t)no * per_obj)) != LSP_OK) return e;
+            void* out = d_out_power ? (char*)d_out_power + (size_t)o0 * row_bytes : nullptr;
+            RangeOpts ro;
+            ro.ext_sums = p->gls_sums.ptr;
+            ro.wgt = xb;
+            ro.w_pass = 1;            // first the w pass (its launch also runs the pre-pass: y = w (y - ybar), aux w)
+            ro.gls = 1;
+            if ((e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, xa, nullptr, false, &n_parts, st, ro)) != LSP_OK) return e;
+            ro.w_pass = 0;
+            ro.skip_prepass = 1;
+            ro.gls = 2;
+            ro.gls_yy = (const double*)p->gls_yy.ptr;
+            if ((e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, xa, out, want_best, &n_parts, st, ro)) != LSP_OK) return e;
+            if (want_best && (e = run_finalize(p, o0, no, n_parts, d_offsets, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+            continue;
+        }
         const size_t pass_bytes = (size_t)s.n_split * no * c.n_freq * 4 * es;
         if ((e = ensure(p, p->gls_sums, 2 * pass_bytes)) != LSP_OK) return e;
-        int n_parts = 0;
         for (int pass = 0; pass < 2; ++pass) {
             RangeOpts ro;
             ro.ext_sums = (char*)p->gls_sums.ptr + (size_t)pass * pass_bytes;
-            ro.wgt = pass == 0 ? xb : nullptr;
-            ro.second_pass = pass;
+            ro.wgt = xb;
+            ro.w_pass = pass;
+            ro.skip_prepass = pass;   // tensor path: pass 2 reuses pass 1's table and statistics
             e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, pass == 0 ? xa : xb, nullptr, false, &n_parts, st, ro);
             if (e != LSP_OK) return e;
         }

@@ -96,7 +96,23 @@ struct TensorParams {
     int weighted;       // generalised mode: the W operand carries the weights w_j (aux.w) instead of 1
     int z_only;         // generalised mode, second pass: only the Z contraction is wanted
     int y_is_w;         // generalised mode, second pass: the Z operand carries the weights (aux.w, scale wscale) instead of y
+    int gls;            // generalised mode fused into the epilogue (n_split = 1): 1 = this launch writes (C, S) = sum w e^{i theta}
+                        // per element in the epilogue's own order (float2); 2 = this launch (weighted W) reads them back and
+                        // evaluates ZK09's power in place of step 5
 };
+
+// Generalised Lomb-Scargle power from the six weighted sums (Zechmeister & Kuerster 2009 Eq. 4-5; lsp_gls.cuh has the notation),
+// FP32 arithmetic for the fused epilogue: weights are normalised (sum w = 1), so CC, SS, CS are O(1).
+__device__ __forceinline__ float gls_power_f32(float YC, float YS, float C, float S, float c2, float s2, float inv_chi0)
+{
+    const float CC = fmaf(-C, C, 0.5f * (1.0f + c2)), SS = fmaf(-S, S, 0.5f * (1.0f - c2)), CS = fmaf(-C, S, 0.5f * s2);
+    const float D = fmaf(CC, SS, -CS * CS);
+    float p = 0.0f;
+    if (D > 1e-5f) p = (SS * YC * YC + CC * YS * YS - 2.0f * CS * YC * YS) / D;
+    else if (CC > 1e-5f) p = YC * YC / CC;                // aliased design matrix: the vanishing direction is dropped
+    else if (SS > 1e-5f) p = YS * YS / SS;
+    return p * inv_chi0;
+}
 
 // Per-object pre-pass results of the tensor path.
 struct TensorObj {
@@ -504,13 +520,16 @@ constexpr size_t tc_smem_bytes(int stages_b, int b_stage)
 // static shared memory of the kernel (generator scratch etc.), for the host's ring sizing
 template <int EW, int NG> constexpr int tc_static_smem() { return NG * 2 * (8 * kTcVRow + 32) * 4 + EW * 16 + 256; }
 
-template <typename T, bool FAST, int EW, int NG, bool WGT>
+// GM (generalised mode): 0 = standard; 1 = the W slot carries the weights (partial-sum output); 2 = 1 + ZK09's power fused into
+// the epilogue (n_split = 1).  A template parameter so that the standard kernel carries none of it.
+template <typename T, bool FAST, int EW, int NG, int GM>
 __global__ void __launch_bounds__((TcRoles<EW, NG>::kThreads), 1)
 lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
                   const unsigned char* __restrict__ table, T* __restrict__ out_power, Best* __restrict__ partials,
-                  float4* __restrict__ sums, int64_t n_obj_launch, long long total_items)
+                  float4* __restrict__ sums, int64_t n_obj_launch, long long total_items, const double* __restrict__ gls_yy)
 {
     using R = TcRoles<EW, NG>;
+    constexpr bool WGT = GM != 0, FUSED = GM == 2;
     constexpr int kEpiWarps = EW, kEpiThreads = R::kEpiThreads;
     constexpr int NOPS = FAST ? 2 : 4;
     constexpr int A_STAGE_COLS = NOPS * 8;                    // TMEM columns of one A stage
@@ -666,6 +685,14 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const TcItem w = tc_decode(gp, tp, item, offsets);
             const TensorObj ob = objs[w.obj_local];
             const bool have = w.kb1 > w.kb0;
+            if (FUSED) {
+                // generalised mode, fused: pull this warp's (C, S) lines of the tile into L2 while the item's MMAs still run
+                const float2* base = reinterpret_cast<const float2*>(sums) + (w.obj_local * gp.n_tiles + w.tile) * ((int64_t)n_chunks * 16 * 128) + 32 * q;
+                for (int ch = ch0; ch < ch1; ++ch) {
+                    const float2* ptr = base + (int64_t)(16 * ch + (lane >> 1)) * 128 + (lane & 1) * 16;      // 32 lines of 128 bytes per chunk
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr));
+                }
+            }
             if (have) {
                 mbar_wait_backoff(tmem_full, n_acc & 1, EW == 4 ? 400u : 100u);     // long items: the wait lasts a whole item
                 tc_fence_after();
@@ -679,11 +706,25 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             T* otile = out_power ? out_power + w.obj_local * (int64_t)gp.n_freq + w.K0 : nullptr;
             const unsigned ta = tmem + ((unsigned)(32 * q) << 16);
             bool released = false;
+            // generalised mode, fused (tp.gls == 2): this tile's (C, S) of the earlier launch, and 1 / chi0^2 of the object
+            const float2* gls_cs = FUSED ? reinterpret_cast<const float2*>(sums) +
+                                                              (w.obj_local * gp.n_tiles + w.tile) * ((int64_t)n_chunks * 16 * 128) + 32 * q + lane
+                                                        : nullptr;
+            float inv_chi0 = 0.f;
+            if (FUSED) {
+                const double c0 = gls_yy[w.obj];
+                inv_chi0 = c0 > 0.0 ? (float)(1.0 / c0) : 0.f;
+            }
             // one chunk = 16 accumulator columns of each of the four TMEM regions; RAG = the tile overhangs the grid
             auto chunk = [&](int ch, auto rag_tag) {
                 constexpr bool RAG = decltype(rag_tag)::value;
                 const int m0 = ch * 16;
                 float zr[16], zi[16], wr[16], wi[16];
+                float2 csv[FUSED ? 16 : 1];
+                if (FUSED) {                                      // the chunk's (C, S): all 16 loads in flight before anything waits
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) csv[i] = __ldcg(gls_cs + (int64_t)(m0 + i) * 128);
+                }
                 if (have) {
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
@@ -733,6 +774,15 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                             pw[e] = power_from_sums<float>(is_im ? zb[e] : za[e], is_im ? za[e] : zb[e], is_im ? wb[e] : wa[e],
                                                            is_im ? wa[e] : wb[e], n_hat, ob.pscale);
                     }
+                    if (FUSED) {                                  // generalised mode: ZK09's power instead (lsp_gls.cuh)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const float2 cs = csv[FUSED ? 4 * v4 + e : 0];                              // lane-oriented, like (za, zb)
+                            const float ya = za[e] * ob.zinv, yb = zb[e] * ob.zinv, ua = wa[e] * ob.winv, ub = wb[e] * ob.winv;
+                            pw[e] = gls_power_f32(is_im ? yb : ya, is_im ? ya : yb, is_im ? cs.y : cs.x, is_im ? cs.x : cs.y,
+                                                  is_im ? ub : ua, is_im ? ua : ub, inv_chi0);
+                        }
+                    }
                     if (partials) {
                         // up lanes meet their frequencies in ascending, down lanes in descending order: "lowest index wins
                         // ties" is "first wins" for the former and "last wins" for the latter
@@ -769,7 +819,9 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const int64_t tile_elems = (int64_t)n_chunks * 16 * 128;
             float4* nat = (sums && tp.fixup) ? sums + (((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_tiles + w.tile) * tile_elems +
                                                    32 * q + lane : nullptr;
-            float4* stile = (sums && !tp.fixup) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
+            float4* stile = (sums && !tp.fixup && !tp.gls) ? sums + ((int64_t)w.split * n_obj_launch + w.obj_local) * gp.n_freq + w.K0 : nullptr;
+            float2* nat2 = (sums && tp.gls == 1) ? reinterpret_cast<float2*>(sums) + (w.obj_local * gp.n_tiles + w.tile) * tile_elems +
+                                                       32 * q + lane : nullptr;
             const float zinv = tp.y_is_w ? ob.winv : ob.zinv;
             auto chunk_sums = [&](int ch) {
                 const int m0 = ch * 16;
@@ -805,6 +857,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     const float wa = (wr[i] - q1) * ob.winv, wb = (wi[i] + q0) * ob.winv;
                     if (nat) {
                         nat[(int64_t)(m0 + i) * 128] = make_float4(za, zb, wa, wb);
+                    } else if (nat2) {
+                        nat2[(int64_t)(m0 + i) * 128] = make_float2(za, zb);
                     } else {
                         const int kl = is_im ? kl0 - i : kl0 + i;
                         if (i < i_lim && kl < n_valid)
@@ -812,7 +866,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     }
                 }
             };
-            if (sums) {
+            if (sums && !FUSED) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk_sums(ch);
             } else if (ragged) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk(ch, std::true_type{});
@@ -827,7 +881,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 }
                 ++n_acc;
             }
-            if (partials && !sums) {
+            if (partials && (!sums || FUSED)) {
                 Best mine;
                 mine.p = (double)bp;
                 mine.k = (bk == 0x7fffffff) ? INT64_MAX : w.K0 + (int64_t)bk;

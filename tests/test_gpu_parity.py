@@ -413,6 +413,48 @@ def test_generalized_batch_parity(lsp, oracle, dtype, kernel):
     assert_best_parity(best, P_ref, w, dtype, oracle, f"generalised {kernel}")
 
 
+@pytest.mark.parametrize("fast", [False, True])
+def test_generalized_fused_epilogue_unsplit_batch(lsp, oracle, fast):
+    """The generalised mode's fused tensor-kernel epilogue (n_split = 1: the w pass leaves (C, S) per element, the weighted
+    pass evaluates ZK09's power in its own epilogue): a config-3-shaped batch large enough to run unsplit, full periodogram +
+    best period; the oracle checks a seeded sample of whole objects, empty and tiny objects included."""
+    import torch
+    w = make_config(3, n_obj=1300, n_freq=9001)
+    off = w.offsets.copy()
+    y, sigma = _with_errors(w, 78)
+    # make object 3 empty and object 4 a single point (P = 0 rows)
+    keep = np.ones(w.n_obs, dtype=bool)
+    keep[off[3]:off[4]] = False
+    keep[off[4] + 1:off[5]] = False
+    lens = np.diff(off)
+    lens[3], lens[4] = 0, 1
+    off2 = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    t2, y2, s2 = w.t[keep], y[keep], sigma[keep]
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f32", fast_math=fast) as plan:
+        P, best = plan.periodogram_generalized(torch.from_numpy(off2).cuda(), torch.from_numpy(t2).cuda(), torch.from_numpy(y2).cuda(),
+                                               torch.from_numpy(s2).cuda(), best=True, h_offsets=torch.from_numpy(off2))
+        info = plan.last_call_info()
+        best_only = plan.periodogram_generalized(torch.from_numpy(off2).cuda(), torch.from_numpy(t2).cuda(), torch.from_numpy(y2).cuda(),
+                                                 torch.from_numpy(s2).cuda(), best=True, want_power=False)[1]
+        P = P.cpu().numpy().astype(np.float64)
+        best = tuple(x.cpu().numpy() for x in best)
+        best_only = tuple(x.cpu().numpy() for x in best_only)
+    assert info["kernel"] == "tensor" and info["n_split"] == 1
+    for a_, b_ in zip(best, best_only):
+        assert np.array_equal(a_, b_, equal_nan=True)
+    rng = np.random.default_rng(8)
+    pick = np.unique(np.concatenate([rng.choice(1300, 20, replace=False), [0, 3, 4, 1299]]))
+    sub_off = np.concatenate([[0], np.cumsum(lens[pick])]).astype(np.int64)
+    sel = np.concatenate([np.arange(off2[o], off2[o + 1]) for o in pick])
+    P_ref = oracle.periodogram_generalized(sub_off, t2[sel], y2[sel], s2[sel], w.f_min, w.f_max, w.n_freq)
+    assert np.all(P[3] == 0.0) and np.all(P[4] == 0.0) and best[2][3] == -1
+    assert np.all(np.isfinite(P)) and P.min() >= -TOL["f32"] and P.max() <= 1.0 + TOL["f32"]
+    big = [i for i, o in enumerate(pick) if lens[o] >= 3]
+    assert_power_parity(P[pick][big], P_ref[big], "f32", "generalised fused")
+    sub = Workload("gls", np.concatenate([[0], np.cumsum(lens[pick][big])]).astype(np.int64), None, None, w.f_min, w.f_max, w.n_freq, "f32")
+    assert_best_parity(tuple(x[pick][big] for x in best), P_ref[big], sub, "f32", oracle, "generalised fused")
+
+
 def test_generalized_single_object_and_edge_cases(lsp, oracle):
     import torch
     w = make_config(2, n_t=3000, n_freq=20000, dtype="f64")
