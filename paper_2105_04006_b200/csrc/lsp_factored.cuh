@@ -51,11 +51,14 @@ template <> struct FactoredCfg<float> {
     using V2 = float2;
 };
 template <> struct FactoredCfg<double> {
-    static constexpr int TH = 2;
+    // 4 x 4 register tile (64 DFMA per 8 LDS.128 and observation; 128 accumulator registers, see the setmaxnreg split in
+    // lsp_factored_ws.cuh) and groups twice as wide as in round 1 (NL = 32): every non-DFMA instruction displaces a DFMA
+    // on this pipe, and both the operand loads and the producers' work per pair halve.
+    static constexpr int TH = 4;
     static constexpr int TM = 4;
-    static constexpr int NL = 16;
+    static constexpr int NL = 32;
     static constexpr int EPC = 1;
-    static constexpr int TILE = kFacGroups * 2 * NL;   // 2048
+    static constexpr int TILE = kFacGroups * 2 * NL;   // 4096
     using V2 = double2;
 };
 

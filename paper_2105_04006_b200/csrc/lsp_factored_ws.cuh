@@ -23,35 +23,37 @@ namespace lsp {
 constexpr int kWsConsumers = 256;
 constexpr int kWsProducers = 128;
 constexpr int kWsThreads = kWsConsumers + kWsProducers;
+constexpr int kWsProducerRegs = 88, kWsConsumerRegs = 208;      // 128 x 88 + 256 x 208 = 64512 = 384 x 168
 
 #ifndef LSP_WS_JC_F32
 #define LSP_WS_JC_F32 16
 #endif
 #ifndef LSP_WS_JC_F64
-#define LSP_WS_JC_F64 32      // FP64: 32-observation stages x 2 (same bytes as 16 x 4): the consumers' loop-carried register
-#endif                        // permutation (~105 moves per unrolled stage, each displacing a DFMA) is paid half as often
+#define LSP_WS_JC_F64 16      // FP64: 16-observation stages x 2 (48 KB each with NL = 32)
+#endif
 #ifndef LSP_WS_STAGES_F32
 #define LSP_WS_STAGES_F32 4
 #endif
 #ifndef LSP_WS_STAGES_F64
 #define LSP_WS_STAGES_F64 2
 #endif
-// An a-operand row (one observation, G = 64 groups) is stored in two halves of 32 elements; inside the second half element i
-// sits at i ^ GSKEW (a 64-byte XOR swizzle) so that the producers' stores -- lanes alternate between the halves
-// (operand_pos) -- fall into different banks: without it every quarter-warp store was a 2-way conflict (r01: 87.7 M
-// conflicts per FP64 launch).  No padding: the FP64 ring already fills shared memory.
+// An a-operand row (one observation, G = 64 groups) is stored in operand_pos order: the TH elements of a thread land in TH
+// (FP32: TH / 2) sub-rows, and consecutive producer lanes alternate between the sub-rows, i.e. between addresses a
+// multiple of 128 bytes apart: without a swizzle every quarter-warp store is a 2- or 4-way bank conflict (r01: 87.7 M
+// conflicts per FP64 launch).  Inside sub-row r element i therefore sits at i ^ (r * SWZ): a 64-byte (FP32: 2 sub-rows of 32)
+// or 32-byte (FP64: 4 sub-rows of 16) XOR swizzle.  No padding: the rings already fill shared memory.
 template <typename T> struct WsCfg;
 template <> struct WsCfg<float> {
     static constexpr int JC = LSP_WS_JC_F32;         // observations per ring stage
     static constexpr int STAGES = LSP_WS_STAGES_F32;
-    static constexpr int GSKEW = 8;                  // 8 float2 = 64 bytes
+    static constexpr int SUB = 32, SWZ = 8;          // sub-rows of 32 float2; XOR 8 float2 = 64 bytes per sub-row index
     static constexpr int GP = kFacGroups;            // a-row length
     static constexpr int STAGE_ELEMS = JC * (2 * GP + 2 * FactoredCfg<float>::NL);   // complex elements per stage
 };
 template <> struct WsCfg<double> {
     static constexpr int JC = LSP_WS_JC_F64;
     static constexpr int STAGES = LSP_WS_STAGES_F64;
-    static constexpr int GSKEW = 4;                  // 4 double2 = 64 bytes
+    static constexpr int SUB = 16, SWZ = 2;          // sub-rows of 16 double2; XOR 2 double2 = 32 bytes per sub-row index
     static constexpr int GP = kFacGroups;
     static constexpr int STAGE_ELEMS = JC * (2 * GP + 2 * FactoredCfg<double>::NL);
 };
@@ -101,7 +103,7 @@ __device__ __forceinline__ void mbar_wait_sleep(unsigned long long* bar, unsigne
     asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                  : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     while (!done) {
-        __nanosleep(ns);
+        __nanosleep(ns);      // measured: the actual sleep is a fraction of `ns`; every poll costs the working warps issue slots
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
     }
@@ -214,7 +216,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     using C = FactoredCfg<T>;
     using V2 = typename C::V2;
     constexpr int G = kFacGroups, TH = C::TH, TM = C::TM, NL = C::NL, L = 2 * NL, TILE = C::TILE, EPC = C::EPC;
-    constexpr int JC = WsCfg<T>::JC, S = WsCfg<T>::STAGES, GP = WsCfg<T>::GP, GSKEW = WsCfg<T>::GSKEW;
+    constexpr int JC = WsCfg<T>::JC, S = WsCfg<T>::STAGES, GP = WsCfg<T>::GP, SUB = WsCfg<T>::SUB, SWZ = WsCfg<T>::SWZ;
     constexpr int NGI = G / TH, NMI = NL / TM;
     constexpr int STAGE = WsCfg<T>::STAGE_ELEMS;             // V2 elements per stage: [JC][GP] a, [JC][GP] a2, [JC][NL] b, [JC][NL] b2
     static_assert(NGI * NMI == kWsConsumers / 2, "Z and W halves each cover the G x NL tile once");
@@ -241,7 +243,10 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
     }
     __syncthreads();
 
+    // Register split (384 threads x 168 at launch): the consumers hold TH x TM x 4 accumulators (FP64: 128 registers) plus their
+    // operands, the producers need little.
     if (tid >= kWsConsumers) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kWsProducerRegs));
         // =========================================== producers ===============================================
         // a_gj = y_j e^{i alpha_gj} with alpha_gj = 2 pi f(c_g) t_j and g = 8 g1 + g0.  f(c_g) = f(c_g0) + g1 (8 L df), so
         //     e^{i alpha_gj} = u_{g0 j} v_{g1 j},   u = e^{2 pi i f(c_g0) t_j},   v = e^{2 pi i (8 g1 L df) t_j}.
@@ -252,7 +257,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
         const int ptid = tid - kWsConsumers;
         const int gen_g = ptid & (G - 1);
         const int gen_pos_raw = operand_pos<TH, NGI, EPC>(gen_g);
-        const int gen_pos_a = gen_pos_raw ^ ((gen_pos_raw >> 5) * GSKEW);       // second half of the row: 64-byte XOR swizzle
+        const int gen_pos_a = gen_pos_raw ^ ((gen_pos_raw / SUB) * SWZ);        // XOR swizzle inside the sub-row
         const int p_q = ptid & 7, p_j = ptid >> 3;                                 // phase 1: phasor index, observation
         static_assert(JC % 16 == 0 && kWsProducers == 128 && G == 64, "producer work split");
         constexpr int NP = JC / 16;                                                // u phasors per thread per chunk
@@ -307,7 +312,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 }
                 named_bar_sync(1, kWsProducers);
                 const int s = c % S;
-                mbar_wait_sleep(&empty[s], ((c / S) & 1) ^ 1, 100);
+                mbar_wait_sleep(&empty[s], ((c / S) & 1) ^ 1, 1500);
                 V2* sA1 = ring + (size_t)s * STAGE;
                 V2* sA2 = sA1 + JC * GP;
                 V2* sB1 = sA2 + JC * GP;
@@ -349,6 +354,7 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             named_bar_sync(1, kWsProducers);         // everyone has read it before thread 0 overwrites it
         }
     } else {
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kWsConsumerRegs));
         // =========================================== consumers ===============================================
         const int lane = tid & 31, wq = (tid >> 5) & 3;
         const bool is_w = tid >= kWsConsumers / 2;             // warps 4-7 contract W (doubled angles)
@@ -362,6 +368,22 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
         }
         const int offA = is_w ? JC * GP : 0;
         const int offB = 2 * JC * GP + (is_w ? JC * NL : 0);
+        // element offsets of this thread's operands inside one observation's rows (the XOR swizzle is folded in here, once):
+        // the inner loop's loads then differ by compile-time multiples of the row lengths only (immediate offsets)
+        int oa[EPC == 2 ? TH / 2 : TH], ob[EPC == 2 ? TM / 2 : TM];
+        if constexpr (EPC == 2) {          // float4 units (two complex operands per load)
+            static_assert(EPC == 1 || (TH / 2 * NGI * 2 == G && NGI * 2 == SUB), "one float4 index step of NGI = one sub-row");
+#pragma unroll
+            for (int q = 0; q < TH / 2; ++q) oa[q] = q * NGI + (gi ^ (q * (SWZ / 2)));
+#pragma unroll
+            for (int q = 0; q < TM / 2; ++q) ob[q] = q * NMI + mi;
+        } else {
+            static_assert(EPC == 2 || NGI == SUB, "one index step of NGI = one sub-row");
+#pragma unroll
+            for (int a = 0; a < TH; ++a) oa[a] = a * NGI + (gi ^ (a * SWZ));
+#pragma unroll
+            for (int cc = 0; cc < TM; ++cc) ob[cc] = cc * NMI + mi;
+        }
 
         V2 acc_r[TH][TM], acc_i[TH][TM];        // (Srr, Sri) and (Sir, Sii) of this thread's (group, m) pairs
 #pragma unroll
@@ -386,21 +408,19 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 if constexpr (EPC == 2) {           // one LDS.128 = two complex operands
 #pragma unroll
                     for (int q = 0; q < TH / 2; ++q) {
-                        static_assert(TH / 2 * NGI * 2 == G && NGI * 2 == 32, "one float4 index step of NGI = one 32-element half row");
-                        const float4 ch = reinterpret_cast<const float4*>(A + jj * GP)[q * NGI + (gi ^ (q * (GSKEW / 2)))];
+                        const float4 ch = reinterpret_cast<const float4*>(A)[jj * (GP / 2) + oa[q]];
                         av[2 * q].x = ch.x; av[2 * q].y = ch.y; av[2 * q + 1].x = ch.z; av[2 * q + 1].y = ch.w;
                     }
 #pragma unroll
                     for (int q = 0; q < TM / 2; ++q) {
-                        const float4 ch = reinterpret_cast<const float4*>(B + jj * NL)[q * NMI + mi];
+                        const float4 ch = reinterpret_cast<const float4*>(B)[jj * (NL / 2) + ob[q]];
                         bv[2 * q].x = ch.x; bv[2 * q].y = ch.y; bv[2 * q + 1].x = ch.z; bv[2 * q + 1].y = ch.w;
                     }
                 } else {                            // one LDS.128 = one complex operand
-                    static_assert(EPC == 2 || NGI == 32, "one index step of NGI = one 32-element half row");
 #pragma unroll
-                    for (int a = 0; a < TH; ++a) av[a] = A[jj * GP + a * NGI + (gi ^ (a * GSKEW))];
+                    for (int a = 0; a < TH; ++a) av[a] = A[jj * GP + oa[a]];
 #pragma unroll
-                    for (int cc = 0; cc < TM; ++cc) bv[cc] = B[jj * NL + cc * NMI + mi];
+                    for (int cc = 0; cc < TM; ++cc) bv[cc] = B[jj * NL + ob[cc]];
                 }
 #pragma unroll
                 for (int a = 0; a < TH; ++a)
