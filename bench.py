@@ -46,9 +46,9 @@ SM_MAX_HZ = 1965e6
 FP32_LANES = 128      # FP32 FMA lanes per SM per clock
 FP64_LANES = 64       # FP64 FMA lanes per SM per clock
 FLOP_PER_PAIR = 8.0   # factored formulation: 4 FMA per (t,f) pair ("4 FMA = 8 flop/pair")
-# Tensor path: the same 4 MAC per pair as one FP16 GEMM; the accurate mode issues three products per MAC
-# (a_hi b_hi + a_hi b_lo + a_lo b_hi), fast_math one.
-TENSOR_PRODUCTS = {False: 3, True: 1}
+# Tensor path: the same 4 MAC per pair as one FP16 GEMM; the accurate mode issues two products per MAC (a_hi (b_hi + b_lo),
+# the library default) or three (a_hi b_hi + a_hi b_lo + a_lo b_hi; --tensor-products 3), fast_math one.
+TENSOR_PRODUCTS = {False: 2, True: 1}
 TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 burst; fp16 : bf16 nominal ratio is 1)
 
 
@@ -119,21 +119,22 @@ def measured_tensor_peak():
         return TENSOR_PEAK_FALLBACK, "of fallback (B200_PROFILING.md 1.59 PFLOP/s bf16 burst; fp16:bf16 = 1)"
 
 
-def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float, workload: str = ""):
+def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float, workload: str = "",
+             products: int = 0):
     """Roofline object of the dominant kernel: achieved = algorithmic flop per launch
     (8 flop per (t,f) pair x pairs) / mean launch duration measured with CUDA events on the launching stream."""
     achieved = pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
     traffic, traffic_from = (None, None) if fast else ncu_traffic(workload, kernel, dtype)
     if kernel == "tensor":
         peak, prov = measured_tensor_peak()
-        prod = TENSOR_PRODUCTS[bool(fast)]
+        prod = products if products else TENSOR_PRODUCTS[bool(fast)]
         return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_from": traffic_from,
                 "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
                 "peak_is": prov,
                 "executed_flop_per_pair": FLOP_PER_PAIR * prod,
                 "executed_tflops": achieved * prod, "frac_executed": achieved * prod / peak,
-                "note": "FP16 hi+lo split operands: %d tcgen05 products per algorithmic MAC" % prod}
+                "note": "FP16 split operands: %d tcgen05 products per algorithmic MAC" % prod}
     lanes = FP32_LANES if dtype == "f32" else FP64_LANES
     peak = N_SM * lanes * 2 * SM_MAX_HZ / 1e12
     if kernel != "factored":
@@ -168,6 +169,8 @@ def parse_args():
     ap.add_argument("--dtype", default="f32", choices=["f32", "f64"], help="precision of the primary line")
     ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
     ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored", "tensor"])
+    ap.add_argument("--tensor-products", type=int, default=0, choices=[0, 2, 3],
+                    help="tensor path, accurate mode: FP16 products per MAC (lsp_config.tensor_products; 0 = library default = 2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="primary leg only (no fp64 / fp32_fma_pipe / c3 / c4 objects)")
     ap.add_argument("--variants", action="store_true", help="add the comparison legs: fast_math, direct kernels, generalised mode")
@@ -332,11 +335,11 @@ def describe_workload(name: str, w) -> str:
 class Leg:
     """One precision of one workload on this rank's GPU: device-resident steps and end-to-end (host buffer) steps."""
 
-    def __init__(self, pkg, torch, w, name: str, dtype: str, fast_math: bool, kernel: str, device: int):
+    def __init__(self, pkg, torch, w, name: str, dtype: str, fast_math: bool, kernel: str, device: int, tensor_products: int = 0):
         self.torch, self.w, self.name, self.dtype = torch, w, name, dtype
         self.tdt = torch.float32 if dtype == "f32" else torch.float64
         self.plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, dtype, fast_math=fast_math and dtype == "f32", kernel=kernel,
-                             device=device)
+                             device=device, tensor_products=tensor_products)
         self.plan.set_timing(False)            # the timed steps run as a user's would: no events inside the library
         self.h_off = torch.from_numpy(w.offsets)
         self.h_t = torch.from_numpy(w.t).pin_memory()
@@ -435,8 +438,9 @@ def timed_loop(torch, dist, world, leg, step, steps: int, warmup: int, flush):
     return total_ms, info
 
 
+ARITHMETIC_3 = "fp16 hi+lo split of both operands (22-bit), 3 tcgen05 products per MAC, fp32 accumulate in TMEM; phases two-float fp32"
 ARITHMETIC = {
-    ("tensor", False): "fp16 hi+lo split operands (22-bit), 3 tcgen05 products per MAC, fp32 accumulate in TMEM; phases two-float fp32",
+    ("tensor", False): "fp16 generated operand (11-bit) x fp16 hi+lo tabulated operand (22-bit), 2 tcgen05 products per MAC, fp32 accumulate in TMEM; phases two-float fp32",
     ("tensor", True): "fp16 operands, 1 tcgen05 product per MAC, fp32 accumulate; MUFU sincos (fast_math)",
     ("factored", False): "all-fp32 FFMA2 contraction (fp64: DFMA)", ("factored", True): "all-fp32 FFMA2 contraction, MUFU sincos",
     ("direct", False): "one accurate sincos per pair", ("direct", True): "one MUFU sincos per pair",
@@ -450,7 +454,8 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     w = workload_for(name, dtype, rank, world)
     kernel = args.kernel if kernel is None else kernel
     fast = bool(args.fast_math if fast is None else fast) and dtype == "f32"
-    leg = Leg(pkg, torch, w, name, dtype, fast, kernel, device)
+    leg = Leg(pkg, torch, w, name, dtype, fast, kernel, device, args.tensor_products)
+    products = 1 if fast else (3 if args.tensor_products == 3 else 2)
     pairs_step = w.pairs
     pairs_all = pairs_step
     if world > 1:
@@ -469,7 +474,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     pipe_ops = 0.0
     if info["kernel"] == "factored":
         pipe_ops, _ = pipe_peak(1 if dtype == "f32" else 2, device)
-    rf = roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, name)
+    rf = roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, name, products)
     es = 4 if dtype == "f32" else 8
     in_bytes = w.n_obs * 2 * es + (w.n_obj + 1) * 8
     out_bytes = w.n_obj * (2 * es + 8) if leg.best_only else w.n_obj * w.n_freq * es
@@ -486,7 +491,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
         "kernel_ms_per_step": k_ms,
         "gpu_launches": dev_launches,
         "roofline": rf,
-        "arithmetic": ARITHMETIC.get((info["kernel"], fast), ""),
+        "arithmetic": ARITHMETIC_3 if (info["kernel"] == "tensor" and products == 3) else ARITHMETIC.get((info["kernel"], fast), ""),
     }
     if world > 1 and name == "c3":
         obs = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(world)]
@@ -597,7 +602,7 @@ def run_c5(args, pkg, torch, device, flush):
             for j, nf in enumerate(C5_NF):
                 w = make_config(5, dtype=dtype, n_t=nt, n_freq=nf, point=i * len(C5_NF) + j)
                 plan = pkg.Plan(w.f_min, w.f_max, w.n_freq, dtype, kernel=args.kernel, fast_math=args.fast_math and dtype == "f32",
-                                device=device)
+                                device=device, tensor_products=args.tensor_products)
                 h_off = torch.from_numpy(w.offsets)
                 d_off, d_t, d_y = h_off.to(dev), torch.from_numpy(w.t).to(dev), torch.from_numpy(w.y).to(dev)
                 d_out = torch.empty((1, nf), dtype=tdt, device=dev)
@@ -621,7 +626,8 @@ def run_c5(args, pkg, torch, device, flush):
                     torch.cuda.synchronize()
                     kms += plan.last_kernel_ms() * steps / 3.0
                 info = plan.last_call_info()
-                rf = roofline(info["kernel"], dtype, args.fast_math and dtype == "f32", w.pairs, kms / steps, pipe_ops)
+                rf = roofline(info["kernel"], dtype, args.fast_math and dtype == "f32", w.pairs, kms / steps, pipe_ops,
+                              products=1 if (args.fast_math and dtype == "f32") else (3 if args.tensor_products == 3 else 2))
                 rows.append({"dtype": dtype, "n_t": nt, "n_freq": nf, "pairs": w.pairs, "kernel": info["kernel"],
                              "n_split": info["n_split"], "ms_per_step": tot / steps, "kernel_ms": kms / steps,
                              "pairs_per_s": w.pairs * steps / (tot * 1e-3), "bound": rf["bound"], "roofline_frac": rf["frac"],

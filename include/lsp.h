@@ -54,8 +54,9 @@ typedef enum {
                                 PAPER.md:L137-216, with smem staging L121-125 and range-reduced phase)     */
     LSP_KERNEL_FACTORED = 2, /* angle-addition outer product: no sincos in the O(N_t N_f) loop, 4 FMA/pair */
     LSP_KERNEL_TENSOR = 3    /* FP32 mode only: the same contraction on the tensor cores (tcgen05.mma kind::f16, FP32
-                                accumulators in TMEM).  Operands are FP16 hi+lo pairs, three MMAs per product
-                                (fast_math = 1: hi only, one MMA, MUFU sincos); phases stay FP64-reduced.          */
+                                accumulators in TMEM).  Operands are FP16 hi(+lo) pairs, two or three MMAs per product
+                                (lsp_config.tensor_products; fast_math = 1: hi only, one MMA, MUFU sincos); phases
+                                stay FP64-reduced.                                                                  */
 } lsp_kernel;
 
 typedef struct lsp_config {
@@ -78,6 +79,11 @@ typedef struct lsp_config {
     int32_t tensor_roles;   /* tensor path warp-role shape: 0 = chosen by item length, 1 = short-item shape
                                    (8 epilogue warps), 2 = long-item shape (4 epilogue warps)               */
     int32_t tensor_b_stages;/* tensor path: depth of the B-operand (TMA) ring, 2..8; 0 = library default    */
+    int32_t tensor_products;/* tensor path, fast_math = 0: FP16 tcgen05 products per multiply-accumulate.
+                                   2 (= 0, default): a_hi (b_hi + b_lo) -- the generated operand a = y e^{i alpha} is
+                                   one FP16 (11 significand bits), the tabulated one an FP16 pair (22 bits);
+                                   3: a_hi b_hi + a_hi b_lo + a_lo b_hi -- both operands FP16 pairs                 */
+    int32_t reserved;       /* must be 0                                                                   */
 } lsp_config;
 
 /* lsp_config.flags */
@@ -90,7 +96,7 @@ typedef struct lsp_config {
  * allocates scratch (argmax partials, split-N_t partial sums, the device chunk ring for host output).
  * The plan owns all of that; the caller owns every buffer passed to the calls below.
  * Errors: LSP_ERR_INVALID_ARG (f_min <= 0, f_max <= f_min, n_freq < 1, fast_math with FP64, unknown
- * enum or flag bit, tensor_roles / tensor_b_stages out of range), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
+ * enum or flag bit, tensor_roles / tensor_b_stages / tensor_products out of range, reserved != 0), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
  * failure.  A plan is not thread-safe; distinct plans are independent.
  */
 lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan /* HOST */);
@@ -205,10 +211,12 @@ const char* lsp_last_error(const lsp_plan* plan);
 
 /* Bookkeeping of the LAST call on the plan, for benchmarks and tests: how many of the library's kernels it launched,
  * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), -- host-output
- * calls only -- chunks copied, and the tensor kernel's warp-role shape (0 = tensor kernel not used, 1 = short-item
- * shape, 2 = long-item shape; see lsp_config.tensor_roles).  Any pointer may be NULL. */
+ * calls only -- chunks copied, the tensor kernel's warp-role shape (0 = tensor kernel not used, 1 = short-item
+ * shape, 2 = long-item shape; see lsp_config.tensor_roles) and its FP16 products per multiply-accumulate in the last
+ * launch (0 = tensor kernel not used; 1 = fast_math; 2 or 3: lsp_config.tensor_products -- a launch that holds an object
+ * of fewer than 32 observations runs with 3 whatever the plan says).  Any pointer may be NULL. */
 void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used,
-                        int32_t* n_split, int64_t* n_chunks, int32_t* tensor_shape);
+                        int32_t* n_split, int64_t* n_chunks, int32_t* tensor_shape, int32_t* tensor_products);
 
 /*
  * Device time of the periodogram kernel(s) of the LAST call, in milliseconds, measured with CUDA events

@@ -38,6 +38,7 @@ class LspConfig(ctypes.Structure):
         ("chunk_bytes", ctypes.c_int64), ("max_objects", ctypes.c_int64), ("max_total_obs", ctypes.c_int64),
         ("kernel", ctypes.c_int32), ("flags", ctypes.c_int32),
         ("table_budget_bytes", ctypes.c_int64), ("tensor_roles", ctypes.c_int32), ("tensor_b_stages", ctypes.c_int32),
+        ("tensor_products", ctypes.c_int32), ("reserved", ctypes.c_int32),
     ]
 
 
@@ -74,7 +75,7 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_last_error.argtypes = [vp]
     lib.lsp_last_error.restype = ctypes.c_char_p
     lib.lsp_last_call_info.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i32),
-                                       ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32)]
+                                       ctypes.POINTER(i32), ctypes.POINTER(i64), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     lib.lsp_last_call_info.restype = None
     lib.lsp_set_timing.argtypes = [vp, i32]
     lib.lsp_set_timing.restype = None
@@ -167,14 +168,14 @@ class Plan:
                  normalize: bool = False, center: bool = False, device: int = 0, n_copy_streams: int = 0,
                  chunk_bytes: int = 0, kernel: str = "auto", max_objects: int = 0, max_total_obs: int = 0,
                  pageable_staged: bool = False, table_budget_bytes: int = 0, tensor_roles: int = 0,
-                 tensor_b_stages: int = 0):
+                 tensor_b_stages: int = 0, tensor_products: int = 0):
         if dtype not in ("f32", "f64"):
             raise ValueError("dtype must be 'f32' or 'f64'")
         self.cfg = LspConfig(float(f_min), float(f_max), int(n_freq), LSP_F32 if dtype == "f32" else LSP_F64,
                              int(fast_math), int(normalize), int(center), int(device), int(n_copy_streams),
                              int(chunk_bytes), int(max_objects), int(max_total_obs), _KERNELS[kernel],
                              LSP_FLAG_PAGEABLE_STAGED if pageable_staged else 0, int(table_budget_bytes),
-                             int(tensor_roles), int(tensor_b_stages))
+                             int(tensor_roles), int(tensor_b_stages), int(tensor_products), 0)
         self.dtype = dtype
         self.torch_dtype = torch.float32 if dtype == "f32" else torch.float64
         self.n_freq = int(n_freq)
@@ -227,11 +228,11 @@ class Plan:
 
     def last_call_info(self) -> dict:
         nl, npairs, nch = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
-        ku, ns, ts = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+        ku, ns, ts, tp = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
         load_library().lsp_last_call_info(self._plan, ctypes.byref(nl), ctypes.byref(npairs), ctypes.byref(ku),
-                                          ctypes.byref(ns), ctypes.byref(nch), ctypes.byref(ts))
+                                          ctypes.byref(ns), ctypes.byref(nch), ctypes.byref(ts), ctypes.byref(tp))
         return {"launches": nl.value, "pairs": npairs.value, "kernel": _KERNEL_NAMES.get(ku.value, ku.value),
-                "n_split": ns.value, "chunks": nch.value, "tensor_shape": ts.value}
+                "n_split": ns.value, "chunks": nch.value, "tensor_shape": ts.value, "tensor_products": tp.value}
 
     # -- the two calls
     def periodogram_batched(self, offsets, t, y, *, out=None, host_out=None, best: bool = False, h_offsets=None,

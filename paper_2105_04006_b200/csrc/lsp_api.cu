@@ -59,6 +59,7 @@ struct lsp_plan {
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     int tc_stages_b = 0;          // B-operand ring depth of the tensor kernel; 0 = as many as fit (cfg.tensor_b_stages)
+    int tc_products = 2;          // FP16 products per MAC of the accurate tensor mode: 2 or 3 (cfg.tensor_products)
     int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
@@ -73,6 +74,7 @@ struct lsp_plan {
     int64_t n_launches = 0, n_pairs = 0, n_chunks = 0;
     int32_t kernel_used = 0, n_split = 1;
     int32_t tensor_shape = 0;     // role shape of the last tensor-kernel launch: 0 = none, 1 = short-item, 2 = long-item
+    int32_t tensor_products = 0;  // FP16 products per MAC of the last tensor-kernel launch (0 = none)
     bool timing = false;
     std::vector<cudaEvent_t> t_start, t_stop;
     size_t t_used = 0;
@@ -164,10 +166,28 @@ struct Schedule {
     int tile;        // frequencies per CTA
     int n_tiles;
     int n_split;
+    int products;      // tensor path: FP16 products per MAC (1 = fast_math, 2, 3)
     TensorParams tp;   // tensor path only
 };
 
-Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int kernel_override = -1)
+// Two-product tensor mode: the generated operand a = y e^{i alpha} is a single FP16, i.e. every term of a sum carries a relative
+// error of up to 2^-12.  That is harmless while step 5 is well conditioned (measured <= 4.5e-4 of max P on pure-noise objects,
+// a few 1e-5 when a signal dominates) but not for objects of a handful of observations, whose 2 x 2 systems are close to
+// singular at many grid frequencies: a launch that holds an object shorter than this runs with three products.
+constexpr int64_t kTcMinNtTwoProducts = 32;
+
+// Smallest N_t > 0 among objects [o0, o0 + no) (INT64_MAX if all are empty); `ho` = host copy of the CSR offsets.
+int64_t range_min_nt(const int64_t* ho, int64_t o0, int64_t no)
+{
+    int64_t m = INT64_MAX;
+    for (int64_t o = o0; o < o0 + no; ++o) {
+        const int64_t n = ho[o + 1] - ho[o];
+        if (n > 0 && n < m) m = n;
+    }
+    return m;
+}
+
+Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int kernel_override = -1, int64_t min_nt = INT64_MAX)
 {
     const lsp_config& c = p->cfg;
     Schedule s{};
@@ -185,6 +205,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
         s.tp.nl = (int)nl;
         s.tp.tile = (int)(kTcGroups * 2 * nl);
         s.tp.n_ops = c.fast_math ? 2 : 4;
+        s.products = c.fast_math ? 1 : ((p->tc_products == 3 || min_nt < kTcMinNtTwoProducts) ? 3 : 2);
         s.tp.b_plane_bytes = 2 * (int)nl * kTcKB * 2;
         s.tp.b_stage_bytes = s.tp.n_ops * s.tp.b_plane_bytes + kTcAuxBytes;
         s.tile = s.tp.tile;
@@ -234,7 +255,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
         // B ring (TMA -> MMA; the generators read its aux blocks): as deep as shared memory allows, at most 8 stages
         const int reserve = (s.tp.long_items ? tc_static_smem<4, 4>() : tc_static_smem<8, 3>()) + (int)tc_smem_bytes(0, 0) + 512;
         const int fit = (int)std::max<int64_t>(2, std::min<int64_t>(8, (int64_t)(p->smem_optin - reserve) / s.tp.b_stage_bytes));
-        const int need = tc_min_stages_b(c.fast_math != 0, s.tp.long_items ? 4 : 3);       // always <= fit for NL <= 112
+        const int need = tc_min_stages_b(s.products == 1 ? 1 : (s.products == 3 ? 0 : 2), s.tp.long_items ? 4 : 3);       // always <= fit for NL <= 112
         s.tp.stages_b = std::max(need, p->tc_stages_b > 0 ? std::min(p->tc_stages_b, fit) : fit);
         s.tp.fixup = split > 1 ? 1 : 0;
     }
@@ -262,16 +283,23 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
                                   gls_yy);
             };
             p->tensor_shape = s.tp.long_items ? 2 : 1;
+            p->tensor_products = s.products;
+            // precision mode of the kernel template: 1 = fast_math, 2 = two products (default), 0 = three (tensor_products = 3)
+            auto go_pm = [&](auto pm_tag) -> cudaError_t {
+                constexpr int PM = decltype(pm_tag)::value;
+                if (s.tp.weighted && s.tp.gls == 2)      // generalised mode, weighted W slot + ZK09's epilogue fused
+                    return s.tp.long_items ? go(lsp_tensor_kernel<float, PM, 4, 4, 2>, TcRoles<4, 4>::kThreads)
+                                           : go(lsp_tensor_kernel<float, PM, 8, 3, 2>, TcRoles<8, 3>::kThreads);
+                if (s.tp.weighted)                       // generalised mode: the W slot carries the weights
+                    return s.tp.long_items ? go(lsp_tensor_kernel<float, PM, 4, 4, 1>, TcRoles<4, 4>::kThreads)
+                                           : go(lsp_tensor_kernel<float, PM, 8, 3, 1>, TcRoles<8, 3>::kThreads);
+                return s.tp.long_items ? go(lsp_tensor_kernel<float, PM, 4, 4, 0>, TcRoles<4, 4>::kThreads)
+                                       : go(lsp_tensor_kernel<float, PM, 8, 3, 0>, TcRoles<8, 3>::kThreads);
+            };
             cudaError_t e;
-            if (s.tp.weighted && s.tp.gls == 2)      // generalised mode, weighted W slot + ZK09's epilogue fused
-                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 2>, TcRoles<4, 4>::kThreads)
-                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 2>, TcRoles<8, 3>::kThreads);
-            else if (s.tp.weighted)                  // generalised mode: the W slot carries the weights
-                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 1>, TcRoles<4, 4>::kThreads)
-                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 1>, TcRoles<8, 3>::kThreads);
-            else
-                e = s.tp.long_items ? go(lsp_tensor_kernel<float, FAST, 4, 4, 0>, TcRoles<4, 4>::kThreads)
-                                    : go(lsp_tensor_kernel<float, FAST, 8, 3, 0>, TcRoles<8, 3>::kThreads);
+            if (FAST) e = go_pm(std::integral_constant<int, 1>{});
+            else if (s.products == 3) e = go_pm(std::integral_constant<int, 0>{});
+            else e = go_pm(std::integral_constant<int, 2>{});
             if (e != cudaSuccess) return e;
         } else {
             return cudaErrorInvalidValue;      // rejected at plan creation
@@ -509,7 +537,7 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     const lsp_config& c = p->cfg;
     p->n_launches = p->n_pairs = p->n_chunks = 0;
     p->t_used = 0;
-    p->tensor_shape = 0;
+    p->tensor_shape = p->tensor_products = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
     const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
@@ -577,9 +605,13 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     // Steps 2-6' for objects [o0, o0 + no) holding `obs` observations, asynchronous on the caller's stream: `out` (device, may be
     // NULL) receives rows relative to o0.  One launch sequence, except on the tensor path when the B-operand table of the range
     // would exceed its memory budget: then the objects go in sub-ranges (same results: an object's sums never span launches).
+    // two-product tensor mode: the launch's shortest object decides (kTcMinNtTwoProducts); needs the offsets on the host
+    const bool need_min_nt = s.kernel == LSP_KERNEL_TENSOR && s.products == 2;
+    if (need_min_nt && !host_offsets()) return fail(p, LSP_ERR_CUDA, "reading offsets back failed");
+    auto min_nt_of = [&](int64_t o0, int64_t no) { return need_min_nt ? range_min_nt(host_offsets(), o0, no) : INT64_MAX; };
     auto run_objs = [&](int64_t o0, int64_t no, int64_t obs, void* out) -> lsp_status {
         int n_parts = 0;
-        const Schedule sc = make_schedule(p, no, obs, s.kernel);
+        const Schedule sc = make_schedule(p, no, obs, s.kernel, min_nt_of(o0, no));
         const bool cut = s.kernel == LSP_KERNEL_TENSOR &&
                          (size_t)(obs / kTcKB + no) * (size_t)sc.tp.b_stage_bytes > p->tc_table_budget;
         if (!cut) {
@@ -599,7 +631,7 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
                 ++na;
             }
             const int64_t obs_a = ho[a0 + na] - ho[a0];
-            const Schedule sa = make_schedule(p, na, obs_a, s.kernel);
+            const Schedule sa = make_schedule(p, na, obs_a, s.kernel, min_nt_of(a0, na));
             lsp_status e = run_range(p, sa, g, a0, na, obs_a, d_off, d_t, d_y,
                                      out ? (char*)out + (size_t)(a0 - o0) * row_bytes : nullptr, want_best, &n_parts, st);
             if (e != LSP_OK) return e;
@@ -705,6 +737,9 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     if (cfg->tensor_roles < 0 || cfg->tensor_roles > 2) return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_roles must be 0, 1 or 2");
     if (cfg->tensor_b_stages != 0 && (cfg->tensor_b_stages < 2 || cfg->tensor_b_stages > 8))
         return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_b_stages must be 0 or 2..8");
+    if (cfg->tensor_products != 0 && cfg->tensor_products != 2 && cfg->tensor_products != 3)
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_products must be 0, 2 or 3");
+    if (cfg->reserved != 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "reserved must be 0");
     if (cfg->n_copy_streams < 0 || cfg->n_copy_streams > 16 || cfg->chunk_bytes < 0 || cfg->max_objects < 0 || cfg->max_total_obs < 0)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "negative / oversized sizing field");
     int n_dev = 0;
@@ -742,6 +777,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     if (cfg->table_budget_bytes > 0) p->tc_table_budget = (size_t)cfg->table_budget_bytes;
     p->pageable_mode = (cfg->flags & LSP_FLAG_PAGEABLE_STAGED) ? 0 : 1;
     p->tc_roles = cfg->tensor_roles;
+    p->tc_products = cfg->tensor_products == 3 ? 3 : 2;
     if (cfg->tensor_b_stages > 0) p->tc_stages_b = cfg->tensor_b_stages;
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
@@ -800,7 +836,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     if (!p) return LSP_ERR_INVALID_ARG;
     p->n_launches = p->n_pairs = p->n_chunks = 0;
     p->t_used = 0;
-    p->tensor_shape = 0;
+    p->tensor_shape = p->tensor_products = 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
     const int n_best = (d_best_period != nullptr) + (d_best_power != nullptr) + (d_best_index != nullptr);
@@ -843,6 +879,17 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     ++p->n_launches;
 
     Schedule s = make_schedule(p, n_obj, total_obs);
+    if (s.kernel == LSP_KERNEL_TENSOR && s.products == 2) {      // two-product mode: the shortest object decides (kTcMinNtTwoProducts)
+        std::vector<int64_t> off_cache;
+        const int64_t* ho = h_offsets;
+        if (!ho) {
+            off_cache.resize((size_t)n_obj + 1);
+            LSP_CUDA(p, cudaMemcpyAsync(off_cache.data(), d_offsets, off_cache.size() * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+            LSP_CUDA(p, cudaStreamSynchronize(st));
+            ho = off_cache.data();
+        }
+        s = make_schedule(p, n_obj, total_obs, -1, range_min_nt(ho, 0, n_obj));
+    }
     if (s.kernel == LSP_KERNEL_TENSOR &&
         (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget) {
         // the tensor path's operand table of the whole batch does not fit: AUTO falls back to the FMA-pipe kernel
@@ -1030,10 +1077,11 @@ const char* lsp_last_error(const lsp_plan* plan)
 }
 
 void lsp_last_call_info(const lsp_plan* p, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used, int32_t* n_split,
-                        int64_t* n_chunks, int32_t* tensor_shape)
+                        int64_t* n_chunks, int32_t* tensor_shape, int32_t* tensor_products)
 {
     if (!p) return;
     if (tensor_shape) *tensor_shape = p->tensor_shape;
+    if (tensor_products) *tensor_products = p->tensor_products;
     if (n_launches) *n_launches = p->n_launches;
     if (n_pairs) *n_pairs = p->n_pairs;
     if (kernel_used) *kernel_used = p->kernel_used;

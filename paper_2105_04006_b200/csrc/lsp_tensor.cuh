@@ -408,13 +408,19 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
     return w;
 }
 
-// The generators wait on the B ring's "full" barriers out of step with the MMA warp; their parity waits stay within one phase of
-// the barrier only if the ring is at least NG + D stages deep (D = A-ring depth; see the kernel's hand-off protocol).
-constexpr int tc_min_stages_b(bool fast, int ng)
+// Depth D of the A ring in use (stages in flight between the generators and the MMA warp): what the ring's 64 TMEM columns
+// hold (2 stages of 4 planes with three products, else 4 stages of 2 planes), at most one per generator group, and -- the
+// generators wait on the B ring's "full" barriers out of step with the MMA warp, and their parity waits stay within one
+// phase of the barrier only if the B ring is at least NG + D stages deep -- small enough for the 7 four-plane B stages that
+// fit in shared memory at NL = 112 (pm = 2; fast_math stages are half as large).
+__host__ __device__ constexpr int tc_a_depth(int pm, int ng)
 {
-    const int as = kTcACols / (fast ? 16 : 32);
-    return ng + (as < ng ? as : ng);
+    const int as = pm == 0 ? 2 : 4;
+    int d = as < ng ? as : ng;
+    if (pm == 2 && d > 7 - ng) d = 7 - ng;
+    return d;
 }
+__host__ __device__ constexpr int tc_min_stages_b(int pm, int ng) { return ng + tc_a_depth(pm, ng); }
 // ---- split-N_t fix-up (n_split > 1) ----------------------------------------------------------------------------------
 // The n_split partial slots of a tile (lane-oriented un-scaled sums in the epilogue's own element order: element (i, row r)
 // at i * 128 + r, see the epilogue) are added in SPLIT ORDER -- results do not depend on scheduling -- and steps 5, 6, 6'
@@ -522,7 +528,10 @@ template <int EW, int NG> constexpr int tc_static_smem() { return NG * 2 * (8 * 
 
 // GM (generalised mode): 0 = standard; 1 = the W slot carries the weights (partial-sum output); 2 = 1 + ZK09's power fused into
 // the epilogue (n_split = 1).  A template parameter so that the standard kernel carries none of it.
-template <typename T, bool FAST, int EW, int NG, int GM>
+// PM (precision mode): 0 = three products a_hi b_hi + a_hi b_lo + a_lo b_hi; 2 = two products a_hi (b_hi + b_lo) -- the A
+// operand is one FP16 (the generators skip the low part, the A ring is twice as deep), the B table is the same;
+// 1 = fast_math: one product and MUFU sincos.
+template <typename T, int PM, int EW, int NG, int GM>
 __global__ void __launch_bounds__((TcRoles<EW, NG>::kThreads), 1)
 lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
                   const unsigned char* __restrict__ table, T* __restrict__ out_power, Best* __restrict__ partials,
@@ -531,9 +540,11 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     using R = TcRoles<EW, NG>;
     constexpr bool WGT = GM != 0, FUSED = GM == 2;
     constexpr int kEpiWarps = EW, kEpiThreads = R::kEpiThreads;
-    constexpr int NOPS = FAST ? 2 : 4;
-    constexpr int A_STAGE_COLS = NOPS * 8;                    // TMEM columns of one A stage
-    constexpr int AS = kTcACols / A_STAGE_COLS;               // A stages that fit in the ring's columns: 2 (accurate) or 4 (fast)
+    constexpr bool FAST = PM == 1;                            // MUFU sincos, B table without low planes
+    constexpr bool A_LO = PM == 0;                            // the A operand carries a low part
+    constexpr int NOPS = FAST ? 2 : 4;                        // FP16 planes of a B stage
+    constexpr int A_STAGE_COLS = (A_LO ? 4 : 2) * 8;          // TMEM columns of one A stage
+    constexpr int AS = kTcACols / A_STAGE_COLS;               // A stages that fit in the ring's columns: 2 (three products) or 4
     // Hand-off protocol of the A ring.  Stage s (numbered per CTA across items) is built by generator group s % NG into TMEM
     // slot s % D, D = min(AS, NG).  mbarrier waits are parity waits: a waiter must never be two phases away from its barrier,
     // so the "slot is free" signal is kept PER GROUP, not per slot: the commit that follows the MMAs of stage j arrives on
@@ -541,7 +552,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     // sees exactly one arrival per stage it builds (none for its first stage if that is one of the first D), waits for
     // them strictly in order, and arrival i + 1 cannot precede its consumption of arrival i (it needs MMA(s + NG - D), which
     // is issued after MMA(s), which needs this group's stage s).  full_a[slot] is waited on by the MMA warp only, in order.
-    constexpr int D = AS < NG ? AS : NG;
+    constexpr int D = tc_a_depth(PM, NG);
+    static_assert(D >= 1 && D <= AS && D <= NG, "A ring depth");
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem_b = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
     const int SB = tp.stages_b;
@@ -632,7 +644,14 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 if (elect_one()) {
                     // planes (A in TMEM and B in shared memory alike): 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
                     const unsigned a = a0 + (unsigned)(sa * A_STAGE_COLS);
-                    if (!FAST) {
+                    if (PM == 2) {
+                        tc_mma_f16_ts(d_z, a, b_zl0 + sob, idesc, acc);
+                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, 1u);
+                        if (do_w) {
+                            tc_mma_f16_ts(d_w, a + 8, b_wl0 + sob, idesc, acc);
+                            tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, 1u);
+                        }
+                    } else if (!FAST) {
                         tc_mma_f16_ts(d_z, a + 16, b_zh0 + sob, idesc, acc);
                         tc_mma_f16_ts(d_z, a, b_zl0 + sob, idesc, 1u);
                         tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, 1u);
@@ -1000,7 +1019,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 auto pack = [&](const float2 x, unsigned& hi, unsigned& lo) {
                     const __half2 hh = __floats2half2_rn(x.x, x.y);
                     hi = *reinterpret_cast<const unsigned*>(&hh);
-                    if (!FAST) {
+                    if (A_LO) {
                         const float2 r = __ffma2_rn(__half22float2(hh), make_float2(-1.f, -1.f), x);     // one packed op
                         const __half2 ll = __floats2half2_rn(r.x, r.y);
                         lo = *reinterpret_cast<const unsigned*>(&ll);
@@ -1026,7 +1045,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             const unsigned ta = trow + (unsigned)(sa * A_STAGE_COLS);
             tc_st8(ta, zh);
             if (do_w) tc_st8(ta + 8, wh);
-            if (!FAST) {
+            if (A_LO) {
                 tc_st8(ta + 16, zl);
                 if (do_w) tc_st8(ta + 24, wl);
             }

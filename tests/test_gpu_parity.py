@@ -78,13 +78,15 @@ def oracle_full(oracle, w: Workload):
     return oracle.periodogram(w.offsets, w.t, w.y, w.f_min, w.f_max, w.n_freq)
 
 
-# Kernel variants every shape test runs: the tensor kernel in BOTH warp-role shapes (lsp_config.tensor_roles: 1 = short-item
-# shape, 2 = long-item shape), so each template instantiation the scheduler can reach gets full-grid element-wise checks.
-KERNEL_VARIANTS = [("direct", 0), ("factored", 0), ("tensor", 1), ("tensor", 2)]
+# Kernel variants every shape test runs, (kernel, tensor_roles, tensor_products): the tensor kernel in BOTH warp-role shapes
+# (lsp_config.tensor_roles: 1 = short-item shape, 2 = long-item shape) and BOTH accurate precision modes (lsp_config.
+# tensor_products: 2 = the default, 3), so each template instantiation the scheduler can reach gets full-grid element-wise checks.
+KERNEL_VARIANTS = [("direct", 0, 0), ("factored", 0, 0), ("tensor", 1, 2), ("tensor", 2, 2), ("tensor", 1, 3), ("tensor", 2, 3)]
+MIN_NT_TWO_PRODUCTS = 32      # a launch holding a shorter object runs with three products (lsp.h, lsp_last_call_info)
 
 
 def variant_id(v):
-    return v[0] if v[1] == 0 else f"tensor-roles{v[1]}"
+    return v[0] if v[1] == 0 else f"tensor-roles{v[1]}-products{v[2]}"
 
 
 def assert_two_point_pin(P_row, t2, y2, w: Workload, dtype, what=""):
@@ -115,14 +117,14 @@ def test_config1_full_and_best_f64(lsp, oracle, kernel):
 @pytest.mark.parametrize("dtype,fast", [("f64", False), ("f32", False), ("f32", True)])
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS, ids=variant_id)
 def test_config2_shape_small(lsp, oracle, dtype, fast, variant):
-    kernel, roles = variant
-    if kernel == "tensor" and dtype == "f64":
-        pytest.skip("the tensor-core kernel is FP32-mode only")
+    kernel, roles, products = variant
+    if kernel == "tensor" and (dtype == "f64" or (fast and products == 3)):
+        pytest.skip("the tensor-core kernel is FP32-mode only; fast_math has one product")
     # N_t = 1500 spans several observation chunks with a ragged tail; N_f = 9001 spans several tiles with a ragged tail
     w = make_config(2, dtype=dtype, n_t=1500, n_freq=9001)
     P_ref = oracle_full(oracle, w)
-    P, best, info = gpu_full(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles)
-    assert info["tensor_shape"] == roles
+    P, best, info = gpu_full(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles, tensor_products=products)
+    assert info["tensor_shape"] == roles and info["tensor_products"] == (0 if kernel != "tensor" else 1 if fast else products)
     assert_power_parity(P, P_ref, dtype, f"c2s/{kernel}/{dtype}/fast={fast}")
     assert_best_parity(best, P_ref, w, dtype, oracle)
 
@@ -176,16 +178,17 @@ def c2_full_oracle(oracle, dtype):
     return _C2_ORACLE[dtype]
 
 
-@pytest.mark.parametrize("dtype,fast", [("f64", False), ("f32", False), ("f32", True)])
-def test_config2_full_size_full_grid(lsp, oracle, dtype, fast):
+@pytest.mark.parametrize("dtype,fast,products", [("f64", False, 0), ("f32", False, 0), ("f32", False, 3), ("f32", True, 0)])
+def test_config2_full_size_full_grid(lsp, oracle, dtype, fast, products):
     """BASELINE config 2 at full size (N_t = 1e4, N_f = 1e6) in the bench launch configuration, EVERY grid frequency against
     the oracle (SURVEY.md 8(d) "Oracle timing": full grid for C1 and C2), plus best period and the bounds of pin p3."""
     w = make_config(2, dtype=dtype)
     P_ref = c2_full_oracle(oracle, dtype)
-    P, best, info = gpu_full(lsp, w, fast_math=fast)
+    P, best, info = gpu_full(lsp, w, fast_math=fast, tensor_products=products)
     assert info["kernel"] == ("tensor" if dtype == "f32" else "factored")
     if dtype == "f32":
         assert info["tensor_shape"] == 2           # the long-item role shape is the one bench.py times on this config
+        assert info["tensor_products"] == (1 if fast else products or 2)     # default = two products, as bench.py times it
     assert_power_parity(P, P_ref, dtype, f"c2 full {dtype} fast={fast}")
     assert_best_parity(best, P_ref, w, dtype, oracle, "c2 full")
     yy = w.y.astype(np.float64)
@@ -196,16 +199,16 @@ def test_config2_full_size_full_grid(lsp, oracle, dtype, fast):
 
 
 # ---- config 3 shape: batch of short night-clustered objects, best period fused ----------------------------
-@pytest.mark.parametrize("kernel,fast,roles", [("factored", False, 0), ("factored", True, 0), ("direct", True, 0),
-                                               ("tensor", False, 1), ("tensor", True, 1), ("tensor", False, 2),
-                                               ("tensor", True, 2)])
-def test_config3_shape_best_only(lsp, oracle, kernel, fast, roles):
+@pytest.mark.parametrize("kernel,fast,roles,products", [("factored", False, 0, 0), ("factored", True, 0, 0), ("direct", True, 0, 0),
+                                                        ("tensor", False, 1, 2), ("tensor", True, 1, 0), ("tensor", False, 2, 2),
+                                                        ("tensor", True, 2, 0), ("tensor", False, 1, 3), ("tensor", False, 2, 3)])
+def test_config3_shape_best_only(lsp, oracle, kernel, fast, roles, products):
     w = make_config(3, n_obj=24, n_freq=20_011)
     P_ref = oracle_full(oracle, w)
-    best, info = gpu_best(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles)
-    assert info["tensor_shape"] == roles
+    best, info = gpu_best(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles, tensor_products=products)
+    assert info["tensor_shape"] == roles and info["tensor_products"] == (0 if kernel != "tensor" else 1 if fast else products)
     assert_best_parity(best, P_ref, w, "f32", oracle, f"c3s/{kernel}")
-    P, best2, _ = gpu_full(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles)
+    P, best2, _ = gpu_full(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles, tensor_products=products)
     assert_power_parity(P, P_ref, "f32", f"c3s/{kernel}")
     # fused best-only and full+best agree bit for bit
     for a, b in zip(best, best2):
@@ -230,6 +233,33 @@ def test_config3_full_size_sampled_objects(lsp, oracle, fast):
     f_best = 1.0 / best[0].astype(np.float64)
     f_true = 2.0 / (w.meta["rotation_period_h"] / 24.0)
     assert np.mean(np.abs(f_best - f_true) < 0.01) > 0.6
+
+
+def test_tensor_products_error_levels_on_noise_only_objects(lsp, oracle):
+    """The two precision modes of the accurate tensor path on the data that is hardest for them: pure-noise objects (no signal
+    to lift max P above the noise floor), N_t from the 32-observation floor of the two-product mode up to 400.  Two products
+    (generated operand = one FP16) must stay within half the tolerance, three products within a twentieth; a launch that holds
+    a shorter object must fall back to three products by itself."""
+    rng = np.random.Generator(np.random.PCG64(777))
+    lens = np.concatenate([[32, 33, 40, 48, 64], rng.integers(32, 401, 59)])
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    t = np.concatenate([np.sort(rng.uniform(0.0, 365.0, n)) for n in lens]).astype(np.float32)
+    y = np.concatenate([(lambda v: v - v.mean())(rng.normal(0.0, 1.0, n)) for n in lens]).astype(np.float32)
+    w = Workload("noise", off, t, y, 0.02, 12.0, 60_000, "f32")
+    P_ref = oracle_full(oracle, w)
+    worst = {}
+    for products in (2, 3):
+        P, best, info = gpu_full(lsp, w, kernel="tensor", tensor_products=products)
+        assert info["tensor_products"] == products
+        worst[products] = max(np.max(np.abs(P[o] - P_ref[o])) / P_ref[o].max() for o in range(w.n_obj))
+        assert_best_parity(best, P_ref, w, "f32", oracle, f"noise/products={products}")
+    assert worst[2] <= 0.5 * TOL["f32"] and worst[3] <= 0.05 * TOL["f32"], worst
+    short = w.take_objects(np.arange(8))
+    short.offsets[-1] = short.offsets[-2] + 12    # last object: 12 observations
+    short = Workload("noise-short", short.offsets, short.t[:short.offsets[-1]], short.y[:short.offsets[-1]], w.f_min, w.f_max, 9000, "f32")
+    P, _, info = gpu_full(lsp, short, kernel="tensor", tensor_products=2)
+    assert info["tensor_products"] == 3
+    assert_power_parity(P, oracle_full(oracle, short), "f32", "noise-short")
 
 
 # ---- config 4 shape: full periodograms to pinned host memory through the chunk ring -----------------------
@@ -284,7 +314,7 @@ def test_config5_split_path(lsp, oracle, dtype, kernel):
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("variant", KERNEL_VARIANTS, ids=variant_id)
 def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
-    kernel, roles = variant
+    kernel, roles, products = variant
     if kernel == "tensor" and dtype == "f64":
         pytest.skip("the tensor-core kernel is FP32-mode only")
     rng = np.random.default_rng(9)
@@ -296,7 +326,9 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
     np_t = np.float32 if dtype == "f32" else np.float64
     w = Workload("edge", off, t.astype(np_t), y.astype(np_t), 0.05, 3.0, 2500, dtype)
     P_ref = oracle_full(oracle, w)
-    P, best, _ = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles)
+    P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
+    if kernel == "tensor":       # objects of a few observations: the launch runs with three products whatever the plan says
+        assert info["tensor_products"] == 3
     assert np.all(np.isfinite(P))
     assert np.all(P[0] == 0) and np.all(P[5] == 0)
     # N_t = 1 and N_t = 2 hit the singular branch at isolated frequencies: there, finite + bounded only (reading a6) ...
@@ -318,9 +350,10 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
 def test_edge_ragged_grid_sizes(lsp, oracle, n_freq):
     w = make_config(1, n_freq=n_freq, dtype="f32")
     P_ref = oracle_full(oracle, w)
-    for kernel, roles in KERNEL_VARIANTS:
-        P, best, _ = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles)
-        assert_power_parity(P, P_ref, "f32", f"nf={n_freq}/{kernel}")
+    for kernel, roles, products in KERNEL_VARIANTS:
+        P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
+        assert info["tensor_products"] == products
+        assert_power_parity(P, P_ref, "f32", f"nf={n_freq}/{kernel}/{products}")
         assert_best_parity(best, P_ref, w, "f32", oracle)
 
 
@@ -536,13 +569,25 @@ def test_random_shapes_all_kernels(lsp, oracle, seed):
     t = np.concatenate([np.sort(rng.uniform(0.0, 400.0, n)) for n in lens]) if lens.sum() else np.zeros(0)
     y = rng.normal(0.0, 1.0, t.size) + np.sin(2 * np.pi * 1.37 * t)
     f_min, f_max = 0.03, float(rng.uniform(2.0, 9.0))
-    for dtype, kernels in (("f32", (("tensor", 1), ("tensor", 2), ("factored", 0), ("direct", 0))), ("f64", (("factored", 0),))):
+    lens0, off0, t0, y0 = lens, off, t, y
+    # (dtype, kernel variants, shift): the two-product tensor mode only runs when every object has >= 32 observations, so its
+    # variants get the same draw with 32 more observations on every non-empty object (48 = 3 stages exactly, 49, 63, ...)
+    for dtype, kernels, shift in (("f32", (("tensor", 1, 3), ("tensor", 2, 3), ("factored", 0, 0), ("direct", 0, 0)), 0),
+                                  ("f32", (("tensor", 1, 2), ("tensor", 2, 2)), MIN_NT_TWO_PRODUCTS), ("f64", (("factored", 0, 0),), 0)):
+        if shift:
+            lens = np.where(lens0 > 0, lens0 + shift, 0)
+            off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+            rng2 = np.random.Generator(np.random.PCG64(19000 + seed))
+            t = np.concatenate([np.sort(rng2.uniform(0.0, 400.0, n)) for n in lens])
+            y = rng2.normal(0.0, 1.0, t.size) + np.sin(2 * np.pi * 1.37 * t)
+        else:
+            lens, off, t, y = lens0, off0, t0, y0
         w = Workload(f"rand{seed}", off, t.astype(np.float32 if dtype == "f32" else np.float64),
                      y.astype(np.float32 if dtype == "f32" else np.float64), f_min, f_max, n_freq, dtype=dtype)
         P_ref = oracle_full(oracle, w)
-        for kernel, roles in kernels:
-            P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles)
-            assert info["tensor_shape"] == roles
+        for kernel, roles, products in kernels:
+            P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
+            assert info["tensor_shape"] == roles and info["tensor_products"] == products
             for o in range(n_obj):
                 if lens[o] == 0:
                     assert np.all(P[o] == 0.0)
