@@ -83,7 +83,9 @@ typedef struct lsp_config {
                                    2 (= 0, default): a_hi (b_hi + b_lo) -- the generated operand a = y e^{i alpha} is
                                    one FP16 (11 significand bits), the tabulated one an FP16 pair (22 bits);
                                    3: a_hi b_hi + a_hi b_lo + a_lo b_hi -- both operands FP16 pairs                 */
-    int32_t reserved;       /* must be 0                                                                   */
+    int32_t tensor_pair;    /* tensor path: CTA pairs (2-CTA clusters, tcgen05 cta_group::2: two frequency tiles of one
+                                   object share every tabulated-operand stage).  0 = when work items are long (>= 48
+                                   stages of 16 observations), 1 = never, 2 = whenever the grid has >= 2 tiles         */
 } lsp_config;
 
 /* lsp_config.flags */
@@ -96,7 +98,7 @@ typedef struct lsp_config {
  * allocates scratch (argmax partials, split-N_t partial sums, the device chunk ring for host output).
  * The plan owns all of that; the caller owns every buffer passed to the calls below.
  * Errors: LSP_ERR_INVALID_ARG (f_min <= 0, f_max <= f_min, n_freq < 1, fast_math with FP64, unknown
- * enum or flag bit, tensor_roles / tensor_b_stages / tensor_products out of range, reserved != 0), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
+ * enum or flag bit, tensor_roles / tensor_b_stages / tensor_products / tensor_pair out of range), LSP_ERR_CUDA (no device / runtime failure), LSP_ERR_OOM.  *out_plan is NULL on
  * failure.  A plan is not thread-safe; distinct plans are independent.
  */
 lsp_status lsp_plan_create(const lsp_config* cfg /* HOST */, lsp_plan** out_plan /* HOST */);
@@ -212,7 +214,7 @@ const char* lsp_last_error(const lsp_plan* plan);
 /* Bookkeeping of the LAST call on the plan, for benchmarks and tests: how many of the library's kernels it launched,
  * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), -- host-output
  * calls only -- chunks copied, the tensor kernel's warp-role shape (0 = tensor kernel not used, 1 = short-item
- * shape, 2 = long-item shape; see lsp_config.tensor_roles) and its FP16 products per multiply-accumulate in the last
+ * shape, 2 = long-item shape, 3 = long-item shape on CTA pairs; see lsp_config.tensor_roles, tensor_pair) and its FP16 products per multiply-accumulate in the last
  * launch (0 = tensor kernel not used; 1 = fast_math; 2 or 3: lsp_config.tensor_products -- a launch that holds an object
  * of fewer than 32 observations runs with 3 whatever the plan says).  Any pointer may be NULL. */
 void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used,

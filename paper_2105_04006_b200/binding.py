@@ -38,7 +38,7 @@ class LspConfig(ctypes.Structure):
         ("chunk_bytes", ctypes.c_int64), ("max_objects", ctypes.c_int64), ("max_total_obs", ctypes.c_int64),
         ("kernel", ctypes.c_int32), ("flags", ctypes.c_int32),
         ("table_budget_bytes", ctypes.c_int64), ("tensor_roles", ctypes.c_int32), ("tensor_b_stages", ctypes.c_int32),
-        ("tensor_products", ctypes.c_int32), ("reserved", ctypes.c_int32),
+        ("tensor_products", ctypes.c_int32), ("tensor_pair", ctypes.c_int32),
     ]
 
 
@@ -168,14 +168,14 @@ class Plan:
                  normalize: bool = False, center: bool = False, device: int = 0, n_copy_streams: int = 0,
                  chunk_bytes: int = 0, kernel: str = "auto", max_objects: int = 0, max_total_obs: int = 0,
                  pageable_staged: bool = False, table_budget_bytes: int = 0, tensor_roles: int = 0,
-                 tensor_b_stages: int = 0, tensor_products: int = 0):
+                 tensor_b_stages: int = 0, tensor_products: int = 0, tensor_pair: int = 0):
         if dtype not in ("f32", "f64"):
             raise ValueError("dtype must be 'f32' or 'f64'")
         self.cfg = LspConfig(float(f_min), float(f_max), int(n_freq), LSP_F32 if dtype == "f32" else LSP_F64,
                              int(fast_math), int(normalize), int(center), int(device), int(n_copy_streams),
                              int(chunk_bytes), int(max_objects), int(max_total_obs), _KERNELS[kernel],
                              LSP_FLAG_PAGEABLE_STAGED if pageable_staged else 0, int(table_budget_bytes),
-                             int(tensor_roles), int(tensor_b_stages), int(tensor_products), 0)
+                             int(tensor_roles), int(tensor_b_stages), int(tensor_products), int(tensor_pair))
         self.dtype = dtype
         self.torch_dtype = torch.float32 if dtype == "f32" else torch.float64
         self.n_freq = int(n_freq)

@@ -60,6 +60,7 @@ struct lsp_plan {
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     int tc_stages_b = 0;          // B-operand ring depth of the tensor kernel; 0 = as many as fit (cfg.tensor_b_stages)
     int tc_products = 2;          // FP16 products per MAC of the accurate tensor mode: 2 or 3 (cfg.tensor_products)
+    int tc_pair = 0;              // CTA pairs on the tensor path: 0 = when items are long, 1 = never, 2 = whenever there are >= 2 tiles (cfg.tensor_pair)
     int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
     DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
@@ -135,19 +136,27 @@ cudaError_t optin_smem(lsp_plan* p, K kern, size_t bytes)
 
 // Launch with programmatic stream serialisation: the kernel may start while its predecessor on the stream drains; it must
 // execute griddepcontrol.wait (pdl_wait in lsp_tensor.cuh) before reading what the predecessor wrote.
+// `cluster` > 1 launches thread-block clusters of that many CTAs (the tensor kernel's CTA pairs).
 template <typename... KArgs, typename... Args>
-cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args... args)
+cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, int cluster, Args... args)
 {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(block);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
     cfg.numAttrs = 1;
+    if (cluster > 1) {
+        attr[1].id = cudaLaunchAttributeClusterDimension;
+        attr[1].val.clusterDim.x = (unsigned)cluster;
+        attr[1].val.clusterDim.y = 1;
+        attr[1].val.clusterDim.z = 1;
+        cfg.numAttrs = 2;
+    }
+    cfg.attrs = attr;
     return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
@@ -187,7 +196,8 @@ int64_t range_min_nt(const int64_t* ho, int64_t o0, int64_t no)
     return m;
 }
 
-Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int kernel_override = -1, int64_t min_nt = INT64_MAX)
+Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int kernel_override = -1, int64_t min_nt = INT64_MAX,
+                       bool allow_pair = true)
 {
     const lsp_config& c = p->cfg;
     Schedule s{};
@@ -196,19 +206,21 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
         k = (c.n_freq < 1024) ? LSP_KERNEL_DIRECT : (c.dtype == LSP_F32 ? LSP_KERNEL_TENSOR : LSP_KERNEL_FACTORED);
     s.kernel = k;
     int64_t slots;                                                // resident CTAs on the whole GPU
-    if (k == LSP_KERNEL_TENSOR) {
-        // tiles of 64 groups x 2 NL frequencies, NL the smallest multiple of 8 that covers N_f with the fewest tiles
-        const int64_t max_tile = (int64_t)kTcGroups * 2 * kTcMaxNL;
-        const int64_t nt = (c.n_freq + max_tile - 1) / max_tile;
+    // tensor path: tiles of 64 groups x 2 NL frequencies, NL the smallest multiple of 8 that covers N_f with `nt` tiles
+    int64_t max_nl = kTcMaxNL;
+    int64_t max_tile = (int64_t)kTcGroups * 2 * max_nl;
+    auto tensor_tiles = [&](int64_t nt) {
         int64_t nl = (c.n_freq + nt * 2 * kTcGroups - 1) / (nt * 2 * kTcGroups);
-        nl = std::min<int64_t>(kTcMaxNL, std::max<int64_t>(8, (nl + 7) / 8 * 8));
+        nl = std::min<int64_t>(max_nl, std::max<int64_t>(8, (nl + 7) / 8 * 8));
         s.tp.nl = (int)nl;
         s.tp.tile = (int)(kTcGroups * 2 * nl);
+        s.tile = s.tp.tile;
+        s.n_tiles = (int)((c.n_freq + s.tile - 1) / s.tile);
+    };
+    if (k == LSP_KERNEL_TENSOR) {
+        tensor_tiles((c.n_freq + max_tile - 1) / max_tile);
         s.tp.n_ops = c.fast_math ? 2 : 4;
         s.products = c.fast_math ? 1 : ((p->tc_products == 3 || min_nt < kTcMinNtTwoProducts) ? 3 : 2);
-        s.tp.b_plane_bytes = 2 * (int)nl * kTcKB * 2;
-        s.tp.b_stage_bytes = s.tp.n_ops * s.tp.b_plane_bytes + kTcAuxBytes;
-        s.tile = s.tp.tile;
         s.direct_r = 0;
         slots = p->sm_count;
     } else if (k == LSP_KERNEL_FACTORED) {
@@ -221,44 +233,78 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
         s.tile = s.direct_r * kDirectThreads;
         slots = (int64_t)p->sm_count * (s.direct_r == 4 ? (c.dtype == LSP_F32 ? 4 : 3) : 8);
     }
-    s.n_tiles = (int)((c.n_freq + s.tile - 1) / s.tile);
+    if (k != LSP_KERNEL_TENSOR) s.n_tiles = (int)((c.n_freq + s.tile - 1) / s.tile);
     // Split the observations of every object when (object, tile) items alone cannot fill the GPU for a few
     // waves (large-N_t / small-N_f problems; PAPER.md:L373, L396 describe the under-filled GPU).  Among the
     // admissible split counts pick the one whose last wave is fullest (wave quantisation), then the smallest.
-    const int64_t items = std::max<int64_t>(1, n_obj * s.n_tiles);
-    int64_t split = 1;
-    if (items < 8 * slots && n_obj > 0) {
-        const int64_t avg_nt = total_obs / std::max<int64_t>(1, n_obj);
-        const int64_t min_obs = (k == LSP_KERNEL_TENSOR) ? 256 : (k == LSP_KERNEL_FACTORED) ? 128 : 64;   // per split, to amortise prologue/epilogue
-        const int64_t s_max = std::max<int64_t>(1, std::min<int64_t>(64, avg_nt / min_obs));
-        double best_score = -1.0;
-        for (int64_t cand = 1; cand <= s_max; ++cand) {
-            const double waves = (double)(items * cand) / (double)slots;
-            const double eff = waves / std::ceil(waves);               // occupancy of the average wave
-            const double score = eff - 0.004 * (double)(cand - 1);     // each split adds a partial-sum pass
-            if (score > best_score + 1e-9) { best_score = score; split = cand; }
-            if (waves >= 8.0) break;
+    const int64_t avg_nt = total_obs / std::max<int64_t>(1, n_obj);
+    auto choose_split = [&](int64_t items, int64_t n_slots) {
+        int64_t split = 1;
+        if (items < 8 * n_slots && n_obj > 0) {
+            const int64_t min_obs = (k == LSP_KERNEL_TENSOR) ? 256 : (k == LSP_KERNEL_FACTORED) ? 128 : 64;   // per split, to amortise prologue/epilogue
+            const int64_t s_max = std::max<int64_t>(1, std::min<int64_t>(64, avg_nt / min_obs));
+            double best_score = -1.0;
+            for (int64_t cand = 1; cand <= s_max; ++cand) {
+                const double waves = (double)(items * cand) / (double)n_slots;
+                const double eff = waves / std::ceil(waves);               // occupancy of the average wave
+                const double score = eff - 0.004 * (double)(cand - 1);     // each split adds a partial-sum pass
+                if (score > best_score + 1e-9) { best_score = score; split = cand; }
+                if (waves >= 8.0) break;
+            }
         }
-    }
-    if (k == LSP_KERNEL_TENSOR && n_obj > 0) {
-        // The tensor cores add into their FP32 accumulators with truncation: the bias grows with the number of accumulations
-        // (measured ~3e-8 of the sum per 16-observation stage).  Items are capped at 1024 stages so it stays below 1e-4 of max P.
-        const int64_t nkb_avg = (total_obs / n_obj + kTcKB - 1) / kTcKB;
-        split = std::max<int64_t>(split, (nkb_avg + 1023) / 1024);
-    }
-    s.n_split = (int)split;
+        if (k == LSP_KERNEL_TENSOR && n_obj > 0) {
+            // The tensor cores add into their FP32 accumulators with truncation: the bias grows with the number of accumulations
+            // (measured ~3e-8 of the sum per 16-observation stage).  Items are capped at 1024 stages so it stays below 1e-4 of max P.
+            const int64_t nkb_avg = (avg_nt + kTcKB - 1) / kTcKB;
+            split = std::max<int64_t>(split, (nkb_avg + 1023) / 1024);
+        }
+        return split;
+    };
+    int64_t split = choose_split(std::max<int64_t>(1, n_obj * s.n_tiles), slots);
     if (k == LSP_KERNEL_TENSOR) {
         // role shape by item length: stages (16 observations) per work item
-        const int64_t avg_nt = n_obj > 0 ? total_obs / n_obj : 0;
-        const int64_t stages_per_item = (avg_nt / kTcKB) / std::max<int64_t>(1, split);
+        int64_t stages_per_item = (avg_nt / kTcKB) / std::max<int64_t>(1, split);
         s.tp.long_items = (p->tc_roles == 0) ? (stages_per_item >= 48 ? 1 : 0) : (p->tc_roles == 2 ? 1 : 0);
+        // CTA pairs (cta_group::2; the long-item shape only): an item is a pair of tiles, one per CTA of a 2-CTA cluster, which
+        // share every B stage (each CTA holds half of its columns).  Halves the shared-memory traffic per MMA, which bounds
+        // the unpaired kernel; taken when the items stay long on half as many (twice as wide) scheduling slots.
+        s.tp.pair = 0;
+        if (allow_pair && p->tc_pair != 1 && s.n_tiles >= 2 && p->sm_count >= 2 && n_obj > 0 && (p->tc_pair == 2 || p->tc_roles != 1)) {
+            const Schedule q = s;                                 // the unpaired schedule, restored if the paired one is rejected
+            max_nl = kTcPairMaxNL;                                // narrower tiles: tensor-memory columns for a deeper A ring
+            max_tile = (int64_t)kTcGroups * 2 * max_nl;
+            const int64_t nt0 = (c.n_freq + max_tile - 1) / max_tile;
+            tensor_tiles(nt0);
+            if ((nt0 & 1) && nt0 > 1) {                           // an even tile count wastes no phantom tile: take it if NL shrinks
+                const int nl0 = s.tp.nl;
+                tensor_tiles(nt0 + 1);
+                if (s.tp.nl >= nl0 || (s.n_tiles & 1)) tensor_tiles(nt0);
+            }
+            const int64_t n_tp = (s.n_tiles + 1) / 2;
+            const int64_t split_p = choose_split(std::max<int64_t>(1, n_obj * n_tp), p->sm_count / 2);
+            const int64_t stages_p = (avg_nt / kTcKB) / std::max<int64_t>(1, split_p);
+            if (p->tc_pair == 2 || stages_p >= 48) {
+                s.tp.pair = 1;
+                s.tp.long_items = 1;
+                split = split_p;
+            } else {
+                s = q;
+            }
+        }
+        s.tp.b_plane_bytes = (s.tp.pair ? 1 : 2) * s.tp.nl * kTcKB * 2;
+        s.tp.b_stage_bytes = s.tp.n_ops * 2 * s.tp.nl * kTcKB * 2 + kTcAuxBytes;
+        s.tp.smem_stage_bytes = s.tp.n_ops * s.tp.b_plane_bytes + kTcAuxBytes;
         // B ring (TMA -> MMA; the generators read its aux blocks): as deep as shared memory allows, at most 8 stages
-        const int reserve = (s.tp.long_items ? tc_static_smem<4, 4>() : tc_static_smem<8, 3>()) + (int)tc_smem_bytes(0, 0) + 512;
-        const int fit = (int)std::max<int64_t>(2, std::min<int64_t>(8, (int64_t)(p->smem_optin - reserve) / s.tp.b_stage_bytes));
-        const int need = tc_min_stages_b(s.products == 1 ? 1 : (s.products == 3 ? 0 : 2), s.tp.long_items ? 4 : 3);       // always <= fit for NL <= 112
+        const int ng = s.tp.pair ? kTcPairNG : (s.tp.long_items ? 4 : 3), ew = s.tp.long_items ? 4 : 8;
+        const int reserve = tc_static_smem_of(ew, ng) + (int)tc_smem_bytes(0, 0) + 512;
+        const int fit = (int)std::max<int64_t>(2, std::min<int64_t>(kTcMaxSB, (int64_t)(p->smem_optin - reserve) / s.tp.smem_stage_bytes));
+        // the kernel's A-ring depth is a compile-time function of its largest tile; smaller tiles only leave more room
+        const int need = ng + tc_a_depth(s.products == 1 ? 1 : (s.products == 3 ? 0 : 2), ew, ng, s.tp.pair != 0,
+                                         s.tp.pair ? kTcPairMaxNL : kTcMaxNL);
         s.tp.stages_b = std::max(need, p->tc_stages_b > 0 ? std::min(p->tc_stages_b, fit) : fit);
         s.tp.fixup = split > 1 ? 1 : 0;
     }
+    s.n_split = (int)split;
     return s;
 }
 
@@ -273,16 +319,19 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
     if (grid > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (s.kernel == LSP_KERNEL_TENSOR) {
         if constexpr (std::is_same<T, float>::value) {
-            const size_t smem = tc_smem_bytes(s.tp.stages_b, s.tp.b_stage_bytes);
-            const unsigned ctas = (unsigned)std::min<int64_t>(grid, p->sm_count);
+            const size_t smem = tc_smem_bytes(s.tp.stages_b, s.tp.smem_stage_bytes);
+            // pair mode: an item is (object, pair of tiles, split), one 2-CTA cluster per item slot
+            const int64_t items = s.tp.pair ? n_obj_launch * ((s.n_tiles + 1) / 2) * s.n_split : grid;
+            const unsigned ctas = s.tp.pair ? 2u * (unsigned)std::min<int64_t>(items, p->sm_count / 2)
+                                            : (unsigned)std::min<int64_t>(items, p->sm_count);
             auto go = [&](auto kern, int threads) -> cudaError_t {
                 const cudaError_t ea = optin_smem(p, kern, smem);
                 if (ea != cudaSuccess) return ea;
-                return launch_pdl(kern, ctas, (unsigned)threads, smem, st, gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
-                                  (const unsigned char*)p->tc_table.ptr, (float*)out, partials, (float4*)sums, n_obj_launch, (long long)grid,
+                return launch_pdl(kern, ctas, (unsigned)threads, smem, st, s.tp.pair ? 2 : 1, gp, s.tp, d_off, (const TensorObj*)p->tc_objs.ptr,
+                                  (const unsigned char*)p->tc_table.ptr, (float*)out, partials, (float4*)sums, n_obj_launch, (long long)items,
                                   gls_yy);
             };
-            p->tensor_shape = s.tp.long_items ? 2 : 1;
+            p->tensor_shape = s.tp.pair ? 3 : (s.tp.long_items ? 2 : 1);
             p->tensor_products = s.products;
             // precision mode of the kernel template: 1 = fast_math, 2 = two products (default), 0 = three (tensor_products = 3)
             auto go_pm = [&](auto pm_tag) -> cudaError_t {
@@ -293,6 +342,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
                 if (s.tp.weighted)                       // generalised mode: the W slot carries the weights
                     return s.tp.long_items ? go(lsp_tensor_kernel<float, PM, 4, 4, 1>, TcRoles<4, 4>::kThreads)
                                            : go(lsp_tensor_kernel<float, PM, 8, 3, 1>, TcRoles<8, 3>::kThreads);
+                if (s.tp.pair) return go(lsp_tensor_kernel<float, PM, 4, kTcPairNG, 0, true, kTcPairMaxNL>, TcRoles<4, kTcPairNG>::kThreads);
                 return s.tp.long_items ? go(lsp_tensor_kernel<float, PM, 4, 4, 0>, TcRoles<4, 4>::kThreads)
                                        : go(lsp_tensor_kernel<float, PM, 8, 3, 0>, TcRoles<8, 3>::kThreads);
             };
@@ -455,7 +505,7 @@ lsp_status run_range(lsp_plan* p, const Schedule& s_in, const GridSpec& g, int64
         // tensor path: add the splits' partial slots in split order and finish the tiles (steps 5, 6, 6')
         const int64_t grid = n_obj_launch * (int64_t)s.n_tiles * kTcFixParts;
         if (grid > 0x7fffffffLL) return fail(p, LSP_ERR_INVALID_ARG, "batch too large for one launch");
-        LSP_CUDA(p, launch_pdl(lsp_tensor_fix_kernel<float>, (unsigned)grid, (unsigned)kTcFixThreads, 0, st, gp, s.tp, d_off,
+        LSP_CUDA(p, launch_pdl(lsp_tensor_fix_kernel<float>, (unsigned)grid, (unsigned)kTcFixThreads, 0, st, 1, gp, s.tp, d_off,
                                (const TensorObj*)p->tc_objs.ptr, (const float4*)sums, (float*)out, partials, n_obj_launch));
         LSP_CUDA(p, cudaGetLastError());
         ++p->n_launches;
@@ -739,7 +789,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_b_stages must be 0 or 2..8");
     if (cfg->tensor_products != 0 && cfg->tensor_products != 2 && cfg->tensor_products != 3)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_products must be 0, 2 or 3");
-    if (cfg->reserved != 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "reserved must be 0");
+    if (cfg->tensor_pair < 0 || cfg->tensor_pair > 2) return fail(nullptr, LSP_ERR_INVALID_ARG, "tensor_pair must be 0, 1 or 2");
     if (cfg->n_copy_streams < 0 || cfg->n_copy_streams > 16 || cfg->chunk_bytes < 0 || cfg->max_objects < 0 || cfg->max_total_obs < 0)
         return fail(nullptr, LSP_ERR_INVALID_ARG, "negative / oversized sizing field");
     int n_dev = 0;
@@ -778,6 +828,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     p->pageable_mode = (cfg->flags & LSP_FLAG_PAGEABLE_STAGED) ? 0 : 1;
     p->tc_roles = cfg->tensor_roles;
     p->tc_products = cfg->tensor_products == 3 ? 3 : 2;
+    p->tc_pair = cfg->tensor_pair;
     if (cfg->tensor_b_stages > 0) p->tc_stages_b = cfg->tensor_b_stages;
     const int n_slots = p->cfg.n_copy_streams + 1;
     for (int i = 0; i < p->cfg.n_copy_streams; ++i) {
@@ -878,7 +929,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     LSP_CUDA(p, cudaGetLastError());
     ++p->n_launches;
 
-    Schedule s = make_schedule(p, n_obj, total_obs);
+    Schedule s = make_schedule(p, n_obj, total_obs, -1, INT64_MAX, false);      // (the generalised passes run unpaired)
     if (s.kernel == LSP_KERNEL_TENSOR && s.products == 2) {      // two-product mode: the shortest object decides (kTcMinNtTwoProducts)
         std::vector<int64_t> off_cache;
         const int64_t* ho = h_offsets;
@@ -888,7 +939,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
             LSP_CUDA(p, cudaStreamSynchronize(st));
             ho = off_cache.data();
         }
-        s = make_schedule(p, n_obj, total_obs, -1, range_min_nt(ho, 0, n_obj));
+        s = make_schedule(p, n_obj, total_obs, -1, range_min_nt(ho, 0, n_obj), false);
     }
     if (s.kernel == LSP_KERNEL_TENSOR &&
         (size_t)(total_obs / kTcKB + n_obj) * (size_t)s.tp.b_stage_bytes > p->tc_table_budget) {

@@ -16,8 +16,9 @@
 // per 128-cycle MMA plus the generators' operand stores plus the TMA fills):
 //   A operands (tile dependent, generated on the fly) are written by the generator warps STRAIGHT INTO TENSOR MEMORY
 //               (tcgen05.st) and the MMAs read them from there (A-from-TMEM form of tcgen05.mma): no shared-memory store,
-//               no shared-memory read, no proxy fence.  TMEM columns: Z accumulators [0, 2NL), W accumulators
-//               [224, 224 + 2NL), A ring [448, 512) = 2 stages x 4 planes x 8 columns (fast_math: 4 stages x 2 planes).
+//               no shared-memory read, no proxy fence.  TMEM columns (MNL = the instantiation's largest NL, 112 or 104): Z
+//               accumulators [0, 2NL), W accumulators [2 MNL, 2 MNL + 2NL), A ring [4 MNL, 512) in stages of 2 planes x 8
+//               columns (4 planes with three products).
 //   B operands  e^{i beta}, e^{2 i beta} depend on (object, observation, m) only -- not on the tile -- so one pre-pass launch
 //               (lsp_tensor_prepass_kernel) writes them once per object into a table already laid out as shared-memory
 //               stages; warp 0 streams the stages in with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx).
@@ -52,11 +53,17 @@ constexpr int kTcKB = 16;                      // observations per MMA / ring st
 #ifndef LSP_TC_MAX_NL
 #define LSP_TC_MAX_NL 112
 #endif
-constexpr int kTcMaxNL = LSP_TC_MAX_NL;        // N = 2 NL <= 224: leaves 64 TMEM columns for the A ring (104: 96 columns)
-constexpr int kTcWCol = 2 * kTcMaxNL;          // first TMEM column of the W accumulators
-constexpr int kTcACol = 4 * kTcMaxNL;          // first TMEM column of the A-operand ring
-constexpr int kTcACols = 512 - kTcACol;        // its width
+constexpr int kTcMaxNL = LSP_TC_MAX_NL;        // N = 2 NL <= 224: leaves 64 TMEM columns for the A ring
+#ifndef LSP_TC_PAIR_MAX_NL
+#define LSP_TC_PAIR_MAX_NL 112
+#endif
+constexpr int kTcPairMaxNL = LSP_TC_PAIR_MAX_NL;   // largest NL of the pair-mode kernel (104 would leave 96 columns = a 6-stage A ring)
 constexpr int kTcPreThreads = 128;             // threads of a pre-pass block
+constexpr int kTcMaxSB = 12;                   // deepest B ring (barrier arrays are sized for it)
+#ifndef LSP_TC_PAIR_NG
+#define LSP_TC_PAIR_NG 4
+#endif
+constexpr int kTcPairNG = LSP_TC_PAIR_NG;      // generator groups of the pair-mode kernel
 // aux block of a table stage (floats): t[16], y[16], w[16], then 16 phasor rows of 16 complex values (+ 4 floats of padding
 // per row: 144-byte rows keep the LDS.128 of lanes that read different rows conflict-free).  Rows 0-7: v_g1 = e^{2 pi i (8 g1 L df) t_j};
 // rows 8-15: v_g1 e^{-i pi/4}, the version the "Im a" rows use (see the generators).  Inside a row the 16 phasors are stored
@@ -78,9 +85,12 @@ template <int EW, int NG> struct TcRoles {
     static constexpr int kEpiThreads = EW * 32;
     static constexpr int kGenGroupThreads = 128;
     static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8;
-    static constexpr int kCtrlRegs = 40, kGenRegs = 72;
+    // long-item shape: the generators are the critical role (they keep a stage's tile-independent phasors in registers while
+    // the tile's own are still being evaluated); its epilogue runs once per few hundred stages
+    static constexpr int kCtrlRegs = NG >= 4 ? 32 : 40, kGenRegs = NG == 4 ? 88 : 72;
     static constexpr int kEpiRegs = ((kLaunchRegs * kThreads - 128 * kCtrlRegs - 4 * NG * 32 * kGenRegs) / kEpiThreads) / 8 * 8;
-    static_assert(EW % 4 == 0 && kThreads <= 1024 && kGenRegs <= kLaunchRegs && kEpiRegs >= 96 && kEpiRegs <= 255, "role split");
+    static_assert(EW % 4 == 0 && kThreads <= 1024 && kCtrlRegs <= kLaunchRegs && kEpiRegs >= 96 && kEpiRegs <= 255 &&
+                  128 * kCtrlRegs + 4 * NG * 32 * kGenRegs + kEpiThreads * kEpiRegs <= kLaunchRegs * kThreads, "role split");
 };
 
 struct TensorParams {
@@ -89,8 +99,12 @@ struct TensorParams {
     int n_ops;          // FP16 operand planes per stage side: 4 (accurate: hi and lo of Z- and W-operands) or 2 (fast)
     int stages_b;       // B-operand ring depth (TMA -> MMA)
     int long_items;     // 1: many stages per item -> the (4 epilogue warps, 4 generator groups) shape; 0: (8, 3)
-    int b_plane_bytes;  // 2 NL * 32
-    int b_stage_bytes;  // n_ops * b_plane_bytes + kTcAuxBytes
+    int b_plane_bytes;  // bytes of one FP16 plane of a B stage in a CTA's shared memory: 2 NL * 32 (pair mode: NL * 32, the CTA's half)
+    int b_stage_bytes;  // bytes of one stage of the TABLE: n_ops * 2 NL * 32 + kTcAuxBytes
+    int smem_stage_bytes;   // bytes of one B stage in a CTA's ring: n_ops * b_plane_bytes + kTcAuxBytes
+    int pair;           // 1: CTA pairs (2-CTA clusters, tcgen05 cta_group::2): an item is (object, PAIR of tiles, split), CTA rank r
+                        // takes tile 2 q + r and holds columns [r NL, (r + 1) NL) of every B plane (the "Re b" / "Im b" half);
+                        // the table stage is laid out [half 0][half 1][aux]
     int fixup;          // n_split > 1: 1 = partial slots in the epilogue's own order, finished by lsp_tensor_fix_kernel;
                         // 0 = partial sums per grid frequency (generalised mode)
     int weighted;       // generalised mode: the W operand carries the weights w_j (aux.w) instead of 1
@@ -228,8 +242,9 @@ lsp_tensor_prepass_kernel(GridParams gp, TensorParams tp, const int64_t* __restr
     if (kb >= tc_n_kb(n_t)) return;                 // slack block between two objects
     unsigned char* stage = table + (size_t)blk * (size_t)tp.b_stage_bytes;
     const int L = 2 * tp.nl;
+    const int full_plane_bytes = L * kTcKB * 2;                     // one FP16 plane of all 2 NL columns
     {   // aux: t, y, w of the 16 observations and the tile-independent phasors v (two versions)
-        float* aux = reinterpret_cast<float*>(stage + (size_t)tp.n_ops * tp.b_plane_bytes);
+        float* aux = reinterpret_cast<float*>(stage + (size_t)tp.n_ops * full_plane_bytes);
         const int j16 = tid & 15, g1 = tid >> 4;
         const int64_t j = (int64_t)kb * kTcKB + j16;
         const bool live = j < n_t;
@@ -254,8 +269,11 @@ lsp_tensor_prepass_kernel(GridParams gp, TensorParams tp, const int64_t* __restr
     const int m = tid;
     if (m >= tp.nl) return;
     const double f_beta = ((double)m + 0.5) * gp.df;
-    const int n_cols = L;
-    const int plane = tp.b_plane_bytes / 2;                         // halfs per plane
+    // unpaired: [plane][k chunk c][column n < 2 NL][8];  pair mode: [half r][plane][k chunk c][column n' < NL][8], half 0 = the
+    // "Re b" columns, half 1 = the "Im b" columns (what CTA rank r of a pair holds)
+    const int n_cols = tp.pair ? tp.nl : L;                         // columns of one plane as stored
+    const int plane = n_cols * kTcKB;                               // halfs per stored plane
+    const size_t im_base = tp.pair ? (size_t)tp.n_ops * plane : (size_t)tp.nl * 8;     // where the "Im b" columns start
     __half* dst = reinterpret_cast<__half*>(stage);
     float c1[kTcKB], s1[kTcKB];
 #pragma unroll
@@ -283,7 +301,7 @@ lsp_tensor_prepass_kernel(GridParams gp, TensorParams tp, const int64_t* __restr
             split_half2(ss0, ss1, &im2_h[p], &im2_l[p]);
         }
         const size_t off_re = (size_t)c * (n_cols * 8) + (size_t)m * 8;            // [c][n/8][n%8][8] == [c][n][8]
-        const size_t off_im = (size_t)c * (n_cols * 8) + (size_t)(tp.nl + m) * 8;
+        const size_t off_im = off_re + im_base;
         auto put = [&](int pl, size_t off, const __half2* v) {
             uint4 u;
             u.x = *reinterpret_cast<const unsigned*>(&v[0]);
@@ -324,6 +342,45 @@ __device__ __forceinline__ void tc_mma_f16_ts(unsigned d_tmem, unsigned a_tmem, 
 __device__ __forceinline__ void tc_commit(unsigned long long* bar)
 {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// ---- CTA pairs (2-CTA clusters, cta_group::2): the leader (cluster rank 0) issues every MMA for both CTAs; M = 256 = the 128
+// A rows each CTA generated into its own tensor memory, N = the two CTAs' halves of B side by side; each CTA accumulates its
+// own 128 x N tile in its own tensor memory.
+__device__ __forceinline__ unsigned cluster_ctarank()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of the same variable in CTA `rank` of the cluster
+__device__ __forceinline__ unsigned cluster_map(unsigned saddr, unsigned rank)
+{
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(unsigned cluster_addr)
+{
+    // default semantics (release at CTA scope), as a local arrive: what crosses the pair is tensor-memory / async-proxy state,
+    // ordered by the tcgen05 fences around it; a cluster-scope release would cost a MEMBAR.ALL.GPU per arrival
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void tc_mma_f16_ts2(unsigned d_tmem, unsigned a_tmem, uint64_t b_desc, unsigned idesc, unsigned accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrives (once the MMAs issued so far have completed) on the barrier at this shared-memory offset in BOTH CTAs of the pair
+__device__ __forceinline__ void tc_commit2(unsigned long long* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(smem_u32(bar)), "h"((unsigned short)3) : "memory");
 }
 // mbarrier wait for roles whose waits are long when they are not the bottleneck (generators on a full ring, epilogue on
 // unfinished accumulators): back off between polls so the spinning warps do not take issue slots from the working ones.
@@ -390,15 +447,23 @@ __device__ __forceinline__ void tma_bulk_g2s(void* smem_dst, const void* gmem_sr
 struct TcItem {
     int64_t obj_local, obj, n_t, K0;
     int tile, split, kb0, kb1;
+    bool tile_ok;       // false: the phantom second tile of the last pair of an odd tile count (pair mode): computed, never stored
 };
 __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorParams& tp, long long item,
-                                            const int64_t* __restrict__ offsets)
+                                            const int64_t* __restrict__ offsets, int rank = 0)
 {
     TcItem w;
     w.split = (int)(item % gp.n_split);
     const long long r = item / gp.n_split;
-    w.tile = (int)(r % gp.n_tiles);
-    w.obj_local = r / gp.n_tiles;
+    if (tp.pair) {
+        const int n_tp = (gp.n_tiles + 1) >> 1;
+        w.tile = 2 * (int)(r % n_tp) + rank;
+        w.obj_local = r / n_tp;
+    } else {
+        w.tile = (int)(r % gp.n_tiles);
+        w.obj_local = r / gp.n_tiles;
+    }
+    w.tile_ok = w.tile < gp.n_tiles;
     w.obj = w.obj_local + gp.obj_base;
     w.n_t = offsets[w.obj + 1] - offsets[w.obj];
     const int nkb = tc_n_kb(w.n_t);
@@ -408,19 +473,29 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
     return w;
 }
 
-// Depth D of the A ring in use (stages in flight between the generators and the MMA warp): what the ring's 64 TMEM columns
-// hold (2 stages of 4 planes with three products, else 4 stages of 2 planes), at most one per generator group, and -- the
-// generators wait on the B ring's "full" barriers out of step with the MMA warp, and their parity waits stay within one
-// phase of the barrier only if the B ring is at least NG + D stages deep -- small enough for the 7 four-plane B stages that
-// fit in shared memory at NL = 112 (pm = 2; fast_math stages are half as large).
-__host__ __device__ constexpr int tc_a_depth(int pm, int ng)
+// static shared memory of the kernel (generator scratch etc.), for the ring sizing here and on the host
+constexpr int tc_static_smem_of(int ew, int ng) { return ng * 2 * (8 * kTcVRow + 32) * 4 + ew * 16 + 256; }
+// B stages of the largest tile (NL = mnl) that fit beside it: dynamic = 1 KB alignment slack + ring + 384 B of barriers
+__host__ __device__ constexpr int tc_b_fit(int pm, int ew, int ng, bool pair, int mnl)
 {
-    const int as = pm == 0 ? 2 : 4;
-    int d = as < ng ? as : ng;
-    if (pm == 2 && d > 7 - ng) d = 7 - ng;
-    return d;
+    const int stage = (pm == 1 ? 2 : 4) * (pair ? 1 : 2) * mnl * 32 + kTcAuxBytes;
+    const int fit = (232448 - tc_static_smem_of(ew, ng) - 1024 - 384 - 512) / stage;
+    return fit < kTcMaxSB ? fit : kTcMaxSB;
 }
-__host__ __device__ constexpr int tc_min_stages_b(int pm, int ng) { return ng + tc_a_depth(pm, ng); }
+// Depth D of the A ring (operand stages in flight between the generators and the MMA warp).  A slot is recycled only after
+// the MMAs that read it have COMPLETED and the news has travelled commit -> generator -> tcgen05.st -> arrive -> MMA warp
+// (measured ~1500 cycles on a CTA pair), so the kernel sustains at most D stages per (that + the stage's MMA time): the ring is
+// made as deep as the tensor-memory columns left of the accumulators allow (512 - 4 mnl columns; a stage is 16 columns, 32 with
+// three products) -- which is why the pair-mode kernel runs tiles of NL <= 104 (6 stages) rather than 112 (4).  The generators
+// wait on the B ring's "full" barriers out of step with the MMA warp, and their parity waits stay within one phase of the
+// barrier only if the B ring is at least NG + D stages deep: D is capped by what fits in shared memory at NL = mnl.
+__host__ __device__ constexpr int tc_a_depth(int pm, int ew, int ng, bool pair, int mnl)
+{
+    int d = (512 - 4 * mnl) / (pm == 0 ? 32 : 16);
+    if (d > 8) d = 8;
+    const int room = tc_b_fit(pm, ew, ng, pair, mnl) - ng;
+    return d < room ? d : room;
+}
 // ---- split-N_t fix-up (n_split > 1) ----------------------------------------------------------------------------------
 // The n_split partial slots of a tile (lane-oriented un-scaled sums in the epilogue's own element order: element (i, row r)
 // at i * 128 + r, see the epilogue) are added in SPLIT ORDER -- results do not depend on scheduling -- and steps 5, 6, 6'
@@ -521,17 +596,19 @@ lsp_tensor_fix_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict_
 
 constexpr size_t tc_smem_bytes(int stages_b, int b_stage)
 {
-    return 1024 /* alignment slack */ + (size_t)stages_b * (size_t)b_stage + 256 /* barriers */;
+    return 1024 /* alignment slack */ + (size_t)stages_b * (size_t)b_stage + 384 /* barriers */;
 }
-// static shared memory of the kernel (generator scratch etc.), for the host's ring sizing
-template <int EW, int NG> constexpr int tc_static_smem() { return NG * 2 * (8 * kTcVRow + 32) * 4 + EW * 16 + 256; }
+template <int EW, int NG> constexpr int tc_static_smem() { return tc_static_smem_of(EW, NG); }
 
 // GM (generalised mode): 0 = standard; 1 = the W slot carries the weights (partial-sum output); 2 = 1 + ZK09's power fused into
 // the epilogue (n_split = 1).  A template parameter so that the standard kernel carries none of it.
 // PM (precision mode): 0 = three products a_hi b_hi + a_hi b_lo + a_lo b_hi; 2 = two products a_hi (b_hi + b_lo) -- the A
 // operand is one FP16 (the generators skip the low part, the A ring is twice as deep), the B table is the same;
 // 1 = fast_math: one product and MUFU sincos.
-template <typename T, int PM, int EW, int NG, int GM>
+// PAIR: CTA pairs (2-CTA clusters; the launch carries the cluster dimension): see TensorParams::pair.
+// MNL: the largest NL the instantiation accepts; fixes the tensor-memory layout: Z accumulators [0, 2 NL), W accumulators
+// [2 MNL, 2 MNL + 2 NL), A ring [4 MNL, 512).
+template <typename T, int PM, int EW, int NG, int GM, bool PAIR = false, int MNL = kTcMaxNL>
 __global__ void __launch_bounds__((TcRoles<EW, NG>::kThreads), 1)
 lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
                   const unsigned char* __restrict__ table, T* __restrict__ out_power, Best* __restrict__ partials,
@@ -544,26 +621,38 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
     constexpr bool A_LO = PM == 0;                            // the A operand carries a low part
     constexpr int NOPS = FAST ? 2 : 4;                        // FP16 planes of a B stage
     constexpr int A_STAGE_COLS = (A_LO ? 4 : 2) * 8;          // TMEM columns of one A stage
-    constexpr int AS = kTcACols / A_STAGE_COLS;               // A stages that fit in the ring's columns: 2 (three products) or 4
+    constexpr int WCOL = 2 * MNL, ACOL = 4 * MNL;             // first TMEM column of the W accumulators / of the A ring
+    constexpr int AS = (512 - ACOL) / A_STAGE_COLS;           // A stages that fit in the ring's columns
     // Hand-off protocol of the A ring.  Stage s (numbered per CTA across items) is built by generator group s % NG into TMEM
-    // slot s % D, D = min(AS, NG).  mbarrier waits are parity waits: a waiter must never be two phases away from its barrier,
-    // so the "slot is free" signal is kept PER GROUP, not per slot: the commit that follows the MMAs of stage j arrives on
-    // free_g[(j + D) % NG], the barrier of the group that will write stage j + D into the slot stage j occupied.  Group k thus
-    // sees exactly one arrival per stage it builds (none for its first stage if that is one of the first D), waits for
-    // them strictly in order, and arrival i + 1 cannot precede its consumption of arrival i (it needs MMA(s + NG - D), which
-    // is issued after MMA(s), which needs this group's stage s).  full_a[slot] is waited on by the MMA warp only, in order.
-    constexpr int D = tc_a_depth(PM, NG);
-    static_assert(D >= 1 && D <= AS && D <= NG, "A ring depth");
+    // slot s % D (tc_a_depth).  full_a[slot]: the generators' arrivals, waited on by the MMA warp only, in order.  "Slot free" is
+    // the commit that follows the MMAs of a stage.  mbarrier waits are parity waits, so a waiter must never be two phases away
+    // from its barrier (in either direction); which barrier carries the signal therefore depends on the shape:
+    //   D >= NG: one barrier per SLOT.  Use u of a slot (stage u D + q) waits for the slot's u-th arrival.  Arrival u + 1 needs use
+    //            u built, whose builder has consumed arrival u; and the builder of stage s has already waited for MMA(s - NG - D),
+    //            which completes after MMA(s - 2 D) (NG <= D), i.e. arrival u - 1 has happened when it starts to wait.
+    //   D <  NG: one barrier per GROUP: the commit after the MMAs of stage j arrives on the barrier of group (j + D) % NG, which
+    //            will write stage j + D into that slot.  A group sees exactly one arrival per stage it builds (none for its first
+    //            if that is one of the CTA's first D), waits for them strictly in order, and arrival i + 1 cannot precede its
+    //            consumption of arrival i (it needs MMA(s + NG - D), issued after MMA(s), which needs this group's stage s).
+    constexpr int D = tc_a_depth(PM, EW, NG, PAIR, MNL);
+    static_assert(D >= 1 && D <= AS && D <= 8 && NG <= 8 && MNL % 8 == 0 && MNL <= 112, "A ring depth");
+    constexpr bool PER_SLOT = D >= NG;
+    constexpr int NFREE = PER_SLOT ? D : NG;                  // "slot free" barriers in use
+    static_assert(!PAIR || GM == 0, "pair mode is built for the standard periodogram only");
     extern __shared__ unsigned char smem_dyn[];
     unsigned char* smem_b = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
     const int SB = tp.stages_b;
-    const unsigned b_bytes = (unsigned)tp.b_stage_bytes;
+    const unsigned b_bytes = (unsigned)tp.smem_stage_bytes;       // one B stage in this CTA's ring
+    const unsigned rank = PAIR ? cluster_ctarank() : 0u;         // pair mode: 0 = leader (issues the MMAs of both CTAs)
+    // this CTA's item sequence: items first, first + stride, ... (pair mode: both CTAs of a cluster walk the same sequence)
+    const long long first = PAIR ? (long long)(blockIdx.x >> 1) : (long long)blockIdx.x;
+    const long long stride = PAIR ? (long long)(gridDim.x >> 1) : (long long)gridDim.x;
     const int aux_off = NOPS * tp.b_plane_bytes;              // byte offset of the aux block inside a B stage
     unsigned long long* full_b = reinterpret_cast<unsigned long long*>(smem_b + (size_t)SB * b_bytes);
-    unsigned long long* empty_b = full_b + 8;
-    unsigned long long* full_a = empty_b + 8;
-    unsigned long long* free_g = full_a + 4;
-    unsigned long long* tmem_full = free_g + 4;
+    unsigned long long* empty_b = full_b + kTcMaxSB;
+    unsigned long long* full_a = empty_b + kTcMaxSB;
+    unsigned long long* free_s = full_a + 8;
+    unsigned long long* tmem_full = free_s + 8;
     unsigned long long* tmem_empty = tmem_full + 1;
     __shared__ unsigned tmem_base_s;
     __shared__ Best sbest[kEpiWarps];
@@ -578,19 +667,31 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             mbar_init(&full_b[s], 1);
             mbar_init(&empty_b[s], 1);
         }
-        for (int s = 0; s < D; ++s) mbar_init(&full_a[s], 4);     // one arrival per generator warp of the stage's group
-        for (int s = 0; s < NG; ++s) mbar_init(&free_g[s], 1);
+        // one arrival per generator warp of the stage's group; pair mode: of both CTAs, on the leader's barrier
+        for (int s = 0; s < D; ++s) mbar_init(&full_a[s], PAIR ? 8 : 4);
+        for (int s = 0; s < NFREE; ++s) mbar_init(&free_s[s], 1);
         mbar_init(tmem_full, 1);
-        mbar_init(tmem_empty, kEpiThreads);
+        mbar_init(tmem_empty, PAIR ? 2 * kEpiThreads : kEpiThreads);      // pair mode: both CTAs' epilogues sign off with the leader
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 2) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        if (PAIR) {
+            asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
+        } else {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base_s)));
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        }
     }
     tc_fence_before();
-    __syncthreads();
+    if (PAIR) cluster_sync_all(); else __syncthreads();          // pair mode: the peer's barriers exist before anything arrives on them
     tc_fence_after();
+    // where the generators / the epilogue arrive: the local barrier, or (pair mode) the leader's copy of it
+    const unsigned full_a_addr0 = PAIR ? cluster_map(smem_u32(&full_a[0]), 0) : smem_u32(&full_a[0]);
+    const unsigned tmem_empty_addr = PAIR ? cluster_map(smem_u32(tmem_empty), 0) : smem_u32(tmem_empty);
+    auto arrive_tmem_empty = [&]() {
+        if (PAIR) mbar_arrive_cluster(tmem_empty_addr); else mbar_arrive(tmem_empty);
+    };
     const unsigned tmem = tmem_base_s;
     pdl_trigger();
     pdl_wait();            // the pre-pass's table and statistics are complete and visible from here on
@@ -601,43 +702,60 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         if (lane == 0) {
             int st = 0;
             unsigned ph = 1;                                      // parity of the "empty" phase to wait for
-            for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
-                const TcItem w = tc_decode(gp, tp, item, offsets);
-                const unsigned char* src = table + (size_t)(tc_kb_off(offsets, gp.obj_base, w.obj_local) + w.kb0) * (size_t)b_bytes;
+            const unsigned t_bytes = (unsigned)tp.b_stage_bytes;      // one stage of the table
+            const unsigned half_bytes = (unsigned)(NOPS * tp.b_plane_bytes);      // pair mode: this CTA's half of the planes
+            for (long long item = first; item < total_items; item += stride) {
+                const TcItem w = tc_decode(gp, tp, item, offsets, (int)rank);
+                const unsigned char* src = table + (size_t)(tc_kb_off(offsets, gp.obj_base, w.obj_local) + w.kb0) * (size_t)t_bytes;
                 for (int kb = w.kb0; kb < w.kb1; ++kb) {
                     mbar_wait(&empty_b[st], ph);
                     mbar_arrive_expect_tx(&full_b[st], b_bytes);
-                    tma_bulk_g2s(smem_b + (size_t)st * b_bytes, src, b_bytes, &full_b[st]);
-                    src += b_bytes;
+                    if (PAIR) {                                   // table stage = [half 0][half 1][aux]: this CTA's half, then the aux block
+                        tma_bulk_g2s(smem_b + (size_t)st * b_bytes, src + (size_t)rank * half_bytes, half_bytes, &full_b[st]);
+                        tma_bulk_g2s(smem_b + (size_t)st * b_bytes + half_bytes, src + 2 * (size_t)half_bytes, (unsigned)kTcAuxBytes, &full_b[st]);
+                    } else {
+                        tma_bulk_g2s(smem_b + (size_t)st * b_bytes, src, b_bytes, &full_b[st]);
+                    }
+                    src += t_bytes;
                     if (++st == SB) { st = 0; ph ^= 1; }
                 }
             }
         }
-    } else if (warp == 1) {
-        // =============================== MMA issuer ===============================================================
+    } else if (warp == 1 && rank == 0) {
+        // =============================== MMA issuer (pair mode: the leader CTA's, for both CTAs) ====================
         // The whole warp runs the loop with warp-uniform values (item ranges are broadcast from lane 0), so descriptors
         // and barrier addresses live in uniform registers; one elected lane issues the MMAs and commits.
-        const unsigned idesc = (1u << 4) | ((unsigned)((2 * tp.nl) >> 3) << 17) | ((unsigned)(128 >> 4) << 24);
-        const unsigned b_lbo = (unsigned)(2 * tp.nl / 8) * 128, sbo = 128;
+        const unsigned idesc = (1u << 4) | ((unsigned)((2 * tp.nl) >> 3) << 17) | ((unsigned)((PAIR ? 256 : 128) >> 4) << 24);
+        // bytes between the two k chunks of a plane = columns stored per plane x 16 (pair mode: the CTA's NL columns)
+        const unsigned b_lbo = (unsigned)((PAIR ? tp.nl : 2 * tp.nl) / 8) * 128, sbo = 128;
         // Descriptors of B stage 0; stage s adds s * stage_bytes / 16 to the 14-bit start-address field (the whole ring
         // lies below 256 KB, so the field never carries into the LBO bits).
         const unsigned sb0 = smem_u32(smem_b);
         const uint64_t b_zh0 = tc_smem_desc(sb0, b_lbo, sbo), b_wh0 = tc_smem_desc(sb0 + tp.b_plane_bytes, b_lbo, sbo);
         const uint64_t b_zl0 = tc_smem_desc(sb0 + 2 * tp.b_plane_bytes, b_lbo, sbo), b_wl0 = tc_smem_desc(sb0 + 3 * tp.b_plane_bytes, b_lbo, sbo);
         const uint64_t stage_inc_b = (uint64_t)(b_bytes >> 4);
-        const unsigned d_z = tmem, d_w = tmem + kTcWCol, a0 = tmem + kTcACol;
+        const unsigned d_z = tmem, d_w = tmem + WCOL, a0 = tmem + ACOL;
         const bool do_w = tp.z_only == 0;
-        int sa = 0, stb = 0, gsel = D % NG;                      // A slot, B slot, group that reuses the A slot next
+        int sa = 0, stb = 0, gsel = D % NG;                      // A slot, B slot, (D < NG) group that reuses the A slot next
         unsigned pha = 0, phb = 0, n_acc = 0;
         uint64_t sob = 0;                                         // stb * stage_inc_b
-        for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
+        auto mma = [&](unsigned d, unsigned a, uint64_t b, unsigned acc_) {
+            if (PAIR) tc_mma_f16_ts2(d, a, b, idesc, acc_); else tc_mma_f16_ts(d, a, b, idesc, acc_);
+        };
+        auto commit = [&](unsigned long long* bar) {
+            if (PAIR) tc_commit2(bar); else tc_commit(bar);
+        };
+        for (long long item = first; item < total_items; item += stride) {
             const TcItem w = tc_decode(gp, tp, item, offsets);
             const int kb0 = __shfl_sync(0xffffffffu, w.kb0, 0), kb1 = __shfl_sync(0xffffffffu, w.kb1, 0);
             if (kb1 <= kb0) continue;
-            mbar_wait(tmem_empty, (n_acc & 1) ^ 1);              // the epilogue has drained the previous accumulators
+            // the epilogue (pair mode: of both CTAs) has drained the previous accumulators
+            mbar_wait(tmem_empty, (n_acc & 1) ^ 1);
             tc_fence_after();
             unsigned acc = 0;
             for (int kb = kb0; kb < kb1; ++kb) {
+                // pair mode: full_a counts the generator warps of both CTAs, and the peer's generators arrive only after the
+                // peer's B stage has landed (they read its aux block), so the two waits cover all four operands
                 mbar_wait(&full_b[stb], phb);
                 mbar_wait(&full_a[sa], pha);
                 tc_fence_after();
@@ -645,27 +763,27 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     // planes (A in TMEM and B in shared memory alike): 0 = Z-operand hi, 1 = W-operand hi, 2 = Z lo, 3 = W lo
                     const unsigned a = a0 + (unsigned)(sa * A_STAGE_COLS);
                     if (PM == 2) {
-                        tc_mma_f16_ts(d_z, a, b_zl0 + sob, idesc, acc);
-                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, 1u);
+                        mma(d_z, a, b_zl0 + sob, acc);
+                        mma(d_z, a, b_zh0 + sob, 1u);
                         if (do_w) {
-                            tc_mma_f16_ts(d_w, a + 8, b_wl0 + sob, idesc, acc);
-                            tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, 1u);
+                            mma(d_w, a + 8, b_wl0 + sob, acc);
+                            mma(d_w, a + 8, b_wh0 + sob, 1u);
                         }
                     } else if (!FAST) {
-                        tc_mma_f16_ts(d_z, a + 16, b_zh0 + sob, idesc, acc);
-                        tc_mma_f16_ts(d_z, a, b_zl0 + sob, idesc, 1u);
-                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, 1u);
+                        mma(d_z, a + 16, b_zh0 + sob, acc);
+                        mma(d_z, a, b_zl0 + sob, 1u);
+                        mma(d_z, a, b_zh0 + sob, 1u);
                         if (do_w) {
-                            tc_mma_f16_ts(d_w, a + 24, b_wh0 + sob, idesc, acc);
-                            tc_mma_f16_ts(d_w, a + 8, b_wl0 + sob, idesc, 1u);
-                            tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, 1u);
+                            mma(d_w, a + 24, b_wh0 + sob, acc);
+                            mma(d_w, a + 8, b_wl0 + sob, 1u);
+                            mma(d_w, a + 8, b_wh0 + sob, 1u);
                         }
                     } else {
-                        tc_mma_f16_ts(d_z, a, b_zh0 + sob, idesc, acc);
-                        if (do_w) tc_mma_f16_ts(d_w, a + 8, b_wh0 + sob, idesc, acc);
+                        mma(d_z, a, b_zh0 + sob, acc);
+                        if (do_w) mma(d_w, a + 8, b_wh0 + sob, acc);
                     }
-                    tc_commit(&free_g[gsel]);                    // both stages are free once these MMAs have read them
-                    tc_commit(&empty_b[stb]);
+                    commit(&free_s[PER_SLOT ? sa : gsel]);       // both stages are free once these MMAs have read them
+                    commit(&empty_b[stb]);
                 }
                 __syncwarp();
                 acc = 1u;
@@ -674,7 +792,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 if (++gsel == NG) gsel = 0;
                 if (++stb == SB) { stb = 0; phb ^= 1; sob = 0; }
             }
-            if (elect_one()) tc_commit(tmem_full);               // accumulators complete
+            if (elect_one()) commit(tmem_full);                  // accumulators complete
             __syncwarp();
             ++n_acc;
         }
@@ -700,8 +818,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         const int kc = g * L + NL;                                // tile-local index of the first frequency above the centre
         const bool do_w = tp.z_only == 0;
         unsigned n_acc = 0;
-        for (long long item = blockIdx.x; item < total_items; item += gridDim.x) {
-            const TcItem w = tc_decode(gp, tp, item, offsets);
+        for (long long item = first; item < total_items; item += stride) {
+            const TcItem w = tc_decode(gp, tp, item, offsets, (int)rank);
             const TensorObj ob = objs[w.obj_local];
             const bool have = w.kb1 > w.kb0;
             if (FUSED) {
@@ -747,12 +865,12 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 if (have) {
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
-                    tc_ld16(ta + kTcWCol + m0, wr);
-                    tc_ld16(ta + kTcWCol + NL + m0, wi);
+                    tc_ld16(ta + WCOL + m0, wr);
+                    tc_ld16(ta + WCOL + NL + m0, wi);
                     tc_ld_wait();
                     if (ch == ch1 - 1) {                          // last TMEM read of this warp: the MMA warp may overwrite
                         tc_fence_before();
-                        mbar_arrive(tmem_empty);
+                        arrive_tmem_empty();
                         released = true;
                     }
                 } else {
@@ -849,13 +967,13 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     tc_ld16(ta + m0, zr);
                     tc_ld16(ta + NL + m0, zi);
                     if (do_w) {
-                        tc_ld16(ta + kTcWCol + m0, wr);
-                        tc_ld16(ta + kTcWCol + NL + m0, wi);
+                        tc_ld16(ta + WCOL + m0, wr);
+                        tc_ld16(ta + WCOL + NL + m0, wi);
                     }
                     tc_ld_wait();
                     if (ch == ch1 - 1) {
                         tc_fence_before();
-                        mbar_arrive(tmem_empty);
+                        arrive_tmem_empty();
                         released = true;
                     }
                 }
@@ -885,7 +1003,9 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                     }
                 }
             };
-            if (sums && !FUSED) {
+            if (!w.tile_ok) {
+                // phantom tile of an odd tile count (pair mode): nothing to store
+            } else if (sums && !FUSED) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk_sums(ch);
             } else if (ragged) {
                 for (int ch = ch0; ch < ch1; ++ch) chunk(ch, std::true_type{});
@@ -894,13 +1014,13 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             }
             const int bk = (bi < 0) ? 0x7fffffff : (is_im ? kc - 1 - bi : kc + bi);
             if (have) {
-                if (!released) {                                  // a warp without chunks (NL <= 16) still signs off
+                if (!released) {                                  // a warp without chunks (NL <= 16, phantom tile) still signs off
                     tc_fence_before();
-                    mbar_arrive(tmem_empty);
+                    arrive_tmem_empty();
                 }
                 ++n_acc;
             }
-            if (partials && (!sums || FUSED)) {
+            if (partials && (!sums || FUSED) && w.tile_ok) {
                 Best mine;
                 mine.p = (double)bp;
                 mine.k = (bk == 0x7fffffff) ? INT64_MAX : w.K0 + (int64_t)bk;
@@ -931,7 +1051,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         // -- the same instruction stream for both halves of the warp (the lane's v row, a 0/1 factor and its y scale are
         // the only differences).  The row's 16 values per plane are split into FP16 hi / lo, packed, and stored with
         // tcgen05.st into the stage's TMEM columns; the MMAs read them from there.
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kGenRegs));
+        if (R::kGenRegs > R::kLaunchRegs) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R::kGenRegs));
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R::kGenRegs));
         const int gw = warp - (4 + kEpiWarps);                    // 0 .. 4 NG - 1
         const int grp = gw >> 2;                                  // generator group: stages with (stage number mod NG) == grp
         const int q = warp & 3;                                   // TMEM lane quadrant (= gw & 3)
@@ -945,17 +1066,17 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         const int NL = tp.nl, L = 2 * NL;
         const float2 gam2 = is_im ? make_float2(1.f, 1.f) : make_float2(0.f, 0.f);
         const bool do_w = tp.z_only == 0;
-        const unsigned trow = tmem + ((unsigned)(32 * q) << 16) + kTcACol;
+        const unsigned trow = tmem + ((unsigned)(32 * q) << 16) + ACOL;
         const unsigned smem_b_u32 = smem_u32(smem_b);
         const int v_row = is_im ? 8 + g1 : g1;
         const int pos1 = g0p * kTcVRow + 4 * (jp >> 1) + (jp & 1);   // phase 1: where u (g0p, jp) goes (pair-planar)
 
         // A cursor walks the CTA's stage sequence (items in round-robin order, 16-observation blocks inside an item).
-        long long item = blockIdx.x;
+        long long item = first;
         int left = 0;                                             // stages of `item` not yet consumed by this group's cursor
         float f_hi = 0.f, f_lo = 0.f, mean = 0.f, ysc = 0.f, wsc = 0.f;
         auto load_item = [&]() {                                  // `item` is set; returns its number of stages
-            const TcItem w = tc_decode(gp, tp, item, offsets);
+            const TcItem w = tc_decode(gp, tp, item, offsets, (int)rank);
             const double fd = gp.f_min + ((double)(w.K0 + (int64_t)g0p * L + NL) - 0.5) * gp.df;
             f_hi = (float)fd;
             f_lo = (float)(fd - (double)f_hi);
@@ -966,23 +1087,36 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             return w.kb1 - w.kb0;
         };
         auto seek = [&]() {                                       // first item at or after `item` that has stages
-            while (item < total_items && (left = load_item()) <= 0) item += gridDim.x;
+            while (item < total_items && (left = load_item()) <= 0) item += stride;
         };
         auto advance = [&](int n) {                               // move the cursor n stages ahead
+            if (left > n) { left -= n; return; }                  // (almost always: the item has more stages)
             while (n > 0 && item < total_items) {
                 if (left > n) { left -= n; n = 0; }
-                else { n -= left; item += gridDim.x; seek(); }
+                else { n -= left; item += stride; seek(); }
             }
         };
         seek();
         advance(grp);
+        // Stage s of the CTA (this group builds s = grp, grp + NG, ...) goes into A slot s % D as that slot's use number s / D.
+        // PER_SLOT: use u waits for the slot's u-th "free" arrival (parity (u - 1) & 1); else the group's n-th wait is for the
+        // n-th arrival on its own barrier (see the protocol notes at the top of the kernel).
         int sb = grp % SB, sa = grp % D;                          // ring slots of this group's current stage
         unsigned phb = (unsigned)((grp / SB) & 1);
-        unsigned it = 0, n_wait = 0;                              // stages built; "slot free" arrivals consumed
+        unsigned it = 0, use = (unsigned)(grp / D), n_wait = 0;   // stages built; use number of slot sa; (per group) arrivals consumed
         while (item < total_items) {
             float* su = &s_u[grp][it & 1][0];
             const unsigned aux = smem_b_u32 + (unsigned)sb * b_bytes + (unsigned)aux_off;     // shared-space address of the aux block
             mbar_wait_backoff(&full_b[sb], phb);                  // the stage's table block (and its aux) has landed
+            // this row's tile-independent phasors v' (in the aux block): loaded now, in flight while phase 1 runs
+            // (register budget permitting: the long-item shape) -- (c0, c1, s0, s1) of observations 2 h, 2 h + 1
+            constexpr bool EARLY_V = R::kGenRegs >= 88;
+            const unsigned vp = aux + 4 * (48 + v_row * kTcVRow);
+            float4 vq[2][4];
+            if (EARLY_V) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) vq[0][e] = lds128(vp + 16 * e);
+            }
             // ---- phase 1: u (g0p, jp), scaled by 16; threads with g0p = 0 also scale the stage's magnitudes
             {
                 const float tv = lds32(aux + 4 * jp);
@@ -1000,46 +1134,58 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 }
             }
             named_bar_sync(4 + grp, R::kGenGroupThreads);
-            // ---- phase 2: this row's 16 operand values per plane
+            // ---- phase 2: this row's 16 operand values per plane; the tile's phasors u in two batches of four loads
             const unsigned up = smem_u32(su + g0 * kTcVRow);
-            const unsigned vp = aux + 4 * (48 + v_row * kTcVRow);
             const unsigned yp = smem_u32(su + 8 * kTcVRow + (is_im ? 16 : 0));
             unsigned zh[8], zl[8], wh[8], wl[8];
             float4 y4 = make_float4(0.f, 0.f, 0.f, 0.f), w4 = y4;
 #pragma unroll
-            for (int h = 0; h < 8; ++h) {                          // observations 2 h, 2 h + 1
-                const float4 uu = lds128(up + 16 * h), vv = lds128(vp + 16 * h);               // (c0, c1, s0, s1)
-                const float2 uc = make_float2(uu.x, uu.y), us = make_float2(uu.z, uu.w);
-                const float2 vc = make_float2(vv.x, vv.y), vs = make_float2(vv.z, vv.w);
-                if ((h & 1) == 0) y4 = lds128(yp + 16 * (h >> 1));
-                const float2 ys2 = (h & 1) ? make_float2(y4.z, y4.w) : make_float2(y4.x, y4.y);
-                const float2 pp = __ffma2_rn(uc, vc, __fmul2_rn(make_float2(-us.x, -us.y), vs));     // uc vc - us vs
-                const float2 qq = __ffma2_rn(uc, vs, __fmul2_rn(us, vc));                            // uc vs + us vc
-                const float2 az = __fmul2_rn(__ffma2_rn(qq, gam2, pp), ys2);
-                auto pack = [&](const float2 x, unsigned& hi, unsigned& lo) {
-                    const __half2 hh = __floats2half2_rn(x.x, x.y);
-                    hi = *reinterpret_cast<const unsigned*>(&hh);
-                    if (A_LO) {
-                        const float2 r = __ffma2_rn(__half22float2(hh), make_float2(-1.f, -1.f), x);     // one packed op
-                        const __half2 ll = __floats2half2_rn(r.x, r.y);
-                        lo = *reinterpret_cast<const unsigned*>(&ll);
+            for (int hb = 0; hb < 8; hb += 4) {
+                float4 uq[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) uq[e] = lds128(up + 16 * (hb + e));
+                const float4 y4a = lds128(yp + 16 * (hb >> 1)), y4b = lds128(yp + 16 * (hb >> 1) + 16);
+                if (EARLY_V ? hb == 0 : true) {                    // v' of the other batch (EARLY_V) / of this batch
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) vq[EARLY_V ? 1 : hb >> 2][e] = lds128(vp + 16 * ((EARLY_V ? 4 : hb) + e));
+                }
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int h = hb + e;                              // observations 2 h, 2 h + 1
+                    const float4 uu = uq[e];
+                    const float2 uc = make_float2(uu.x, uu.y), us = make_float2(uu.z, uu.w);
+                    const float4 vv = vq[hb >> 2][e];
+                    const float2 vc = make_float2(vv.x, vv.y), vs = make_float2(vv.z, vv.w);
+                    y4 = (e & 2) ? y4b : y4a;
+                    const float2 ys2 = (h & 1) ? make_float2(y4.z, y4.w) : make_float2(y4.x, y4.y);
+                    const float2 pp = __ffma2_rn(uc, vc, __fmul2_rn(make_float2(-us.x, -us.y), vs));     // uc vc - us vs
+                    const float2 qq = __ffma2_rn(uc, vs, __fmul2_rn(us, vc));                            // uc vs + us vc
+                    const float2 az = __fmul2_rn(__ffma2_rn(qq, gam2, pp), ys2);
+                    auto pack = [&](const float2 x, unsigned& hi, unsigned& lo) {
+                        const __half2 hh = __floats2half2_rn(x.x, x.y);
+                        hi = *reinterpret_cast<const unsigned*>(&hh);
+                        if (A_LO) {
+                            const float2 r = __ffma2_rn(__half22float2(hh), make_float2(-1.f, -1.f), x);     // one packed op
+                            const __half2 ll = __floats2half2_rn(r.x, r.y);
+                            lo = *reinterpret_cast<const unsigned*>(&ll);
+                        }
+                    };
+                    pack(az, zh[h], zl[h]);
+                    if (do_w) {
+                        float2 aw = __ffma2_rn(make_float2(-qq.x, -qq.y), qq, __fmul2_rn(pp, pp));       // p^2 - q^2 (x 256)
+                        if (WGT) {
+                            if ((h & 1) == 0) w4 = lds128(aux + 128 + 16 * (h >> 1));
+                            const float2 ww = (h & 1) ? make_float2(w4.z, w4.w) : make_float2(w4.x, w4.y);
+                            aw = __fmul2_rn(aw, __fmul2_rn(ww, make_float2(wsc, wsc)));
+                        }
+                        pack(aw, wh[h], wl[h]);
                     }
-                };
-                pack(az, zh[h], zl[h]);
-                if (do_w) {
-                    float2 aw = __ffma2_rn(make_float2(-qq.x, -qq.y), qq, __fmul2_rn(pp, pp));       // p^2 - q^2 (x 256)
-                    if (WGT) {
-                        if ((h & 1) == 0) w4 = lds128(aux + 128 + 16 * (h >> 1));
-                        const float2 ww = (h & 1) ? make_float2(w4.z, w4.w) : make_float2(w4.x, w4.y);
-                        aw = __fmul2_rn(aw, __fmul2_rn(ww, make_float2(wsc, wsc)));
-                    }
-                    pack(aw, wh[h], wl[h]);
                 }
             }
             // ---- into the stage's TMEM columns once the MMAs that read its previous contents have completed
-            if (it > 0 || grp >= D) {                             // not one of the CTA's first D stages
-                mbar_wait(&free_g[grp], n_wait & 1);              // on the critical path (2-deep ring): no sleep between polls
-                ++n_wait;
+            if (use > 0) {                                        // not one of the CTA's first D stages; on the critical path: no sleep
+                if (PER_SLOT) mbar_wait(&free_s[sa], (use - 1) & 1);
+                else { mbar_wait(&free_s[grp], n_wait & 1); ++n_wait; }
             }
             tc_fence_after();
             const unsigned ta = trow + (unsigned)(sa * A_STAGE_COLS);
@@ -1052,19 +1198,27 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             tc_st_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&full_a[sa]);
+            if (lane == 0) {
+                if (PAIR) mbar_arrive_cluster(full_a_addr0 + 8u * (unsigned)sa); else mbar_arrive(&full_a[sa]);
+            }
             // ---- next stage of this group
             advance(NG);
             sb += NG;
-            while (sb >= SB) { sb -= SB; phb ^= 1; }
-            sa = (sa + NG) % D;
+            if (sb >= SB) { sb -= SB; phb ^= 1; }                // NG <= SB
+            sa += NG;
+            while (sa >= D) { sa -= D; ++use; }
             ++it;
         }
     }
     // teardown: everyone is done with TMEM before it is freed
     tc_fence_before();
-    __syncthreads();
-    if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+    if (PAIR) {
+        cluster_sync_all();           // the peer has stopped arriving on this CTA's barriers and reading its shared memory
+        if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+    } else {
+        __syncthreads();
+        if (warp == 2) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem));
+    }
 }
 
 }  // namespace lsp

@@ -55,7 +55,7 @@ def test_config_struct_layout_matches_header(pkg):
     assert pkg.LspConfig.n_freq.offset == 16 and pkg.LspConfig.chunk_bytes.offset == 48 and pkg.LspConfig.kernel.offset == 72
     assert pkg.LspConfig.flags.offset == 76 and pkg.LspConfig.table_budget_bytes.offset == 80
     assert pkg.LspConfig.tensor_roles.offset == 88 and pkg.LspConfig.tensor_b_stages.offset == 92
-    assert pkg.LspConfig.tensor_products.offset == 96 and pkg.LspConfig.reserved.offset == 100
+    assert pkg.LspConfig.tensor_products.offset == 96 and pkg.LspConfig.tensor_pair.offset == 100
     # the header's struct has the same fields in the same order
     src = re.sub(r"/\*.*?\*/", "", open(HEADER).read(), flags=re.S)
     body = re.search(r"typedef struct lsp_config \{(.*?)\} lsp_config;", src, flags=re.S).group(1)
@@ -76,11 +76,11 @@ def test_library_is_built_for_sm_100a_only():
                                 dict(dtype=1, fast_math=1), dict(dtype=7), dict(kernel=9), dict(flags=2),
                                 dict(n_copy_streams=99), dict(table_budget_bytes=-1), dict(tensor_roles=3),
                                 dict(tensor_b_stages=1), dict(tensor_b_stages=9), dict(tensor_products=1),
-                                dict(tensor_products=4), dict(reserved=1)])
+                                dict(tensor_products=4), dict(tensor_pair=3), dict(tensor_pair=-1)])
 def test_plan_create_rejects_bad_arguments_on_host(pkg, kw):
     args = dict(f_min=0.1, f_max=2.0, n_freq=10, dtype=0, fast_math=0, normalize=0, center=0, device=0,
                 n_copy_streams=0, chunk_bytes=0, max_objects=0, max_total_obs=0, kernel=0, flags=0,
-                table_budget_bytes=0, tensor_roles=0, tensor_b_stages=0, tensor_products=0, reserved=0)
+                table_budget_bytes=0, tensor_roles=0, tensor_b_stages=0, tensor_products=0, tensor_pair=0)
     args.update(kw)
     cfg = pkg.LspConfig(**args)
     with pytest.raises(pkg.LspError) as ei:

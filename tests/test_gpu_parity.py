@@ -29,7 +29,20 @@ def to_device(w: Workload):
     return (torch.from_numpy(w.offsets).cuda(), torch.from_numpy(w.t).to(dt).cuda(), torch.from_numpy(w.y).to(dt).cuda())
 
 
+def plan_kw(kw):
+    """tensor_roles in the tests: 1 / 2 = that warp-role shape on single CTAs (tensor_pair = 1: never pair), 3 = CTA pairs
+    forced (tensor_pair = 2); 0 or absent = the scheduler's own choice."""
+    kw = dict(kw)
+    roles = kw.pop("tensor_roles", 0)
+    if roles in (1, 2):
+        kw.update(tensor_roles=roles, tensor_pair=1)
+    elif roles == 3:
+        kw.update(tensor_pair=2)
+    return kw
+
+
 def gpu_full(lsp, w: Workload, *, kernel="auto", fast_math=False, best=True, **kw):
+    kw = plan_kw(kw)
     off, t, y = to_device(w)
     with lsp.Plan(w.f_min, w.f_max, w.n_freq, w.dtype, kernel=kernel, fast_math=fast_math, **kw) as plan:
         power, b = plan.periodogram_batched(off, t, y, best=best, h_offsets=__import__("torch").from_numpy(w.offsets))
@@ -40,6 +53,7 @@ def gpu_full(lsp, w: Workload, *, kernel="auto", fast_math=False, best=True, **k
 
 
 def gpu_best(lsp, w: Workload, *, kernel="auto", fast_math=False, **kw):
+    kw = plan_kw(kw)
     off, t, y = to_device(w)
     with lsp.Plan(w.f_min, w.f_max, w.n_freq, w.dtype, kernel=kernel, fast_math=fast_math, **kw) as plan:
         b = plan.best_period(off, t, y)
@@ -78,15 +92,18 @@ def oracle_full(oracle, w: Workload):
     return oracle.periodogram(w.offsets, w.t, w.y, w.f_min, w.f_max, w.n_freq)
 
 
-# Kernel variants every shape test runs, (kernel, tensor_roles, tensor_products): the tensor kernel in BOTH warp-role shapes
-# (lsp_config.tensor_roles: 1 = short-item shape, 2 = long-item shape) and BOTH accurate precision modes (lsp_config.
-# tensor_products: 2 = the default, 3), so each template instantiation the scheduler can reach gets full-grid element-wise checks.
-KERNEL_VARIANTS = [("direct", 0, 0), ("factored", 0, 0), ("tensor", 1, 2), ("tensor", 2, 2), ("tensor", 1, 3), ("tensor", 2, 3)]
+# Kernel variants every shape test runs, (kernel, shape, tensor_products): the tensor kernel in ALL THREE launch shapes (1 =
+# short-item warp roles, 2 = long-item warp roles, 3 = long-item roles on CTA pairs / cta_group::2; see plan_kw) and BOTH accurate
+# precision modes (lsp_config.tensor_products: 2 = the default, 3), so each template instantiation the scheduler can reach gets
+# full-grid element-wise checks.  Shape 3 needs a grid of at least two tiles (> 14,336 frequencies): the shape tests give the
+# pair variants a larger grid where their own is a single tile.
+KERNEL_VARIANTS = [("direct", 0, 0), ("factored", 0, 0), ("tensor", 1, 2), ("tensor", 2, 2), ("tensor", 1, 3), ("tensor", 2, 3),
+                   ("tensor", 3, 2), ("tensor", 3, 3)]
 MIN_NT_TWO_PRODUCTS = 32      # a launch holding a shorter object runs with three products (lsp.h, lsp_last_call_info)
 
 
 def variant_id(v):
-    return v[0] if v[1] == 0 else f"tensor-roles{v[1]}-products{v[2]}"
+    return v[0] if v[1] == 0 else f"tensor-shape{v[1]}-products{v[2]}"
 
 
 def assert_two_point_pin(P_row, t2, y2, w: Workload, dtype, what=""):
@@ -121,7 +138,8 @@ def test_config2_shape_small(lsp, oracle, dtype, fast, variant):
     if kernel == "tensor" and (dtype == "f64" or (fast and products == 3)):
         pytest.skip("the tensor-core kernel is FP32-mode only; fast_math has one product")
     # N_t = 1500 spans several observation chunks with a ragged tail; N_f = 9001 spans several tiles with a ragged tail
-    w = make_config(2, dtype=dtype, n_t=1500, n_freq=9001)
+    # (CTA pairs: 30,011 = three tensor tiles, i.e. one full pair and one pair with a phantom second tile, ragged)
+    w = make_config(2, dtype=dtype, n_t=1500, n_freq=30_011 if roles == 3 else 9001)
     P_ref = oracle_full(oracle, w)
     P, best, info = gpu_full(lsp, w, kernel=kernel, fast_math=fast, tensor_roles=roles, tensor_products=products)
     assert info["tensor_shape"] == roles and info["tensor_products"] == (0 if kernel != "tensor" else 1 if fast else products)
@@ -129,20 +147,23 @@ def test_config2_shape_small(lsp, oracle, dtype, fast, variant):
     assert_best_parity(best, P_ref, w, dtype, oracle)
 
 
+@pytest.mark.parametrize("pair", [1, 0], ids=["single-cta", "auto"])
 @pytest.mark.parametrize("n_freq,fast", [(100_000, False), (99_999, False), (100_002, True)])
-def test_long_single_object_full_grid_long_item_shape(lsp, oracle, n_freq, fast):
+def test_long_single_object_full_grid_long_item_shape(lsp, oracle, n_freq, fast, pair):
     """The long-item role shape through the scheduler's OWN choice (no override): one object of N_t = 20,000 on a grid of
     seven tiles is split by observations into items of >= 48 stages (config 2's launch configuration on a smaller grid);
     the last split of every tile to arrive finishes the tile in-kernel.  Full grid against the oracle, N_f % 4 in {0, 3, 2}."""
     w = make_config(2, dtype="f32", n_t=20_000, n_freq=n_freq)
     P_ref = oracle_full(oracle, w)
-    P, best, info = gpu_full(lsp, w, fast_math=fast)
-    assert info["kernel"] == "tensor" and info["tensor_shape"] == 2 and info["n_split"] > 1
+    P, best, info = gpu_full(lsp, w, fast_math=fast, tensor_pair=pair)
+    # left to itself the scheduler puts these long items on CTA pairs (shape 3); tensor_pair = 1 keeps single CTAs (shape 2)
+    assert info["kernel"] == "tensor" and info["tensor_shape"] == (2 if pair == 1 else 3) and info["n_split"] > 1
     assert_power_parity(P, P_ref, "f32", f"long single nf={n_freq}")
     assert_best_parity(best, P_ref, w, "f32", oracle)
 
 
-def test_long_items_unsplit_batch_long_item_shape(lsp, oracle):
+@pytest.mark.parametrize("pair", [1, 0], ids=["single-cta", "auto"])
+def test_long_items_unsplit_batch_long_item_shape(lsp, oracle, pair):
     """The long-item shape's NON-split epilogue (power + vector stores + fused argmax in the kernel) by the scheduler's own
     choice: 1,300 objects of N_t = 1,024 on a 16,384-point grid give >= 8 x 148 items of 64 stages each, split 1.  Full
     periodogram + best period; the oracle checks a seeded sample of 16 WHOLE objects element by element."""
@@ -154,15 +175,15 @@ def test_long_items_unsplit_batch_long_item_shape(lsp, oracle):
     y = 0.5 * np.sin(2 * np.pi * t / per[:, None] + rng.uniform(0, 2 * np.pi, (n_obj, 1))) + rng.normal(0, 0.2, (n_obj, n_t))
     y -= y.mean(axis=1, keepdims=True)
     w = Workload("long-batch", off, t.reshape(-1).astype(np.float32), y.reshape(-1).astype(np.float32), 0.05, 12.0, n_freq, "f32")
-    P, best, info = gpu_full(lsp, w)
-    assert info["kernel"] == "tensor" and info["tensor_shape"] == 2 and info["n_split"] == 1
+    P, best, info = gpu_full(lsp, w, tensor_pair=pair)
+    assert info["kernel"] == "tensor" and info["tensor_shape"] == (2 if pair == 1 else 3) and info["n_split"] == 1
     pick = np.sort(rng.choice(n_obj, 16, replace=False))
     pick[0], pick[-1] = 0, n_obj - 1
     sub = w.take_objects(pick)
     P_ref = oracle_full(oracle, sub)
     assert_power_parity(P[pick], P_ref, "f32", "long batch")
     assert_best_parity(tuple(x[pick] for x in best), P_ref, sub, "f32", oracle, "long batch")
-    best_only, _ = gpu_best(lsp, w)
+    best_only, _ = gpu_best(lsp, w, tensor_pair=pair)
     for a, b in zip(best, best_only):
         assert np.array_equal(a, b, equal_nan=True)
 
@@ -187,7 +208,7 @@ def test_config2_full_size_full_grid(lsp, oracle, dtype, fast, products):
     P, best, info = gpu_full(lsp, w, fast_math=fast, tensor_products=products)
     assert info["kernel"] == ("tensor" if dtype == "f32" else "factored")
     if dtype == "f32":
-        assert info["tensor_shape"] == 2           # the long-item role shape is the one bench.py times on this config
+        assert info["tensor_shape"] == 3           # long-item roles on CTA pairs: the launch shape bench.py times on this config
         assert info["tensor_products"] == (1 if fast else products or 2)     # default = two products, as bench.py times it
     assert_power_parity(P, P_ref, dtype, f"c2 full {dtype} fast={fast}")
     assert_best_parity(best, P_ref, w, dtype, oracle, "c2 full")
@@ -201,7 +222,8 @@ def test_config2_full_size_full_grid(lsp, oracle, dtype, fast, products):
 # ---- config 3 shape: batch of short night-clustered objects, best period fused ----------------------------
 @pytest.mark.parametrize("kernel,fast,roles,products", [("factored", False, 0, 0), ("factored", True, 0, 0), ("direct", True, 0, 0),
                                                         ("tensor", False, 1, 2), ("tensor", True, 1, 0), ("tensor", False, 2, 2),
-                                                        ("tensor", True, 2, 0), ("tensor", False, 1, 3), ("tensor", False, 2, 3)])
+                                                        ("tensor", True, 2, 0), ("tensor", False, 1, 3), ("tensor", False, 2, 3),
+                                                        ("tensor", False, 3, 2), ("tensor", False, 3, 3), ("tensor", True, 3, 0)])
 def test_config3_shape_best_only(lsp, oracle, kernel, fast, roles, products):
     w = make_config(3, n_obj=24, n_freq=20_011)
     P_ref = oracle_full(oracle, w)
@@ -324,7 +346,7 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
     t = np.concatenate([np.sort(rng.uniform(0, 30, n)) for n in lens])
     y = rng.normal(0, 1, t.size)
     np_t = np.float32 if dtype == "f32" else np.float64
-    w = Workload("edge", off, t.astype(np_t), y.astype(np_t), 0.05, 3.0, 2500, dtype)
+    w = Workload("edge", off, t.astype(np_t), y.astype(np_t), 0.05, 3.0, 20_000 if roles == 3 else 2500, dtype)
     P_ref = oracle_full(oracle, w)
     P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
     if kernel == "tensor":       # objects of a few observations: the launch runs with three products whatever the plan says
@@ -334,7 +356,8 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
     # N_t = 1 and N_t = 2 hit the singular branch at isolated frequencies: there, finite + bounded only (reading a6) ...
     for o in (1, 2):
         yy = w.y[off[o]:off[o + 1]].astype(np.float64)
-        slack = 2e-2 if dtype == "f32" else 1e-6   # near-singular frequencies amplify rounding (reading a6)
+        # near-singular frequencies amplify rounding (reading a6); the pair variants' 8x denser grid comes 8x closer to them
+        slack = (2e-2 if dtype == "f32" else 1e-6) * (w.n_freq / 2500) ** 2
         assert P[o].min() >= 0 and P[o].max() <= 0.5 * (yy @ yy) * (1 + slack) + 1e-30
     # ... and away from them N_t = 2 has a closed form (pin p7)
     assert_two_point_pin(P[2], w.t[off[2]:off[3]], w.y[off[2]:off[3]], w, dtype, f"edge/{kernel}")
@@ -346,13 +369,17 @@ def test_edge_empty_and_tiny_objects(lsp, oracle, dtype, variant):
     assert_best_parity(tuple(x[keep] for x in best), P_ref[keep], sub, dtype, oracle)
 
 
-@pytest.mark.parametrize("n_freq", [1, 255, 4096, 4097])
+@pytest.mark.parametrize("n_freq", [1, 255, 4096, 4097, 28_672, 28_673, 43_009])
 def test_edge_ragged_grid_sizes(lsp, oracle, n_freq):
+    """Grid sizes around the tile sizes: one point, a ragged single tile, exact tiles, one over; for the CTA-pair shape exactly
+    two tiles of 14,336, one over (three tiles: a phantom fourth), and three full tiles + 1."""
     w = make_config(1, n_freq=n_freq, dtype="f32")
     P_ref = oracle_full(oracle, w)
     for kernel, roles, products in KERNEL_VARIANTS:
+        if (roles == 3) != (n_freq > 14_336):
+            continue
         P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
-        assert info["tensor_products"] == products
+        assert info["tensor_products"] == products and (roles != 3 or info["tensor_shape"] == 3)
         assert_power_parity(P, P_ref, "f32", f"nf={n_freq}/{kernel}/{products}")
         assert_best_parity(best, P_ref, w, "f32", oracle)
 
@@ -572,8 +599,9 @@ def test_random_shapes_all_kernels(lsp, oracle, seed):
     lens0, off0, t0, y0 = lens, off, t, y
     # (dtype, kernel variants, shift): the two-product tensor mode only runs when every object has >= 32 observations, so its
     # variants get the same draw with 32 more observations on every non-empty object (48 = 3 stages exactly, 49, 63, ...)
-    for dtype, kernels, shift in (("f32", (("tensor", 1, 3), ("tensor", 2, 3), ("factored", 0, 0), ("direct", 0, 0)), 0),
-                                  ("f32", (("tensor", 1, 2), ("tensor", 2, 2)), MIN_NT_TWO_PRODUCTS), ("f64", (("factored", 0, 0),), 0)):
+    for dtype, kernels, shift in (("f32", (("tensor", 1, 3), ("tensor", 2, 3), ("tensor", 3, 3), ("factored", 0, 0), ("direct", 0, 0)), 0),
+                                  ("f32", (("tensor", 1, 2), ("tensor", 2, 2), ("tensor", 3, 2)), MIN_NT_TWO_PRODUCTS),
+                                  ("f64", (("factored", 0, 0),), 0)):
         if shift:
             lens = np.where(lens0 > 0, lens0 + shift, 0)
             off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
@@ -586,6 +614,8 @@ def test_random_shapes_all_kernels(lsp, oracle, seed):
                      y.astype(np.float32 if dtype == "f32" else np.float64), f_min, f_max, n_freq, dtype=dtype)
         P_ref = oracle_full(oracle, w)
         for kernel, roles, products in kernels:
+            if roles == 3 and n_freq <= 14_336:
+                continue                 # a single tile: nothing to pair
             P, best, info = gpu_full(lsp, w, kernel=kernel, tensor_roles=roles, tensor_products=products)
             assert info["tensor_shape"] == roles and info["tensor_products"] == products
             for o in range(n_obj):
