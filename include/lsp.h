@@ -168,7 +168,20 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj,
                                        void* cuda_stream);
 
 /*
- * End-to-end form of the two calls above for callers whose data lives on the HOST (the paper's own call
+ * The generalised periodogram for callers whose data lives on the HOST: every pointer is a HOST pointer (h_sigma like h_t, h_y;
+ * h_out_power may be NULL for best-period-only output).  Inputs are copied to plan-owned device buffers on cuda_stream; full
+ * periodograms come back round by round through the plan's chunk ring and copy streams (chunk_bytes per round: the D2H of one
+ * round overlaps the kernels of the next), best-period arrays by one small D2H each.  Returns after everything
+ * has landed on the host.  Errors as lsp_periodogram_generalized.
+ */
+lsp_status lsp_periodogram_generalized_host(lsp_plan* plan, int64_t n_obj,
+                                            const int64_t* h_offsets, const void* h_t, const void* h_y, const void* h_sigma,
+                                            void* h_out_power,
+                                            void* h_best_period, void* h_best_power, int64_t* h_best_index,
+                                            void* cuda_stream);
+
+/*
+ * End-to-end form of lsp_periodogram_batched / lsp_best_period for callers whose data lives on the HOST (the paper's own call
  * shape: H2D of the concatenated (t, y) arrays, kernel, D2H of periodograms and/or periods,
  * PAPER.md:L85-91, L103-117).  Every pointer is a HOST pointer (pinned memory lets the copies overlap;
  * pageable memory works but serialises):

@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     lsp_periodogram_batched,
     lsp_periodogram_batched_host,
     lsp_periodogram_generalized,
+    lsp_periodogram_generalized_host,
     lsp_plan_create,
     lsp_version,
 )

@@ -23,7 +23,7 @@ _KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LS
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
 EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host",
-           "lsp_periodogram_generalized", "lsp_best_merge", "lsp_destroy",
+           "lsp_periodogram_generalized", "lsp_periodogram_generalized_host", "lsp_best_merge", "lsp_destroy",
            "lsp_last_error",
            "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_version")
 LSP_FLAG_PAGEABLE_STAGED = 1
@@ -68,6 +68,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_periodogram_batched_host.restype = ctypes.c_int
     lib.lsp_periodogram_generalized.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.lsp_periodogram_generalized.restype = ctypes.c_int
+    lib.lsp_periodogram_generalized_host.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.lsp_periodogram_generalized_host.restype = ctypes.c_int
     lib.lsp_best_merge.argtypes = [vp, i64, i32, vp, vp, vp, vp, vp, vp]
     lib.lsp_best_merge.restype = ctypes.c_int
     lib.lsp_destroy.argtypes = [vp]
@@ -133,6 +135,14 @@ def lsp_periodogram_batched_host(plan, n_obj: int, h_offsets, h_t, h_y, h_out_po
     _check(load_library().lsp_periodogram_batched_host(plan, int(n_obj), _dptr(h_offsets), _dptr(h_t), _dptr(h_y),
                                                        _dptr(h_out_power), _dptr(h_best_period), _dptr(h_best_power),
                                                        _dptr(h_best_index), _stream_ptr(stream)), plan)
+
+
+def lsp_periodogram_generalized_host(plan, n_obj: int, h_offsets, h_t, h_y, h_sigma, h_out_power=None, h_best_period=None,
+                                     h_best_power=None, h_best_index=None, stream=None) -> None:
+    """All-HOST form of the generalised LSP (include/lsp.h): H2D, kernels and D2H (chunk ring + copy streams) inside the call."""
+    _check(load_library().lsp_periodogram_generalized_host(plan, int(n_obj), _dptr(h_offsets), _dptr(h_t), _dptr(h_y),
+                                                           _dptr(h_sigma), _dptr(h_out_power), _dptr(h_best_period),
+                                                           _dptr(h_best_power), _dptr(h_best_index), _stream_ptr(stream)), plan)
 
 
 def lsp_periodogram_generalized(plan, n_obj: int, d_offsets, h_offsets, d_t, d_y, d_sigma, d_out_power=None,
@@ -301,6 +311,29 @@ class Plan:
             bi = torch.empty(n_obj, dtype=torch.int64, device=self.device)
         lsp_periodogram_generalized(self._plan, n_obj, offsets, h_offsets, t, y, sigma, power, bp, bw, bi, stream)
         return power, ((bp, bw, bi) if best else None)
+
+    def periodogram_generalized_host(self, h_offsets, h_t, h_y, h_sigma, *, host_out=None, best_out=None, stream=None):
+        """Generalised LSP end to end on HOST tensors (pinned for overlap): fills `host_out` [n_obj, n_freq] (or skips the
+        periodogram when None) and `best_out` = (period, power, index) host tensors.  Returns after all results are on the host."""
+        if h_offsets.is_cuda or h_offsets.dtype != torch.int64 or not h_offsets.is_contiguous() or h_offsets.numel() < 1:
+            raise TypeError("h_offsets must be a contiguous host int64 tensor of n_obj + 1 elements")
+        n_obj = int(h_offsets.numel() - 1)
+        for x in (h_t, h_y, h_sigma):
+            if x.is_cuda or x.dtype != self.torch_dtype or not x.is_contiguous():
+                raise TypeError(f"h_t, h_y and h_sigma must be contiguous host tensors of {self.torch_dtype}")
+        if not (h_t.numel() == h_y.numel() == h_sigma.numel()) or int(h_offsets[-1]) > h_t.numel():
+            raise TypeError("h_t, h_y and h_sigma must have the same length, at least offsets[n_obj]")
+        if host_out is not None and (host_out.is_cuda or host_out.dtype != self.torch_dtype or not host_out.is_contiguous()
+                                     or host_out.numel() != n_obj * self.n_freq):
+            raise TypeError("host_out must be a contiguous host tensor [n_obj, n_freq] of the plan dtype")
+        bp = bw = bi = None
+        if best_out is not None:
+            bp, bw, bi = best_out
+            if bp.is_cuda or bw.is_cuda or bi.is_cuda or bp.dtype != self.torch_dtype or bw.dtype != self.torch_dtype \
+                    or bi.dtype != torch.int64 or min(bp.numel(), bw.numel(), bi.numel()) < n_obj:
+                raise TypeError("best_out must be host tensors (period, power, index[int64]) of n_obj elements")
+        lsp_periodogram_generalized_host(self._plan, n_obj, h_offsets, h_t, h_y, h_sigma, host_out, bp, bw, bi, stream)
+        return host_out, best_out
 
     def best_merge(self, part_power, part_index, *, stream=None):
         """Merge per-shard (power, GLOBAL index) candidates, tensors [n_parts, n_obj] on this plan's device, into

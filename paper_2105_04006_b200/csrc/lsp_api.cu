@@ -62,7 +62,7 @@ struct lsp_plan {
     int tc_products = 2;          // FP16 products per MAC of the accurate tensor mode: 2 or 3 (cfg.tensor_products)
     int tc_pair = 0;              // CTA pairs on the tensor path: 0 = when items are long, 1 = never, 2 = whenever there are >= 2 tiles (cfg.tensor_pair)
     int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
-    DeviceBuffer in_off, in_t, in_y, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
+    DeviceBuffer in_off, in_t, in_y, in_sigma, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
     int64_t ws_table_obs = 0;     // observations the table was built for (this call)
     DeviceBuffer gls_x, gls_yy, gls_sums;        // generalised mode: x_A / x_B arrays, chi0^2 per object, 3 passes of partial sums
     int64_t* h_offsets_pinned = nullptr;
@@ -879,9 +879,14 @@ lsp_status lsp_best_period(lsp_plan* plan, int64_t n_obj, const int64_t* d_offse
                     cuda_stream);
 }
 
-lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
-                                       const void* d_t, const void* d_y, const void* d_sigma, void* d_out_power,
-                                       void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
+}  // extern "C"
+
+namespace {
+// The generalised call; `out_power` is a device pointer, or (out_is_host) a host pointer filled round by round through the plan's
+// chunk ring and copy streams, like step 7 of the standard call.
+lsp_status gls_call(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
+                    const void* d_t, const void* d_y, const void* d_sigma, void* d_out_power, int out_is_host,
+                    void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
 {
     lsp_plan* p = plan;
     if (!p) return LSP_ERR_INVALID_ARG;
@@ -960,15 +965,44 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
     const bool fused = s.kernel == LSP_KERNEL_TENSOR && s.n_split == 1;
     const size_t tile_elems = fused ? (size_t)((s.tp.nl + 15) / 16) * 16 * 128 : 0;
     const size_t per_obj = fused ? (size_t)s.n_tiles * tile_elems * sizeof(float2) : (size_t)2 * s.n_split * c.n_freq * 4 * es;
-    const int64_t objs_per_round = std::max<int64_t>(1, (int64_t)(((size_t)12 << 30) / per_obj));
+    int64_t objs_per_round = std::max<int64_t>(1, (int64_t)(((size_t)12 << 30) / per_obj));
     const size_t row_bytes = (size_t)c.n_freq * es;
     const int n_cparts = (int)((c.n_freq + kCombineThreads * kCombinePerThread - 1) / (kCombineThreads * kCombinePerThread));
-    for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_round) {
+    // host output: a round is a chunk of the ring (step 7: compute into a ring slot, event, D2H on a copy stream, overlapped with
+    // the next round's compute)
+    const bool to_host = d_out_power && out_is_host;
+    const int n_slots = (int)p->slot_ready.size();
+    size_t slot_bytes = 0;
+    if (to_host) {
+        const size_t chunk_bytes = c.chunk_bytes > 0 ? (size_t)c.chunk_bytes : ((size_t)64 << 20);
+        objs_per_round = std::min<int64_t>(objs_per_round, std::max<int64_t>(1, (int64_t)(chunk_bytes / row_bytes)));
+        slot_bytes = (size_t)objs_per_round * row_bytes;
+        if ((e = ensure(p, p->ring, slot_bytes * n_slots)) != LSP_OK) return e;
+        std::fill(p->slot_used.begin(), p->slot_used.end(), 0);
+    }
+    int64_t round = 0;
+    for (int64_t o0 = 0; o0 < n_obj; o0 += objs_per_round, ++round) {
         const int64_t no = std::min(objs_per_round, n_obj - o0);
         int n_parts = 0;
+        const int slot = (int)(round % n_slots);
+        void* const out = !d_out_power ? nullptr
+                          : to_host    ? (void*)((char*)p->ring.ptr + (size_t)slot * slot_bytes)
+                                       : (void*)((char*)d_out_power + (size_t)o0 * row_bytes);
+        if (to_host && p->slot_used[slot]) LSP_CUDA(p, cudaStreamWaitEvent(st, p->slot_free[slot], 0));
+        // after this round's kernels: hand the slot to a copy stream
+        auto ship = [&]() -> lsp_status {
+            if (!to_host) return LSP_OK;
+            LSP_CUDA(p, cudaEventRecord(p->slot_ready[slot], st));
+            cudaStream_t cs = p->copy_streams[round % p->copy_streams.size()];
+            LSP_CUDA(p, cudaStreamWaitEvent(cs, p->slot_ready[slot], 0));
+            LSP_CUDA(p, cudaMemcpyAsync((char*)d_out_power + (size_t)o0 * row_bytes, out, (size_t)no * row_bytes, cudaMemcpyDeviceToHost, cs));
+            LSP_CUDA(p, cudaEventRecord(p->slot_free[slot], cs));
+            p->slot_used[slot] = 1;
+            ++p->n_chunks;
+            return LSP_OK;
+        };
         if (fused) {
             if ((e = ensure(p, p->gls_sums, (size_t)no * per_obj)) != LSP_OK) return e;
-            void* out = d_out_power ? (char*)d_out_power + (size_t)o0 * row_bytes : nullptr;
             RangeOpts ro;
             ro.ext_sums = p->gls_sums.ptr;
             ro.wgt = xb;
@@ -981,6 +1015,7 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
             ro.gls_yy = (const double*)p->gls_yy.ptr;
             if ((e = run_range(p, s, g, o0, no, total_obs, d_offsets, d_t, xa, out, want_best, &n_parts, st, ro)) != LSP_OK) return e;
             if (want_best && (e = run_finalize(p, o0, no, n_parts, d_offsets, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+            if ((e = ship()) != LSP_OK) return e;
             continue;
         }
         const size_t pass_bytes = (size_t)s.n_split * no * c.n_freq * 4 * es;
@@ -1003,7 +1038,6 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
         gp.obj_base = (int)o0;
         if (want_best && (e = ensure(p, p->partials, (size_t)no * n_cparts * sizeof(Best))) != LSP_OK) return e;
         Best* partials = want_best ? (Best*)p->partials.ptr : nullptr;
-        void* out = d_out_power ? (char*)d_out_power + (size_t)o0 * row_bytes : nullptr;
         const int64_t grid = no * n_cparts;
         if (c.dtype == LSP_F32) {
             const float4* sa = (const float4*)p->gls_sums.ptr;
@@ -1017,7 +1051,75 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int6
         LSP_CUDA(p, cudaGetLastError());
         ++p->n_launches;
         if (want_best && (e = run_finalize(p, o0, no, n_cparts, d_offsets, d_best_period, d_best_power, d_best_index, st)) != LSP_OK) return e;
+        if ((e = ship()) != LSP_OK) return e;
     }
+    if (to_host)
+        for (cudaStream_t cs : p->copy_streams) LSP_CUDA(p, cudaStreamSynchronize(cs));
+    return LSP_OK;
+}
+}  // namespace
+
+extern "C" {
+
+lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj, const int64_t* d_offsets, const int64_t* h_offsets,
+                                       const void* d_t, const void* d_y, const void* d_sigma, void* d_out_power,
+                                       void* d_best_period, void* d_best_power, int64_t* d_best_index, void* cuda_stream)
+{
+    return gls_call(plan, n_obj, d_offsets, h_offsets, d_t, d_y, d_sigma, d_out_power, 0, d_best_period, d_best_power, d_best_index,
+                    cuda_stream);
+}
+
+lsp_status lsp_periodogram_generalized_host(lsp_plan* plan, int64_t n_obj, const int64_t* h_offsets, const void* h_t,
+                                            const void* h_y, const void* h_sigma, void* h_out_power, void* h_best_period,
+                                            void* h_best_power, int64_t* h_best_index, void* cuda_stream)
+{
+    lsp_plan* p = plan;
+    if (!p) return LSP_ERR_INVALID_ARG;
+    const lsp_config& c = p->cfg;
+    if (n_obj < 0) return fail(p, LSP_ERR_INVALID_ARG, "n_obj < 0");
+    const int n_best = (h_best_period != nullptr) + (h_best_power != nullptr) + (h_best_index != nullptr);
+    if (n_best != 0 && n_best != 3) return fail(p, LSP_ERR_INVALID_ARG, "best_period/best_power/best_index: give all three or none");
+    if (!h_out_power && n_best == 0) return fail(p, LSP_ERR_INVALID_ARG, "no output requested");
+    p->n_launches = p->n_pairs = p->n_chunks = 0;
+    if (n_obj == 0) return LSP_OK;
+    if (!h_offsets) return fail(p, LSP_ERR_INVALID_ARG, "h_offsets is NULL");
+    if (h_offsets[0] != 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[0] != 0");
+    for (int64_t o = 0; o < n_obj; ++o)
+        if (h_offsets[o + 1] < h_offsets[o]) return fail(p, LSP_ERR_INVALID_ARG, "offsets decrease at object %lld", (long long)o);
+    const int64_t total_obs = h_offsets[n_obj];
+    if (total_obs > 0 && (!h_t || !h_y || !h_sigma)) return fail(p, LSP_ERR_INVALID_ARG, "h_t / h_y / h_sigma is NULL");
+    LSP_CUDA(p, cudaSetDevice(c.device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t es = elem_size(c);
+    lsp_status e;
+    if ((e = ensure(p, p->in_off, (size_t)(n_obj + 1) * sizeof(int64_t))) != LSP_OK) return e;
+    if ((e = ensure(p, p->in_t, std::max<size_t>(16, (size_t)total_obs * es))) != LSP_OK) return e;
+    if ((e = ensure(p, p->in_y, std::max<size_t>(16, (size_t)total_obs * es))) != LSP_OK) return e;
+    if ((e = ensure(p, p->in_sigma, std::max<size_t>(16, (size_t)total_obs * es))) != LSP_OK) return e;
+    LSP_CUDA(p, cudaMemcpyAsync(p->in_off.ptr, h_offsets, (size_t)(n_obj + 1) * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    if (total_obs > 0) {
+        LSP_CUDA(p, cudaMemcpyAsync(p->in_t.ptr, h_t, (size_t)total_obs * es, cudaMemcpyHostToDevice, st));
+        LSP_CUDA(p, cudaMemcpyAsync(p->in_y.ptr, h_y, (size_t)total_obs * es, cudaMemcpyHostToDevice, st));
+        LSP_CUDA(p, cudaMemcpyAsync(p->in_sigma.ptr, h_sigma, (size_t)total_obs * es, cudaMemcpyHostToDevice, st));
+    }
+    char* d_bper = nullptr;
+    char* d_bpow = nullptr;
+    int64_t* d_bidx = nullptr;
+    if (n_best) {
+        if ((e = ensure(p, p->out_best, (size_t)n_obj * (2 * es + sizeof(int64_t)))) != LSP_OK) return e;
+        d_bidx = (int64_t*)p->out_best.ptr;
+        d_bper = (char*)p->out_best.ptr + (size_t)n_obj * sizeof(int64_t);
+        d_bpow = d_bper + (size_t)n_obj * es;
+    }
+    e = gls_call(p, n_obj, (const int64_t*)p->in_off.ptr, h_offsets, p->in_t.ptr, p->in_y.ptr, p->in_sigma.ptr, h_out_power,
+                 h_out_power ? 1 : 0, d_bper, d_bpow, d_bidx, cuda_stream);
+    if (e != LSP_OK) return e;
+    if (n_best) {
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_index, d_bidx, (size_t)n_obj * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_period, d_bper, (size_t)n_obj * es, cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaMemcpyAsync(h_best_power, d_bpow, (size_t)n_obj * es, cudaMemcpyDeviceToHost, st));
+    }
+    LSP_CUDA(p, cudaStreamSynchronize(st));
     return LSP_OK;
 }
 
@@ -1114,7 +1216,7 @@ void lsp_destroy(lsp_plan* p)
     for (cudaEvent_t e : p->slot_free) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_start) cudaEventDestroy(e);
     for (cudaEvent_t e : p->t_stop) cudaEventDestroy(e);
-    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->gls_x, &p->gls_yy, &p->gls_sums, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->out_best})
+    for (DeviceBuffer* b : {&p->ring, &p->partials, &p->sums, &p->stats, &p->counter, &p->ws_table, &p->gls_x, &p->gls_yy, &p->gls_sums, &p->tc_objs, &p->tc_table, &p->in_off, &p->in_t, &p->in_y, &p->in_sigma, &p->out_best})
         if (b->ptr) cudaFree(b->ptr);
     if (p->h_offsets_pinned) cudaFreeHost(p->h_offsets_pinned);
     if (p->stage_host) cudaFreeHost(p->stage_host);

@@ -515,6 +515,38 @@ def test_generalized_fused_epilogue_unsplit_batch(lsp, oracle, fast):
     assert_best_parity(tuple(x[pick][big] for x in best), P_ref[big], sub, "f32", oracle, "generalised fused")
 
 
+@pytest.mark.parametrize("dtype,kernel", [("f32", "auto"), ("f32", "factored"), ("f64", "auto")])
+def test_generalized_host_output_through_the_chunk_ring(lsp, oracle, dtype, kernel):
+    """lsp_periodogram_generalized_host: inputs and outputs on the host, full periodograms back through the chunk ring and the
+    copy streams in several rounds (5 objects per chunk, ragged last round), best periods by their own small copies; equal to
+    the device-output call bit for bit and to the oracle within tolerance; best-only form as well."""
+    import torch
+    w = make_config(3, n_obj=23, n_freq=12_007, dtype=dtype)
+    y, sigma = _with_errors(w, 91)
+    P_ref = oracle.periodogram_generalized(w.offsets, w.t, y, sigma, w.f_min, w.f_max, w.n_freq)
+    tdt = torch.float32 if dtype == "f32" else torch.float64
+    h_off = torch.from_numpy(w.offsets)
+    h_t, h_y, h_s = (torch.from_numpy(x).pin_memory() for x in (w.t, y, sigma))
+    host = torch.full((w.n_obj, w.n_freq), float("nan"), dtype=tdt).pin_memory()
+    hb = (torch.empty(w.n_obj, dtype=tdt).pin_memory(), torch.empty(w.n_obj, dtype=tdt).pin_memory(),
+          torch.empty(w.n_obj, dtype=torch.int64).pin_memory())
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, dtype, kernel=kernel, n_copy_streams=2, chunk_bytes=5 * w.n_freq * host.element_size()) as plan:
+        plan.periodogram_generalized_host(h_off, h_t, h_y, h_s, host_out=host, best_out=hb)
+        info = plan.last_call_info()
+        dev, db = plan.periodogram_generalized(h_off.cuda(), h_t.cuda(), h_y.cuda(), h_s.cuda(), best=True, h_offsets=h_off)
+        hb2 = tuple(torch.empty_like(x) for x in hb)
+        plan.periodogram_generalized_host(h_off, h_t, h_y, h_s, best_out=hb2)
+        torch.cuda.synchronize()
+    assert info["chunks"] == 5
+    P = host.numpy().astype(np.float64)
+    assert_power_parity(P, P_ref, dtype, f"generalised host {dtype}/{kernel}")
+    assert np.array_equal(host.numpy(), dev.cpu().numpy())
+    best = tuple(x.numpy() for x in hb)
+    assert_best_parity(best, P_ref, w, dtype, oracle, "generalised host")
+    for a, b, c in zip(hb, db, hb2):
+        assert np.array_equal(a.numpy(), b.cpu().numpy(), equal_nan=True) and np.array_equal(a.numpy(), c.numpy(), equal_nan=True)
+
+
 def test_generalized_single_object_and_edge_cases(lsp, oracle):
     import torch
     w = make_config(2, n_t=3000, n_freq=20000, dtype="f64")
