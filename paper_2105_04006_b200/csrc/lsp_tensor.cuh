@@ -1065,7 +1065,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
         const int g0 = g & 7, g1 = g >> 3;
         const int NL = tp.nl, L = 2 * NL;
         const float2 gam2 = is_im ? make_float2(1.f, 1.f) : make_float2(0.f, 0.f);
-        const bool do_w = tp.z_only == 0;
+        const bool do_w = PAIR ? true : tp.z_only == 0;           // (pair mode runs the standard periodogram only)
+        const bool y_is_w = PAIR ? false : tp.y_is_w != 0;
         const unsigned trow = tmem + ((unsigned)(32 * q) << 16) + ACOL;
         const unsigned smem_b_u32 = smem_u32(smem_b);
         const int v_row = is_im ? 8 + g1 : g1;
@@ -1081,8 +1082,8 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             f_hi = (float)fd;
             f_lo = (float)(fd - (double)f_hi);
             const TensorObj ob = objs[w.obj_local];
-            mean = tp.y_is_w ? 0.f : (float)ob.mean;
-            ysc = (tp.y_is_w ? ob.wscale : ob.yscale) * (1.0f / kTcPhasorScale);
+            mean = y_is_w ? 0.f : (float)ob.mean;
+            ysc = (y_is_w ? ob.wscale : ob.yscale) * (1.0f / kTcPhasorScale);
             wsc = ob.wscale * (1.0f / kTcUnitScale);
             return w.kb1 - w.kb0;
         };
@@ -1124,11 +1125,12 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                 const float e = fmaf(f_hi, tv, -p);
                 const float r = (p - rintf(p)) + fmaf(f_lo, tv, e);
                 float sn, cs;
-                if (FAST) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
+                // two products: the operand is rounded to 11 bits right after, MUFU's 2^-21 is far below that
+                if (FAST || PM == 2) sincos_cycles<true>(r, &sn, &cs); else sincos_cycles_reduced(r, &sn, &cs);
                 su[pos1] = cs * kTcPhasorScale;
                 su[pos1 + 2] = sn * kTcPhasorScale;
                 if (g0p == 0) {
-                    const float ys = (lds32(aux + (tp.y_is_w ? 128 : 64) + 4 * jp) - mean) * ysc;
+                    const float ys = (lds32(aux + (y_is_w ? 128 : 64) + 4 * jp) - mean) * ysc;
                     su[8 * kTcVRow + jp] = ys;                                  // "Re a" rows: y p
                     su[8 * kTcVRow + 16 + jp] = ys * 0.70710678118654752f;      // "Im a" rows: y (p + q) / sqrt 2
                 }
@@ -1208,6 +1210,7 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
             sa += NG;
             while (sa >= D) { sa -= D; ++use; }
             ++it;
+            asm volatile("" : "+r"(sb), "+r"(phb), "+r"(sa), "+r"(use), "+r"(it));
         }
     }
     // teardown: everyone is done with TMEM before it is freed
