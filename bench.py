@@ -279,18 +279,29 @@ def oracle_sample_runner(w, seconds_per_step: float):
         desc = f"first {n_o} of {w.n_obj} objects x {ks.size} of {w.n_freq} grid frequencies (strided)"
 
     def run():
-        oracle.periodogram(sub.offsets, sub.t, sub.y, w.f_min, w.f_max, w.n_freq, k_list=ks)
+        return oracle.periodogram(sub.offsets, sub.t, sub.y, w.f_min, w.f_max, w.n_freq, k_list=ks)
 
+    run.sub, run.ks = sub, ks
     return run, int(sub.n_obs) * int(ks.size), int(cores), desc
 
 
-def cpu_baseline(w, seconds: float):
+def cpu_baseline(w, seconds: float, gpu_power=None):
+    """The oracle timed on the host cores on a bounded sample of the workload.  `gpu_power(sub)`, if given, returns the CUDA
+    path's full periodogram of the sample's objects (library defaults, as timed): the sample then doubles as a parity spot
+    check of the timed configuration, max |dP| / max P over the sample (tolerances: BASELINE.json, 1e-3 FP32 / 1e-9 FP64)."""
     run, pairs, cores, desc = oracle_sample_runner(w, seconds)
     t0 = time.perf_counter()
-    run()
+    p_ref = run()
     dt = time.perf_counter() - t0
-    return {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-            "seconds": round(dt, 3)}
+    out = {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc, "seconds": round(dt, 3)}
+    if gpu_power is not None:
+        import numpy as np
+        p_gpu = gpu_power(run.sub)[:, run.ks].astype(np.float64)
+        err = float(np.max(np.max(np.abs(p_gpu - p_ref), axis=1) / np.max(p_ref, axis=1)))
+        out["parity_sample"] = {"max_err_over_max_p": err, "tolerance": 1e-3 if w.dtype == "f32" else 1e-9,
+                                "note": "CUDA path (library defaults, as timed) vs the oracle on the sampled grid points; "
+                                        "max P is the sample's"}
+    return out
 
 
 def run_reference(args, rank: int, world: int):
@@ -745,7 +756,16 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         overlap = c4_overlap(args, pkg, torch, local_rank, flush)
     cpu = None
     if solo and not args.no_cpu_baseline:
-        cpu = cpu_baseline(w, args.cpu_seconds)
+        def gpu_power(sub):
+            with pkg.Plan(sub.f_min, sub.f_max, sub.n_freq, args.dtype, kernel=args.kernel, fast_math=args.fast_math and args.dtype == "f32",
+                          device=local_rank, tensor_products=args.tensor_products) as plan:
+                dev = torch.device("cuda", local_rank)
+                h_off = torch.from_numpy(sub.offsets)
+                P, _ = plan.periodogram_batched(h_off.to(dev), torch.from_numpy(sub.t).to(dev), torch.from_numpy(sub.y).to(dev),
+                                                h_offsets=h_off)
+                torch.cuda.synchronize()
+                return P.cpu().numpy()
+        cpu = cpu_baseline(w, args.cpu_seconds, gpu_power if args.workload in ("c2", "c3") else None)
     if rank == 0:
         sharded = world > 1 and args.workload == "c3"
         rf_keys = ("bound", "achieved", "peak", "unit", "frac", "traffic", "traffic_from", "algorithmic_bytes", "hbm_write_gbs",

@@ -25,11 +25,12 @@
 //               Each table stage also carries an "aux" block (t_j, y_j, w_j and the tile-independent phasors v of its 16
 //               observations), so the generators never touch global memory.
 //
-// Precision: operands are FP16 pairs x = x_hi + x_lo (22 significand bits, the same class as
-// FP32's 24) and the product is a_hi b_hi + a_hi b_lo + a_lo b_hi (three MMAs; a_lo b_lo < 2^-22 is dropped), with y
-// pre-scaled by a power of two per object so FP16 never overflows or loses the low part.  fast_math = 1 keeps only
-// a_hi b_hi (one MMA, ~2^-11 per operand) and evaluates sincos with MUFU: the "fast vs accurate" comparison of
-// PAPER.md:L423-433 carried over to this formulation.  Phases are range-reduced before any FP32 trigonometry.
+// Precision: the tabulated operand b is an FP16 pair b_hi + b_lo (22 significand bits, the same class
+// as FP32's 24); the generated operand a is one FP16 (two products a_hi b_hi + a_hi b_lo per multiply-accumulate: the default)
+// or a pair as well (three products, + a_lo b_hi; a_lo b_lo < 2^-22 is dropped), with y pre-scaled by a power of two per object
+// so FP16 never overflows or loses the low part.  fast_math = 1 keeps only a_hi b_hi (one MMA, ~2^-11 per operand) and
+// evaluates sincos with MUFU: the "fast vs accurate" comparison of PAPER.md:L423-433 carried over to this formulation.
+// Phases are range-reduced before any FP32 trigonometry.
 //
 // Roles of one CTA (persistent, one per SM, static round-robin over (object, tile, split) work items):
 //   warp 0      TMA producer of the B ring          warp 1   MMA issuer (one elected lane)        warp 2   TMEM allocator
