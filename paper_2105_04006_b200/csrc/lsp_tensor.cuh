@@ -454,22 +454,30 @@ __device__ __forceinline__ TcItem tc_decode(const GridParams& gp, const TensorPa
                                             const int64_t* __restrict__ offsets, int rank = 0)
 {
     TcItem w;
-    w.split = (int)(item % gp.n_split);
-    const long long r = item / gp.n_split;
+    // (the host launches at most 2^31 - 1 items: 32-bit divisions; every role decodes every item of its CTA)
+    const unsigned it32 = (unsigned)item, ns = (unsigned)gp.n_split;
+    const unsigned r = ns == 1 ? it32 : it32 / ns;
+    w.split = (int)(it32 - r * ns);
     if (tp.pair) {
-        const int n_tp = (gp.n_tiles + 1) >> 1;
-        w.tile = 2 * (int)(r % n_tp) + rank;
-        w.obj_local = r / n_tp;
+        const unsigned n_tp = (unsigned)(gp.n_tiles + 1) >> 1, o = r / n_tp;
+        w.tile = 2 * (int)(r - o * n_tp) + rank;
+        w.obj_local = o;
     } else {
-        w.tile = (int)(r % gp.n_tiles);
-        w.obj_local = r / gp.n_tiles;
+        const unsigned o = r / (unsigned)gp.n_tiles;
+        w.tile = (int)(r - o * (unsigned)gp.n_tiles);
+        w.obj_local = o;
     }
     w.tile_ok = w.tile < gp.n_tiles;
     w.obj = w.obj_local + gp.obj_base;
     w.n_t = offsets[w.obj + 1] - offsets[w.obj];
     const int nkb = tc_n_kb(w.n_t);
-    w.kb0 = (int)(((long long)nkb * w.split) / gp.n_split);
-    w.kb1 = (int)(((long long)nkb * (w.split + 1)) / gp.n_split);
+    if (ns == 1) {
+        w.kb0 = 0;
+        w.kb1 = nkb;
+    } else {
+        w.kb0 = (int)(((long long)nkb * w.split) / gp.n_split);
+        w.kb1 = (int)(((long long)nkb * (w.split + 1)) / gp.n_split);
+    }
     w.K0 = (int64_t)w.tile * tp.tile;
     return w;
 }
@@ -487,7 +495,8 @@ __host__ __device__ constexpr int tc_b_fit(int pm, int ew, int ng, bool pair, in
 // the MMAs that read it have COMPLETED and the news has travelled commit -> generator -> tcgen05.st -> arrive -> MMA warp
 // (measured ~1500 cycles on a CTA pair), so the kernel sustains at most D stages per (that + the stage's MMA time): the ring is
 // made as deep as the tensor-memory columns left of the accumulators allow (512 - 4 mnl columns; a stage is 16 columns, 32 with
-// three products) -- which is why the pair-mode kernel runs tiles of NL <= 104 (6 stages) rather than 112 (4).  The generators
+// three products); narrower tiles would buy a deeper ring, but the generators redo their work per tile (measured: NL <= 104 and
+// a 6-deep ring is 8 % slower than NL <= 112 and 4).  The generators
 // wait on the B ring's "full" barriers out of step with the MMA warp, and their parity waits stay within one phase of the
 // barrier only if the B ring is at least NG + D stages deep: D is capped by what fits in shared memory at NL = mnl.
 __host__ __device__ constexpr int tc_a_depth(int pm, int ew, int ng, bool pair, int mnl)
@@ -505,7 +514,10 @@ __host__ __device__ constexpr int tc_a_depth(int pm, int ew, int ng, bool pair, 
 // own because it needs the whole GPU's memory parallelism: the same sums inside the main kernel's epilogue warps (a few
 // hundred threads per tile) are bound by the latency of their few loads in flight.
 constexpr int kTcFixThreads = 256;
-constexpr int kTcFixParts = 4;
+#ifndef LSP_TC_FIX_PARTS
+#define LSP_TC_FIX_PARTS 8
+#endif
+constexpr int kTcFixParts = LSP_TC_FIX_PARTS;
 template <typename T>
 __global__ void __launch_bounds__(kTcFixThreads)
 lsp_tensor_fix_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ offsets, const TensorObj* __restrict__ objs,
