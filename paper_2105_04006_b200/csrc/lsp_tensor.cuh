@@ -402,6 +402,12 @@ __device__ __forceinline__ bool elect_one()
     asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
     return pred != 0;
 }
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_ld16(unsigned taddr, float* v)
@@ -912,11 +918,15 @@ lsp_tensor_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict__ of
                         // of the c2 term, so with (c, s) = (wa, wb) on Re lanes and (-wb, wa) on Im lanes
                         //   P = [ n (A + B) - c (A - B) - 2 s za zb ] / (n^2 - wa^2 - wb^2),  A = za^2, B = zb^2.
                         const float cc = is_im ? -wb[e] : wa[e], ss = is_im ? wa[e] : wb[e];
-                        const float A = __fmul_rn(za[e], za[e]), B = __fmul_rn(zb[e], zb[e]);
-                        const float den = nn - fmaf(wa[e], wa[e], __fmul_rn(wb[e], wb[e]));
-                        const float num = fmaf(-2.0f * ss, __fmul_rn(za[e], zb[e]), fmaf(-cc, A - B, __fmul_rn(n_hat, A + B)));
+                        // (the epilogue is issue-bound on short items: A + B and A - B as two FMAs on B, the denominator as two)
+                        const float B = __fmul_rn(zb[e], zb[e]);
+                        const float ApB = fmaf(za[e], za[e], B), AmB = fmaf(za[e], za[e], -B);
+                        const float den = fmaf(-wa[e], wa[e], fmaf(-wb[e], wb[e], nn));
+                        const float num = fmaf(-2.0f * ss, __fmul_rn(za[e], zb[e]), fmaf(-cc, AmB, __fmul_rn(n_hat, ApB)));
                         bad = bad || !(den > nn_eps);
-                        pw[e] = __fdividef(num, den) * ob.pscale;
+                        // den > nn_eps > 0 here or the value is replaced below: the bare reciprocal (MUFU.RCP + FMUL), without
+                        // __fdividef's range scaling
+                        pw[e] = __fmul_rn(num, rcp_approx(den)) * ob.pscale;
                     }
                     if (bad) {                                    // vanishing denominator (reading a6): the full epilogue, rarely
 #pragma unroll
