@@ -79,8 +79,8 @@ constexpr float kTcPhasorScale = 16.0f;        // sqrt of it: carried by the pha
 // Warp roles of one CTA: 4 control warps, EW epilogue warps, NG generator groups of 4 warps.  Two shapes are built:
 //   (EW, NG) = (8, 3): short items (batches of short light curves): the per-item epilogue is on the critical path
 //   (EW, NG) = (4, 4): long items (hundreds of stages): the generators are, the epilogue is rare
-// Both have 768 threads (80 registers at launch).  Registers are re-split with setmaxnreg: control 40, generators 72,
-// epilogue what is left (112 resp. 152).
+// Both have 768 threads (80 registers at launch).  Registers are re-split with setmaxnreg: short-item shape control 40,
+// generators 72, epilogue 112; long-item shape (single CTAs and CTA pairs) control 32, generators 88, epilogue 96.
 template <int EW, int NG> struct TcRoles {
     static constexpr int kThreads = (4 + EW + 4 * NG) * 32;
     static constexpr int kEpiThreads = EW * 32;
@@ -97,7 +97,7 @@ template <int EW, int NG> struct TcRoles {
 struct TensorParams {
     int nl;             // NL: half-width of a frequency group (multiple of 8, <= 112); group width L = 2 NL = MMA N
     int tile;           // frequencies per tile = 64 * 2 NL
-    int n_ops;          // FP16 operand planes per stage side: 4 (accurate: hi and lo of Z- and W-operands) or 2 (fast)
+    int n_ops;          // FP16 planes of a B stage: 4 (hi and lo of the Z- and W-operands) or 2 (fast_math: hi only)
     int stages_b;       // B-operand ring depth (TMA -> MMA)
     int long_items;     // 1: many stages per item -> the (4 epilogue warps, 4 generator groups) shape; 0: (8, 3)
     int b_plane_bytes;  // bytes of one FP16 plane of a B stage in a CTA's shared memory: 2 NL * 32 (pair mode: NL * 32, the CTA's half)
