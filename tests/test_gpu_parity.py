@@ -306,6 +306,15 @@ def test_config4_shape_host_output_streams(lsp, oracle):
     # summation order (not the result) can differ
     assert np.max(np.abs(host.numpy() - dev.cpu().numpy())) <= 1e-5 * P_ref.max()
     assert_best_parity(tuple(x.cpu().numpy() for x in best), P_ref, w, "f32", oracle)
+    # the same through CTA pairs (three tiles: a phantom fourth), accurate mode, chunks of 7 objects
+    host2 = torch.full((w.n_obj, w.n_freq), float("nan"), dtype=torch.float32).pin_memory()
+    with lsp.Plan(w.f_min, w.f_max, w.n_freq, "f32", tensor_pair=2, n_copy_streams=2, chunk_bytes=7 * w.n_freq * 4) as plan:
+        _, best2 = plan.periodogram_batched(off, t, y, host_out=host2, best=True)
+        info2 = plan.last_call_info()
+        torch.cuda.synchronize()
+    assert info2["tensor_shape"] == 3 and info2["chunks"] == 6
+    assert_power_parity(host2.numpy().astype(np.float64), P_ref, "f32", "c4s host pairs")
+    assert_best_parity(tuple(x.cpu().numpy() for x in best2), P_ref, w, "f32", oracle)
     # pageable destination: plain cudaMemcpyAsync (default) and the paper's staging scheme (LSP_FLAG_PAGEABLE_STAGED)
     for staged in (False, True):
         pageable = torch.full((w.n_obj, w.n_freq), float("nan"), dtype=torch.float32)
@@ -403,8 +412,9 @@ def test_edge_zero_objects_and_errors(lsp):
         assert ei.value.status == 1
 
 
-def test_normalize_and_center_options(lsp, oracle):
-    w = make_config(3, n_obj=5, n_freq=5000)
+@pytest.mark.parametrize("roles,n_freq", [(0, 5000), (3, 20_000)], ids=["auto", "cta-pairs"])
+def test_normalize_and_center_options(lsp, oracle, roles, n_freq):
+    w = make_config(3, n_obj=5, n_freq=n_freq)
     shifted = Workload(w.name, w.offsets, w.t, (w.y + np.float32(3.25)).astype(np.float32), w.f_min, w.f_max, w.n_freq, "f32")
     # center=1 on shifted data == plain call on data centred by numpy in FP64 (to FP32 tolerance)
     yc = shifted.y.astype(np.float64).copy()
@@ -412,9 +422,10 @@ def test_normalize_and_center_options(lsp, oracle):
         s = slice(w.offsets[o], w.offsets[o + 1])
         yc[s] -= yc[s].mean()
     P_ref = oracle.periodogram(w.offsets, w.t, yc, w.f_min, w.f_max, w.n_freq)
-    P, _, _ = gpu_full(lsp, shifted, center=True, best=False)
+    P, _, info = gpu_full(lsp, shifted, center=True, best=False, tensor_roles=roles)
+    assert roles != 3 or info["tensor_shape"] == 3
     assert_power_parity(P, P_ref, "f32", "center")
-    Pn, _, _ = gpu_full(lsp, shifted, center=True, normalize=True, best=False)
+    Pn, _, _ = gpu_full(lsp, shifted, center=True, normalize=True, best=False, tensor_roles=roles)
     for o in range(w.n_obj):
         s = slice(w.offsets[o], w.offsets[o + 1])
         ref = P_ref[o] / (0.5 * (yc[s] @ yc[s]))
