@@ -394,16 +394,12 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
                 acc_i[a][cc].x = acc_i[a][cc].y = T(0);
             }
         unsigned c = 0;
-        while (true) {
-            const int s = c % S;
-            mbar_wait(&full[s], (c / S) & 1);
-            const long long item = meta[s].item;
-            const int last = meta[s].last;
-            if (item < 0) break;
+        // One ring stage: JC observations into this thread's accumulators (step 4).
+        auto contract_stage = [&](int s) {
             const V2* A = ring + (size_t)s * STAGE + offA;
             const V2* B = ring + (size_t)s * STAGE + offB;
 #pragma unroll
-            for (int jj = 0; jj < JC; ++jj) {                  // step 4
+            for (int jj = 0; jj < JC; ++jj) {
                 V2 av[TH], bv[TM];
                 if constexpr (EPC == 2) {           // one LDS.128 = two complex operands
 #pragma unroll
@@ -429,8 +425,37 @@ lsp_factored_ws_kernel(GridParams gp, const int64_t* __restrict__ offsets, const
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[s]);
-            ++c;
-            if (!last) continue;
+        };
+        while (true) {
+            // The stages of one item, TWO per trip of the loop.  ptxas renames the 64 accumulators through the unrolled stage body
+            // and restores the loop-carried assignment with ~250 moves at the back edge (0.47 other instructions per DFMA; a DFMA
+            // holds its scheduler for two cycles, so every one of them displaces half a DFMA).  The renaming is an involution: a
+            // second copy of the body brings the accumulators home and the moves disappear (0.14 per DFMA).
+            long long item;
+            int last;
+            bool fin = false;
+            do {
+                {
+                    const int s = c % S;
+                    mbar_wait(&full[s], (c / S) & 1);
+                    item = meta[s].item;
+                    last = meta[s].last;
+                    if (item < 0) { fin = true; break; }
+                    contract_stage(s);
+                    ++c;
+                }
+                if (last) break;
+                {
+                    const int s = c % S;
+                    mbar_wait(&full[s], (c / S) & 1);
+                    item = meta[s].item;
+                    last = meta[s].last;
+                    if (item < 0) { fin = true; break; }
+                    contract_stage(s);
+                    ++c;
+                }
+            } while (!last);
+            if (fin) break;
 
             // ---- epilogue of `item` (steps 5, 6, 6') -------------------------------------------------------------
             const WsItem w = ws_decode<TILE>(gp, item, offsets);
