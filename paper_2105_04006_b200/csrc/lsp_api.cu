@@ -600,11 +600,20 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     LSP_CUDA(p, cudaSetDevice(c.device));
 
     int64_t total_obs;
+    std::vector<int64_t> off_cache;      // host copy of the offsets when the caller gave none
     if (h_off) {
         if (h_off[0] != 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[0] != 0");
         for (int64_t o = 0; o < n_obj; ++o)
             if (h_off[o + 1] < h_off[o]) return fail(p, LSP_ERR_INVALID_ARG, "offsets decrease at object %lld", (long long)o);
         total_obs = h_off[n_obj];
+    } else if (n_obj < (1 << 17)) {
+        // one synchronous read-back of the whole (small) array instead of its last element now and the rest later (the
+        // two-product tensor mode and the table-budget cuts look at the objects' lengths)
+        off_cache.resize((size_t)n_obj + 1);
+        LSP_CUDA(p, cudaMemcpyAsync(off_cache.data(), d_off, off_cache.size() * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        LSP_CUDA(p, cudaStreamSynchronize(st));
+        total_obs = off_cache[(size_t)n_obj];
+        if (total_obs < 0) return fail(p, LSP_ERR_INVALID_ARG, "offsets[n_obj] < 0");
     } else {
         if (!p->h_offsets_pinned) LSP_CUDA(p, cudaMallocHost((void**)&p->h_offsets_pinned, sizeof(int64_t)));
         LSP_CUDA(p, cudaMemcpyAsync(p->h_offsets_pinned, d_off + n_obj, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
@@ -638,8 +647,7 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
 
     const size_t es = elem_size(c);
     const size_t row_bytes = (size_t)c.n_freq * es;
-    // Host copy of the offsets, fetched only when an object range has to be cut by observation count.
-    std::vector<int64_t> off_cache;
+    // Host copy of the offsets (large batches without one: fetched only when needed).
     auto host_offsets = [&]() -> const int64_t* {
         if (h_off) return h_off;
         if (off_cache.empty()) {
