@@ -221,7 +221,61 @@ lsp_status lsp_best_merge(lsp_plan* plan, int64_t n_obj, int32_t n_parts,
 void lsp_destroy(lsp_plan* plan);
 
 /* Message of the last failure on this plan (plan-owned, valid until the next call on the plan); with
- * plan == NULL, the message of the last failed lsp_plan_create on this thread.  Never NULL. */
+ * plan == NULL, the message of the last failed lsp_plan_create or lsp_best_period_static on this thread.  Never NULL. */
+/*
+ * Best period per object WITHOUT ANY ALLOCATION: no plan, no cudaMalloc / cudaFree / cudaMallocHost, no stream or event
+ * creation, nothing that grows on the device or on the host.
+ *
+ * Who this is for.  Every other call works on a plan, and a plan allocates (lsp_plan_create up front, the calls whenever their
+ * scratch has to grow).  Some programs cannot afford that at the point where they need a period search: a service whose whole
+ * HBM has been handed to its own pool or caching allocator, so that a raw cudaMalloc from a library fails or eats into a budget
+ * it does not own; a real-time or latency-bound loop, where cudaMalloc / cudaFree stall every stream of the device; a plug-in
+ * that runs under a host application's rule "no driver allocations after start-up".  Such a caller passes its inputs and its
+ * three output arrays, all allocated by itself, and the library brings its own scratch: one fixed array of
+ * LSP_STATIC_SCRATCH_BYTES that is part of the library image.  Every GPU whose context loads the library holds that array
+ * from then until the process exits, whether or not this function is ever called.
+ *
+ * What runs: the fused-argmax route of lsp_best_period on the direct kernel family (LSP_KERNEL_DIRECT, one sincos per (t, f)
+ * pair; best period PAPER.md:L87, L105), always with one observation split, followed by the same finalize
+ * kernel; the per-CTA (power, index) candidates and, with center / normalize, the per-object statistics live in the static
+ * array instead of plan-owned memory.  Same grid, tie rule and empty-object convention as lsp_best_period (readings a1, a2,
+ * a7, a8).  Results agree with lsp_best_period on a LSP_KERNEL_DIRECT plan to rounding (bit for bit when that plan also runs
+ * one split), and with the other kernel families within the library's tolerances.
+ *
+ *   cfg          HOST.  Read: f_min, f_max, n_freq, dtype, fast_math, normalize, center, device.  Every other field is ignored
+ *                (a plan's lsp_config can be passed as it is; `kernel` does not select anything here).
+ *   n_obj        objects (>= 0).  n_obj = 0 does the one-time set-up described below and nothing else.
+ *   d_offsets    DEVICE, int64[n_obj+1], non-decreasing, indices into d_t / d_y.  offsets[0] need not be 0, so an object range
+ *                [o0, o0+n) of a larger batch is (d_offsets + o0, same d_t and d_y, d_best_* + o0).
+ *   d_t, d_y     DEVICE, elements of cfg.dtype, as for lsp_best_period.
+ *   d_best_*     DEVICE, n_obj elements each, all three required: period and power (cfg.dtype), grid index (int64; -1, power 0
+ *                and NaN period for an object without observations).
+ *   cuda_stream  cudaStream_t as void* (NULL = default stream); the call is asynchronous on it.
+ *
+ * Limit.  The scratch need is 16 bytes x n_obj x (ceil(n_freq / 1024) + 1) and must not exceed LSP_STATIC_SCRATCH_BYTES
+ * (16 MiB: n_obj x (ceil(n_freq / 1024) + 1) <= 1,048,576 -- e.g. 10,000 objects on a 100,000-point grid, or one object on
+ * a grid of a billion points).  A larger request is rejected with LSP_ERR_UNSUPPORTED before anything is launched; run it as
+ * object ranges.
+ *
+ * Set-up.  The first call for a given device looks up where that device keeps the array and how many SMs it has (two queries,
+ * no allocation) and remembers both for the life of the process; it makes cfg.device current to do so, as every call of this
+ * library does.  Make that first call (n_obj = 0 is enough) before the device is inside a stream capture.
+ *
+ * Sharing.  There is ONE array per device for the whole process.  Nothing in it has to start at zero -- each call writes every
+ * slot it later reads -- so no clearing is done and a call leaves its candidates behind for the next one to overwrite.  Two
+ * calls that can overlap on the same GPU (different streams, different host threads, different "plans" of the caller) would
+ * write the same slots: they RACE and both results are garbage.  Order them on one stream or with events.  Plan-based calls
+ * never touch the array and may overlap with it freely.
+ *
+ * Errors: LSP_ERR_INVALID_ARG (bad grid / dtype / fast_math with FP64 / device ordinal, NULL pointer with n_obj > 0, n_obj < 0),
+ * LSP_ERR_UNSUPPORTED (over the limit above; device not sm_100), LSP_ERR_CUDA.  The message is read with lsp_last_error(NULL).
+ */
+#define LSP_STATIC_SCRATCH_BYTES (16 << 20)
+lsp_status lsp_best_period_static(const lsp_config* cfg /* HOST */, int64_t n_obj,
+                                  const int64_t* d_offsets, const void* d_t, const void* d_y,
+                                  void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                                  void* cuda_stream);
+
 const char* lsp_last_error(const lsp_plan* plan);
 
 /* Bookkeeping of the LAST call on the plan, for benchmarks and tests: how many of the library's kernels it launched,

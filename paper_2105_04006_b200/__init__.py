@@ -7,11 +7,13 @@ from .binding import (  # noqa: F401
     EXPORTS,
     LspConfig,
     LSP_FLAG_PAGEABLE_STAGED,
+    LSP_STATIC_SCRATCH_BYTES,
     LspError,
     Plan,
     load_library,
     lsp_best_merge,
     lsp_best_period,
+    lsp_best_period_static,
     lsp_destroy,
     lsp_periodogram_batched,
     lsp_periodogram_batched_host,

@@ -23,10 +23,12 @@ _KERNELS = {"auto": LSP_KERNEL_AUTO, "direct": LSP_KERNEL_DIRECT, "factored": LS
 _KERNEL_NAMES = {v: k for k, v in _KERNELS.items()}
 
 EXPORTS = ("lsp_plan_create", "lsp_periodogram_batched", "lsp_best_period", "lsp_periodogram_batched_host",
-           "lsp_periodogram_generalized", "lsp_periodogram_generalized_host", "lsp_best_merge", "lsp_destroy",
+           "lsp_periodogram_generalized", "lsp_periodogram_generalized_host", "lsp_best_merge", "lsp_best_period_static",
+           "lsp_destroy",
            "lsp_last_error",
            "lsp_last_call_info", "lsp_set_timing", "lsp_last_kernel_ms", "lsp_version")
 LSP_FLAG_PAGEABLE_STAGED = 1
+LSP_STATIC_SCRATCH_BYTES = 16 << 20      # include/lsp.h: fixed scratch of lsp_best_period_static
 
 
 class LspConfig(ctypes.Structure):
@@ -72,6 +74,8 @@ def load_library(path: Optional[str] = None) -> ctypes.CDLL:
     lib.lsp_periodogram_generalized_host.restype = ctypes.c_int
     lib.lsp_best_merge.argtypes = [vp, i64, i32, vp, vp, vp, vp, vp, vp]
     lib.lsp_best_merge.restype = ctypes.c_int
+    lib.lsp_best_period_static.argtypes = [ctypes.POINTER(LspConfig), i64, vp, vp, vp, vp, vp, vp, vp]
+    lib.lsp_best_period_static.restype = ctypes.c_int
     lib.lsp_destroy.argtypes = [vp]
     lib.lsp_destroy.restype = None
     lib.lsp_last_error.argtypes = [vp]
@@ -160,6 +164,16 @@ def lsp_best_merge(plan, n_obj: int, n_parts: int, d_part_power, d_part_index, d
     _check(load_library().lsp_best_merge(plan, int(n_obj), int(n_parts), _dptr(d_part_power), _dptr(d_part_index),
                                          _dptr(d_best_period), _dptr(d_best_power), _dptr(d_best_index),
                                          _stream_ptr(stream)), plan)
+
+
+def lsp_best_period_static(cfg: LspConfig, n_obj: int, d_offsets, d_t, d_y, d_best_period, d_best_power, d_best_index,
+                           stream=None) -> None:
+    """Best period per object through the library's allocation-free entry point (include/lsp.h): no plan, scratch in a fixed
+    array inside the library (LSP_STATIC_SCRATCH_BYTES), for callers that may not allocate device memory.  All tensors are the
+    caller's own CUDA tensors; asynchronous on `stream`; calls that could overlap on one GPU must be ordered by the caller."""
+    _check(load_library().lsp_best_period_static(ctypes.byref(cfg), int(n_obj), _dptr(d_offsets), _dptr(d_t), _dptr(d_y),
+                                                 _dptr(d_best_period), _dptr(d_best_power), _dptr(d_best_index),
+                                                 _stream_ptr(stream)))
 
 
 def lsp_destroy(plan) -> None:

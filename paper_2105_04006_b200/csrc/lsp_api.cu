@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <utility>
@@ -1274,3 +1275,146 @@ const char* lsp_version(void)
 }
 
 }  // extern "C"
+
+// =============================================================================================================
+// lsp_best_period_static: the one entry point that allocates nothing (include/lsp.h says who needs that and why).
+//
+// It is the best-period route of the direct kernel family -- lsp_object_stats_kernel (only with center / normalize),
+// lsp_direct_kernel with the fused argmax, lsp_finalize_best_kernel: the very kernels the plan-based calls launch -- with
+// the scratch those kernels need (per-CTA argmax candidates, per-object statistics) taken from the file-scope array below
+// instead of plan-owned cudaMalloc memory.  No plan exists on this path, so there are no streams, events or host vectors
+// to create either.
+namespace {
+
+// The scratch itself.  It lives in the library's device image: each GPU context that loads the library gets its own
+// zero-filled copy at load time and keeps it until the process exits.  256-byte alignment keeps both sub-arrays below
+// (16-byte elements) naturally aligned and the base on a memory-sector boundary.
+static __device__ __align__(256) unsigned char g_static_scratch[LSP_STATIC_SCRATCH_BYTES];
+
+// Host code must never pass `g_static_scratch` itself to a kernel.  On the host that name is only nvcc's handle for the
+// symbol -- an ordinary host variable whose address means nothing to the GPU (a kernel given it faults, or on a system where
+// the GPU can reach host memory it quietly scribbles over that handle).  The real address is per device and comes from
+// cudaGetSymbolAddress, asked once per device while that device is current, and kept here.
+constexpr int kStaticMaxDevices = 64;
+struct StaticDevice {
+    unsigned char* scratch;   // DEVICE address of g_static_scratch on this device; NULL = set-up not done yet
+    int sm_count;
+};
+StaticDevice g_static_devices[kStaticMaxDevices];   // zero-initialised
+std::mutex g_static_mutex;                          // guards the table above (first calls from several host threads)
+
+// One-time set-up for `device`; the caller has already made it current.  Two queries, no allocation.
+lsp_status static_device_setup(int device, StaticDevice* out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_devices[device];
+    if (!d.scratch) {
+        int major = 0, sms = 0;
+        LSP_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+        if (major < 10)
+            return fail(nullptr, LSP_ERR_UNSUPPORTED, "device is not sm_100 class (this library is built for sm_100a only)");
+        LSP_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+        unsigned char* ptr = nullptr;
+        LSP_CUDA(nullptr, cudaGetSymbolAddress((void**)&ptr, g_static_scratch));
+        if (!ptr) return fail(nullptr, LSP_ERR_CUDA, "cudaGetSymbolAddress returned a NULL address for the static scratch");
+        d.sm_count = sms;
+        d.scratch = ptr;
+    }
+    *out = d;
+    return LSP_OK;
+}
+
+template <typename T, bool FAST>
+lsp_status static_launch(const lsp_config& c, const StaticDevice& dev, int64_t n_obj, const int64_t* d_off, const T* d_t,
+                         const T* d_y, T* d_best_period, T* d_best_power, int64_t* d_best_index, cudaStream_t st)
+{
+    using V4 = typename Vec4<T>::type;
+    // schedule: as make_schedule does for the direct kernel, with n_split fixed at 1 (partial sums would need N_f-sized scratch)
+    const int64_t tiles4 = (c.n_freq + 4 * kDirectThreads - 1) / (4 * kDirectThreads);
+    const int r = (n_obj * tiles4 >= (int64_t)dev.sm_count * 8) ? 4 : 1;
+    const int64_t n_tiles = (c.n_freq + (int64_t)r * kDirectThreads - 1) / ((int64_t)r * kDirectThreads);
+    // scratch layout: ObjStats[n_obj] | Best[n_obj * n_tiles], both 16-byte elements
+    static_assert(sizeof(ObjStats) == 16 && sizeof(Best) == 16, "scratch layout assumes 16-byte elements");
+    const int64_t need = 16 * n_obj * (n_tiles + 1);
+    if (need > (int64_t)LSP_STATIC_SCRATCH_BYTES)      // not reachable past the documented check in the caller; kept as the guard
+        return fail(nullptr, LSP_ERR_UNSUPPORTED, "static scratch too small: need %lld bytes, have %lld", (long long)need,
+                    (long long)LSP_STATIC_SCRATCH_BYTES);
+    ObjStats* stats = (ObjStats*)dev.scratch;
+    Best* partials = (Best*)(dev.scratch + (size_t)n_obj * sizeof(ObjStats));
+    const bool use_stats = c.center || c.normalize;
+    if (use_stats) {
+        lsp_object_stats_kernel<T><<<(unsigned)n_obj, 128, 0, st>>>(d_off, d_y, stats, c.center, c.normalize);
+        LSP_CUDA(nullptr, cudaGetLastError());
+    }
+    GridParams gp;
+    gp.f_min = c.f_min;
+    gp.df = (c.f_max - c.f_min) / (double)c.n_freq;
+    gp.n_freq = (int)c.n_freq;
+    gp.n_tiles = (int)n_tiles;
+    gp.n_split = 1;
+    gp.obj_base = 0;
+    // Every CTA (object, tile) stores its candidate, and the finalize kernel reads exactly those n_obj * n_tiles slots (and the
+    // statistics kernel above wrote the n_obj entries the main kernel reads): whatever an earlier call left in the array is
+    // overwritten before it is looked at, so nothing is cleared here.
+    const unsigned grid = (unsigned)(n_obj * n_tiles);
+    const ObjStats* ks = use_stats ? stats : nullptr;
+    if (r == 4)
+        lsp_direct_kernel<T, FAST, 4, false><<<grid, kDirectThreads, 0, st>>>(gp, d_off, d_t, d_y, ks, (T*)nullptr, partials,
+                                                                             (V4*)nullptr, n_obj, (const T*)nullptr);
+    else
+        lsp_direct_kernel<T, FAST, 1, false><<<grid, kDirectThreads, 0, st>>>(gp, d_off, d_t, d_y, ks, (T*)nullptr, partials,
+                                                                             (V4*)nullptr, n_obj, (const T*)nullptr);
+    LSP_CUDA(nullptr, cudaGetLastError());
+    const int wpb = 4;
+    lsp_finalize_best_kernel<T><<<(unsigned)((n_obj + wpb - 1) / wpb), wpb * 32, 0, st>>>(gp, d_off, partials, (int)n_tiles, n_obj,
+                                                                                         d_best_period, d_best_power, d_best_index);
+    LSP_CUDA(nullptr, cudaGetLastError());
+    return LSP_OK;
+}
+
+}  // namespace
+
+extern "C" lsp_status lsp_best_period_static(const lsp_config* cfg, int64_t n_obj, const int64_t* d_offsets, const void* d_t,
+                                             const void* d_y, void* d_best_period, void* d_best_power, int64_t* d_best_index,
+                                             void* cuda_stream)
+{
+    if (!cfg) return fail(nullptr, LSP_ERR_INVALID_ARG, "cfg is NULL");
+    const lsp_config& c = *cfg;
+    if (!(c.f_min > 0.0) || !(c.f_max > c.f_min) || !std::isfinite(c.f_max))
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "need 0 < f_min < f_max (got %g, %g)", c.f_min, c.f_max);
+    if (c.n_freq < 1 || c.n_freq > 0x7fffffffLL) return fail(nullptr, LSP_ERR_INVALID_ARG, "n_freq out of range");
+    if (c.dtype != LSP_F32 && c.dtype != LSP_F64) return fail(nullptr, LSP_ERR_INVALID_ARG, "unknown dtype");
+    if (c.fast_math != 0 && c.fast_math != 1) return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math must be 0 or 1");
+    if (c.fast_math && c.dtype == LSP_F64) return fail(nullptr, LSP_ERR_INVALID_ARG, "fast_math (MUFU sincos) is FP32-only");
+    if (n_obj < 0) return fail(nullptr, LSP_ERR_INVALID_ARG, "n_obj < 0");
+    if (n_obj > 0 && (!d_offsets || !d_t || !d_y || !d_best_period || !d_best_power || !d_best_index))
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "lsp_best_period_static: NULL argument (offsets, t, y and all three outputs are required)");
+    // the documented limit, checked on the host before any CUDA call: 16 B x n_obj x (ceil(n_freq / 1024) + 1)
+    const int64_t tiles_doc = (c.n_freq + 1023) / 1024 + 1;
+    const int64_t max_slots = (int64_t)LSP_STATIC_SCRATCH_BYTES / 16;
+    if (n_obj > max_slots / tiles_doc)
+        return fail(nullptr, LSP_ERR_UNSUPPORTED,
+                    "request exceeds the static scratch: n_obj (%lld) x (ceil(n_freq / 1024) + 1 = %lld) x 16 bytes > %lld bytes; "
+                    "run the batch as object ranges of at most %lld objects",
+                    (long long)n_obj, (long long)tiles_doc, (long long)LSP_STATIC_SCRATCH_BYTES, (long long)(max_slots / tiles_doc));
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0) {
+        cudaGetLastError();
+        return fail(nullptr, LSP_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+    }
+    if (c.device < 0 || c.device >= n_dev || c.device >= kStaticMaxDevices)
+        return fail(nullptr, LSP_ERR_INVALID_ARG, "device ordinal out of range");
+    LSP_CUDA(nullptr, cudaSetDevice(c.device));
+    StaticDevice dev{};
+    const lsp_status es = static_device_setup(c.device, &dev);
+    if (es != LSP_OK) return es;
+    if (n_obj == 0) return LSP_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (c.dtype == LSP_F64)
+        return static_launch<double, false>(c, dev, n_obj, d_offsets, (const double*)d_t, (const double*)d_y, (double*)d_best_period,
+                                            (double*)d_best_power, d_best_index, st);
+    return c.fast_math ? static_launch<float, true>(c, dev, n_obj, d_offsets, (const float*)d_t, (const float*)d_y,
+                                                    (float*)d_best_period, (float*)d_best_power, d_best_index, st)
+                       : static_launch<float, false>(c, dev, n_obj, d_offsets, (const float*)d_t, (const float*)d_y,
+                                                     (float*)d_best_period, (float*)d_best_power, d_best_index, st);
+}
