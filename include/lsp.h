@@ -80,9 +80,14 @@ typedef struct lsp_config {
                                    (8 epilogue warps), 2 = long-item shape (4 epilogue warps)               */
     int32_t tensor_b_stages;/* tensor path: depth of the B-operand (TMA) ring, 2..8; 0 = library default    */
     int32_t tensor_products;/* tensor path, fast_math = 0: FP16 tcgen05 products per multiply-accumulate.
-                                   2 (= 0, default): a_hi (b_hi + b_lo) -- the generated operand a = y e^{i alpha} is
-                                   one FP16 (11 significand bits), the tabulated one an FP16 pair (22 bits);
-                                   3: a_hi b_hi + a_hi b_lo + a_lo b_hi -- both operands FP16 pairs                 */
+                                   3 (= 0, default): a_hi b_hi + a_hi b_lo + a_lo b_hi -- both operands FP16 pairs
+                                   (22 significand bits): within the FP32 tolerance on every cadence tested, ~1e-6 of max P;
+                                   2 (opt-in, ~1.35x faster on long objects, no gain on short ones): a_hi (b_hi + b_lo) --
+                                   the generated operand a = y e^{i alpha} is ONE FP16 (11 bits).  Its error follows the
+                                   conditioning of the 2 x 2 system: <= 4.5e-4 of max P on year-long cadences, but several
+                                   1e-3 (over the 1e-3 tolerance) on noise-only objects observed on <= 12 nights inside a
+                                   0.05 d window -- choose it only for well-sampled data.  A call that holds
+                                   an object of fewer than 32 observations runs with 3 all the same                 */
     int32_t tensor_pair;    /* tensor path: CTA pairs (2-CTA clusters, tcgen05 cta_group::2: two frequency tiles of one
                                    object share every tabulated-operand stage).  0 = when work items are long (>= 48
                                    stages of 16 observations), 1 = never, 2 = whenever the grid has >= 2 tiles         */
@@ -172,7 +177,9 @@ lsp_status lsp_periodogram_generalized(lsp_plan* plan, int64_t n_obj,
  * h_out_power may be NULL for best-period-only output).  Inputs are copied to plan-owned device buffers on cuda_stream; full
  * periodograms come back round by round through the plan's chunk ring and copy streams (chunk_bytes per round: the D2H of one
  * round overlaps the kernels of the next), best-period arrays by one small D2H each.  Returns after everything
- * has landed on the host.  Errors as lsp_periodogram_generalized.
+ * has landed on the host.  LSP_FLAG_PAGEABLE_STAGED does not apply to this call: a pageable h_out_power is handed to
+ * cudaMemcpyAsync as it is (the staged scheme belongs to lsp_periodogram_batched / _batched_host).
+ * Errors as lsp_periodogram_generalized.
  */
 lsp_status lsp_periodogram_generalized_host(lsp_plan* plan, int64_t n_obj,
                                             const int64_t* h_offsets, const void* h_t, const void* h_y, const void* h_sigma,
@@ -217,11 +224,6 @@ lsp_status lsp_best_merge(lsp_plan* plan, int64_t n_obj, int32_t n_parts,
                           void* d_best_period, void* d_best_power, int64_t* d_best_index,
                           void* cuda_stream);
 
-/* Frees the plan and everything it owns (synchronises its streams first).  NULL is a no-op. */
-void lsp_destroy(lsp_plan* plan);
-
-/* Message of the last failure on this plan (plan-owned, valid until the next call on the plan); with
- * plan == NULL, the message of the last failed lsp_plan_create or lsp_best_period_static on this thread.  Never NULL. */
 /*
  * Best period per object WITHOUT ANY ALLOCATION: no plan, no cudaMalloc / cudaFree / cudaMallocHost, no stream or event
  * creation, nothing that grows on the device or on the host.
@@ -276,13 +278,18 @@ lsp_status lsp_best_period_static(const lsp_config* cfg /* HOST */, int64_t n_ob
                                   void* d_best_period, void* d_best_power, int64_t* d_best_index,
                                   void* cuda_stream);
 
+/* Frees the plan and everything it owns (synchronises its streams first).  NULL is a no-op. */
+void lsp_destroy(lsp_plan* plan);
+
+/* Message of the last failure on this plan (plan-owned, valid until the next call on the plan); with
+ * plan == NULL, the message of the last failed lsp_plan_create or lsp_best_period_static on this thread.  Never NULL. */
 const char* lsp_last_error(const lsp_plan* plan);
 
 /* Bookkeeping of the LAST call on the plan, for benchmarks and tests: how many of the library's kernels it launched,
  * (t,f) pairs evaluated, the kernel family used (lsp_kernel), observation splits per (object, tile), -- host-output
  * calls only -- chunks copied, the tensor kernel's warp-role shape (0 = tensor kernel not used, 1 = short-item
  * shape, 2 = long-item shape, 3 = long-item shape on CTA pairs; see lsp_config.tensor_roles, tensor_pair) and its FP16 products per multiply-accumulate in the last
- * launch (0 = tensor kernel not used; 1 = fast_math; 2 or 3: lsp_config.tensor_products -- a launch that holds an object
+ * launch (0 = tensor kernel not used; 1 = fast_math; 2 or 3: lsp_config.tensor_products -- a call that holds an object
  * of fewer than 32 observations runs with 3 whatever the plan says).  Any pointer may be NULL. */
 void lsp_last_call_info(const lsp_plan* plan, int64_t* n_launches, int64_t* n_pairs, int32_t* kernel_used,
                         int32_t* n_split, int64_t* n_chunks, int32_t* tensor_shape, int32_t* tensor_products);

@@ -60,7 +60,7 @@ struct lsp_plan {
     DeviceBuffer tc_table;        // B-operand table of the launch's objects (tensor path)
     size_t tc_table_budget = (size_t)12 << 30;    // objects per launch are capped so the table stays below this
     int tc_stages_b = 0;          // B-operand ring depth of the tensor kernel; 0 = as many as fit (cfg.tensor_b_stages)
-    int tc_products = 2;          // FP16 products per MAC of the accurate tensor mode: 2 or 3 (cfg.tensor_products)
+    int tc_products = 3;          // FP16 products per MAC of the accurate tensor mode: 3 (default) or 2 (cfg.tensor_products)
     int tc_pair = 0;              // CTA pairs on the tensor path: 0 = when items are long, 1 = never, 2 = whenever there are >= 2 tiles (cfg.tensor_pair)
     int tc_roles = 0;             // 0 = by item length, 1 = force the short-item role shape, 2 = force the long-item one (cfg.tensor_roles)
     DeviceBuffer in_off, in_t, in_y, in_sigma, out_best;   // device copies of host inputs / best-period outputs (lsp_periodogram_batched_host)
@@ -180,10 +180,14 @@ struct Schedule {
     TensorParams tp;   // tensor path only
 };
 
-// Two-product tensor mode: the generated operand a = y e^{i alpha} is a single FP16, i.e. every term of a sum carries a relative
-// error of up to 2^-12.  That is harmless while step 5 is well conditioned (measured <= 4.5e-4 of max P on pure-noise objects,
-// a few 1e-5 when a signal dominates) but not for objects of a handful of observations, whose 2 x 2 systems are close to
-// singular at many grid frequencies: a launch that holds an object shorter than this runs with three products.
+// Two-product tensor mode (lsp_config.tensor_products = 2, an explicit opt-in; the default is three): the generated operand
+// a = y e^{i alpha} is a single FP16, i.e. every term of a sum carries a relative error of up to 2^-12.  What that does to P is set
+// by the conditioning of step 5's 2 x 2 system (n^2 - c2^2 - s2^2), not by N_t: a few 1e-5 of max P when a signal dominates,
+// <= 4.5e-4 on pure-noise objects observed over a year, but several 1e-3 -- over the FP32 tolerance -- on noise-only objects
+// taken on a handful of nights inside a short nightly window (tests/test_gpu_parity.py, few-night cadences).
+// The caller who opts in vouches for the cadence.  One guard stays: objects of a handful of observations are close to singular
+// at many grid frequencies whatever the cadence, so a CALL that holds an object shorter than this runs with three products.
+// The decision is per call -- never per launch -- so chunks and table-budget sub-ranges of one call all run the same mode.
 constexpr int64_t kTcMinNtTwoProducts = 32;
 
 // Smallest N_t > 0 among objects [o0, o0 + no) (INT64_MAX if all are empty); `ho` = host copy of the CSR offsets.
@@ -221,7 +225,7 @@ Schedule make_schedule(const lsp_plan* p, int64_t n_obj, int64_t total_obs, int 
     if (k == LSP_KERNEL_TENSOR) {
         tensor_tiles((c.n_freq + max_tile - 1) / max_tile);
         s.tp.n_ops = c.fast_math ? 2 : 4;
-        s.products = c.fast_math ? 1 : ((p->tc_products == 3 || min_nt < kTcMinNtTwoProducts) ? 3 : 2);
+        s.products = c.fast_math ? 1 : ((p->tc_products != 2 || min_nt < kTcMinNtTwoProducts) ? 3 : 2);
         s.direct_r = 0;
         slots = p->sm_count;
     } else if (k == LSP_KERNEL_FACTORED) {
@@ -334,7 +338,7 @@ cudaError_t launch_main(lsp_plan* p, const Schedule& s, const GridParams& gp, in
             };
             p->tensor_shape = s.tp.pair ? 3 : (s.tp.long_items ? 2 : 1);
             p->tensor_products = s.products;
-            // precision mode of the kernel template: 1 = fast_math, 2 = two products (default), 0 = three (tensor_products = 3)
+            // precision mode of the kernel template: 1 = fast_math, 2 = two products (opt-in), 0 = three (the default)
             auto go_pm = [&](auto pm_tag) -> cudaError_t {
                 constexpr int PM = decltype(pm_tag)::value;
                 if (s.tp.weighted && s.tp.gls == 2)      // generalised mode, weighted W slot + ZK09's epilogue fused
@@ -664,10 +668,12 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
     // Steps 2-6' for objects [o0, o0 + no) holding `obs` observations, asynchronous on the caller's stream: `out` (device, may be
     // NULL) receives rows relative to o0.  One launch sequence, except on the tensor path when the B-operand table of the range
     // would exceed its memory budget: then the objects go in sub-ranges (same results: an object's sums never span launches).
-    // two-product tensor mode: the launch's shortest object decides (kTcMinNtTwoProducts); needs the offsets on the host
+    // two-product tensor mode (opt-in): the CALL's shortest object decides for every launch of the call (kTcMinNtTwoProducts), so
+    // chunks, table-budget sub-ranges and the uncut device call give the same bits; needs the offsets on the host
     const bool need_min_nt = s.kernel == LSP_KERNEL_TENSOR && s.products == 2;
     if (need_min_nt && !host_offsets()) return fail(p, LSP_ERR_CUDA, "reading offsets back failed");
-    auto min_nt_of = [&](int64_t o0, int64_t no) { return need_min_nt ? range_min_nt(host_offsets(), o0, no) : INT64_MAX; };
+    const int64_t call_min_nt = need_min_nt ? range_min_nt(host_offsets(), 0, n_obj) : INT64_MAX;
+    auto min_nt_of = [&](int64_t, int64_t) { return call_min_nt; };
     auto run_objs = [&](int64_t o0, int64_t no, int64_t obs, void* out) -> lsp_status {
         int n_parts = 0;
         const Schedule sc = make_schedule(p, no, obs, s.kernel, min_nt_of(o0, no));
@@ -711,7 +717,7 @@ lsp_status run_call(lsp_plan* p, int64_t n_obj, const int64_t* d_off, const int6
         if (e != LSP_OK) return e;
     }
     // A pinned (or registered) destination is written directly by the async copies.  A pageable one is either handed to
-    // cudaMemcpyAsync as it is (the driver stages it; default) or goes the paper's way (L117; LSP_PAGEABLE=staged): D2H into a
+    // cudaMemcpyAsync as it is (the driver stages it; default) or goes the paper's way (L117; LSP_FLAG_PAGEABLE_STAGED): D2H into a
     // pinned staging slot, then a host-side memcpy into the caller's buffer run by the copy stream's callback thread, the
     // slot's "free" event covering both the device slot and its staging twin.  Measured on config 4 (4 GB): pinned 76 ms,
     // pageable plain 229 ms, pageable staged 283 ms -- the callback threads' memcpy (~14 GB/s) is slower than the driver's
@@ -836,7 +842,7 @@ lsp_status lsp_plan_create(const lsp_config* cfg, lsp_plan** out_plan)
     if (cfg->table_budget_bytes > 0) p->tc_table_budget = (size_t)cfg->table_budget_bytes;
     p->pageable_mode = (cfg->flags & LSP_FLAG_PAGEABLE_STAGED) ? 0 : 1;
     p->tc_roles = cfg->tensor_roles;
-    p->tc_products = cfg->tensor_products == 3 ? 3 : 2;
+    p->tc_products = cfg->tensor_products == 2 ? 2 : 3;            // three products unless the caller opts in to two
     p->tc_pair = cfg->tensor_pair;
     if (cfg->tensor_b_stages > 0) p->tc_stages_b = cfg->tensor_b_stages;
     const int n_slots = p->cfg.n_copy_streams + 1;

@@ -10,6 +10,7 @@ from .configs import (  # noqa: F401
     make_config,
     single_object,
     asteroid_batch,
+    few_night_batch,
     config_seed,
     as_dtype,
     C5_NT,

@@ -128,6 +128,31 @@ def asteroid_batch(rng: np.random.Generator, n_obj: int, *, nt_lo=50, nt_hi=500,
     return offsets, t, y, amps, periods_h
 
 
+def few_night_batch(n_nights: int, window: float, *, n_obj: int = 30, nt_lo: int = 32, nt_hi: int = 60, signal: bool = False,
+                    n_freq: int = 100_000, dtype: str = "f32", seed: int = 0) -> Workload:
+    """Ill-conditioned survey cadences (ZTF/LSST-like records of a few short nights): the asteroid_batch
+    recipe with short objects (N_t = integers[nt_lo, nt_hi]) on `n_nights` nights and a nightly window of `window` days, on
+    config 3's grid.  signal = False: y = N(0, 1) only (nothing lifts max P above the noise floor -- the hardest case for a
+    reduced-precision contraction); signal = True: asteroid_batch's sinusoid + N(0, 0.05^2).  Seed: BASE_SEED + 9000 + seed."""
+    rng = np.random.Generator(np.random.PCG64(BASE_SEED + 9000 + seed))
+    if signal:
+        offsets, t, y, _, _ = asteroid_batch(rng, n_obj, nt_lo=nt_lo, nt_hi=nt_hi, n_nights=n_nights, intranight=window)
+    else:
+        n_t = rng.integers(nt_lo, nt_hi + 1, size=n_obj)
+        offsets = np.zeros(n_obj + 1, dtype=np.int64)
+        np.cumsum(n_t, out=offsets[1:])
+        t = np.empty(int(offsets[-1]), dtype=np.float64)
+        y = np.empty_like(t)
+        for i in range(n_obj):
+            n = int(n_t[i])
+            ti = np.sort(rng.integers(0, n_nights, size=n) + rng.uniform(0.0, window, n))
+            t[offsets[i]:offsets[i + 1]] = ti
+            y[offsets[i]:offsets[i + 1]] = _centre(rng.normal(0.0, 1.0, n))
+    w = Workload(f"fewnight_{n_nights}x{window}_{'signal' if signal else 'noise'}", offsets, t, y, 24.0 / 200.0, 24.0, n_freq,
+                 meta={"n_nights": n_nights, "window": window})
+    return as_dtype(w, dtype)
+
+
 def make_config(config: int, *, dtype: str = None, n_obj: int = None, n_freq: int = None,
                 n_t: int = None, point: int = 0) -> Workload:
     """BASELINE.json config `config` (1..5).  `n_obj`, `n_freq`, `n_t` shrink a config for parity tests
