@@ -35,7 +35,9 @@
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): chi^2 reduction of a brute-force
  * least-squares sinusoid fit, time-shift and amplitude-scaling invariance, exact recovery of an on-grid
  * noiseless sinusoid, the N_t = 2 closed form, the even-sampling reduction to the textbook DFT
- * periodogram, scipy.signal.lombscargle (library call), and the long-double self-bound.
+ * periodogram, scipy.signal.lombscargle (library call), the long-double self-bound, the phase reduction
+ * against exact rational arithmetic at f*t ~ 1.8e5 cycles (p11: fractions.Fraction products mod 1), and the
+ * object-parallel loop of the batch driver against single-object calls (n_threads = 1).
  * No printed P values exist in the paper, so "parity on paper data" is unpinned;
  * every function below is pinned by the identities listed.
  */

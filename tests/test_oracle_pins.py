@@ -232,3 +232,65 @@ def test_config3_peak_is_half_rotation_period(oracle):
         yy = one.y
         hits += P.max() > 0.25 * 0.5 * (yy @ yy)
     assert hits == 3
+
+
+# ---- p11: the low-order bits of the phase at config-2 magnitudes, against exact rational arithmetic -------------
+def test_p11_phase_reduction_against_exact_rationals(oracle):
+    """At config 2's scale f*t reaches ~1.8e5 cycles: the fractional part keeps only ~35 of the product's 53 bits unless the
+    rounding error of f*t is carried along (the oracle's compensation term).  Here the phase of every (f_k, t_j) is reduced
+    with exact rationals -- Fraction(f) * Fraction(t) mod 1, every double is a dyadic rational -- and the power follows from
+    the tau-free normal equations  P = 1/2 b^T M^-1 b  (b = sum y (cos, sin), M = sum (cos, sin)(cos, sin)^T), a route that
+    shares neither the reduction nor Eq. 1's tau with the oracle.  Dropping or mis-signing the compensation term moves the
+    phase by ulp(1.8e5)/2 ~ 1.5e-11 cycles and P by ~1e-10 of max P; the bound is 1e-12."""
+    from fractions import Fraction
+    rng = np.random.default_rng(1105)
+    f_min, f_max, n_freq = 0.05, 50.0, 1_000_000                       # config 2's grid
+    ks = np.sort(rng.choice(np.arange(900_000, n_freq), 20, replace=False))      # f ~ 45-50 c/d
+    t = np.sort(rng.uniform(3000.0, 3650.0, 40))                        # f * t ~ 1.4e5 .. 1.8e5 cycles
+    y = rng.normal(0.0, 1.0, t.size)
+    y -= y.mean()
+    off = np.array([0, t.size], dtype=np.int64)
+    P = oracle.periodogram(off, t, y, f_min, f_max, n_freq, k_list=ks)[0]
+    f = oracle.grid(f_min, f_max, n_freq, k_list=ks)
+    ref = np.empty_like(P)
+    for i, fk in enumerate(f):
+        ff = Fraction(float(fk))
+        r = np.array([float(((ff * Fraction(float(tj))) % 1)) for tj in t])          # exact product, exact mod, one rounding
+        c, s = np.cos(TWO_PI * r), np.sin(TWO_PI * r)
+        b = np.array([y @ c, y @ s])
+        M = np.array([[c @ c, c @ s], [c @ s, s @ s]])
+        ref[i] = 0.5 * b @ np.linalg.solve(M, b)
+    assert np.max(np.abs(P - ref)) <= 1e-12 * ref.max()
+    # the pin bites: the same evaluation with the naively reduced double product is off by far more than the bound
+    naive = np.empty_like(P)
+    for i, fk in enumerate(f):
+        r = np.mod(fk * t, 1.0)
+        c, s = np.cos(TWO_PI * r), np.sin(TWO_PI * r)
+        b = np.array([y @ c, y @ s])
+        M = np.array([[c @ c, c @ s], [c @ s, s @ s]])
+        naive[i] = 0.5 * b @ np.linalg.solve(M, b)
+    assert np.max(np.abs(naive - ref)) > 1e-11 * ref.max()
+
+
+# ---- the object-parallel branch of the batch driver (n_obj >= 2 x threads), reachable on any box with one thread -------
+def test_object_parallel_branch_equals_single_object_calls(oracle):
+    """lsp_oracle_periodogram loops over objects in parallel when n_obj >= 2 x threads, else over frequencies.  On a many-core
+    box small CPU batches only ever take the second loop; with n_threads = 1 a 5-object batch takes the first.  Both must
+    return, row for row, what single-object calls return (those take the frequency loop)."""
+    rng = np.random.default_rng(77)
+    series = [_rand_series(rng, n) for n in (5, 0, 31, 2, 64)]
+    off, t, y = _csr(*series)
+    f_min, f_max, n_freq = 0.1, 4.0, 301
+    ks = np.array([0, 7, 150, 300])
+    _, default_threads = oracle.periodogram(off[:2], t[:5], y[:5], f_min, f_max, n_freq, return_threads=True)
+    try:
+        P1, used = oracle.periodogram(off, t, y, f_min, f_max, n_freq, n_threads=1, return_threads=True)
+        Pk = oracle.periodogram(off, t, y, f_min, f_max, n_freq, k_list=ks, n_threads=1)
+    finally:
+        oracle.periodogram(off[:2], t[:5], y[:5], f_min, f_max, n_freq, n_threads=default_threads)     # give the threads back
+    assert used == 1 and P1.shape == (5, n_freq)
+    for o, (to, yo) in enumerate(series):
+        single = oracle.periodogram(np.array([0, len(to)], dtype=np.int64), to, yo, f_min, f_max, n_freq)[0]
+        assert np.array_equal(P1[o], single)
+        assert np.array_equal(Pk[o], single[ks])
+    assert np.all(P1[1] == 0.0)
