@@ -8,9 +8,14 @@ A "step" is one pass of the whole hot path (SURVEY.md section 8(a) steps 1-6/6',
 batch of seeded synthetic input.  Default workload: BASELINE.json configs[1] (single object, N_t = 10,000,
 N_f = 1,000,000, full periodogram) in FP32 (the primary keys).  The same line then carries, as short objects,
   fp64           the same workload in FP64 (value, e2e, roofline)
-  fp32_fma_pipe  the all-FP32 FFMA2 contraction on the FMA pipe (north_star's "FP32 issue-bound roofline")
+  fp32_fma_pipe  the all-FP32 FFMA2 contraction on the FMA pipe (north_star's "FP32 issue-bound roofline": value, e2e, roofline, clocks)
+  fp32_tensor_2products  the tensor path's two-product opt-in (faster, not safe on few-night cadences)
   c3, c4         BASELINE.json configs[2] (batch, fused best period) and configs[3] (4 GB of periodograms to pinned host
                  through the copy streams: T_compute, T_d2h, T_pipelined)
+  fast_vs_accurate  MUFU (__sincosf-class) vs accurate sincos: the paper-shaped direct kernel and the tensor path
+  c5             BASELINE.json configs[4], compact: pairs/s and roofline fraction of the 12 sweep points per dtype
+`dtype` is the arithmetic of the multiply-accumulates ("f16x3-split/f32acc" for the default tensor path, "f32", "f64");
+config.io_dtype is the element type of t, y and the powers.
 and, with --variants, the comparison legs (fast_math, the paper-shaped direct kernels, the generalised mode).
   value       device-resident: inputs and output in HBM, CUDA events around each step on the launching stream
   e2e         the same pass through lsp_periodogram_batched_host: pinned HOST inputs, H2D + kernels + D2H inside
@@ -46,9 +51,9 @@ SM_MAX_HZ = 1965e6
 FP32_LANES = 128      # FP32 FMA lanes per SM per clock
 FP64_LANES = 64       # FP64 FMA lanes per SM per clock
 FLOP_PER_PAIR = 8.0   # factored formulation: 4 FMA per (t,f) pair ("4 FMA = 8 flop/pair")
-# Tensor path: the same 4 MAC per pair as one FP16 GEMM; the accurate mode issues two products per MAC (a_hi (b_hi + b_lo),
-# the library default) or three (a_hi b_hi + a_hi b_lo + a_lo b_hi; --tensor-products 3), fast_math one.
-TENSOR_PRODUCTS = {False: 2, True: 1}
+# Tensor path: the same 4 MAC per pair as one FP16 GEMM; the accurate mode issues three products per MAC (a_hi b_hi + a_hi b_lo +
+# a_lo b_hi, the library default) or two (a_hi (b_hi + b_lo); --tensor-products 2, an opt-in), fast_math one.
+TENSOR_PRODUCTS = {False: 3, True: 1}
 TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 burst; fp16 : bf16 nominal ratio is 1)
 
 
@@ -56,16 +61,21 @@ TENSOR_PEAK_FALLBACK = 1590.0     # TFLOP/s, B200_PROFILING.md fallback (bf16 bu
 # committed `ncu --set full` summary of the same workload and kernel (profiles/*.csv; the commands are in the README beside
 # them).  No capture for this (workload, kernel) -> null.  Newest round first.
 NCU_SUMMARIES = {
-    ("c2", "tensor", "f32"): ("profiles/r02_ncu_full_tensor_f32_c2.csv", "profiles/r01_ncu_full_tensor_f32_c2.csv"),
-    ("c3", "tensor", "f32"): ("profiles/r02_ncu_full_tensor_f32_c3.csv", "profiles/r01_ncu_full_tensor_f32_c3.csv"),
-    ("c2", "factored", "f32"): ("profiles/r02_ncu_full_factored_ws_f32.csv", "profiles/r01_ncu_full_factored_ws_f32.csv"),
-    ("c2", "factored", "f64"): ("profiles/r02_ncu_full_factored_ws_f64.csv", "profiles/r01_ncu_full_factored_ws_f64.csv"),
+    # tensor kernel: keyed by FP16 products per MAC as well (r02 captures: the two-product launches; r03: three products)
+    ("c2", "tensor", "f32", 3): ("profiles/r03_ncu_full_tensor_f32_c2_3products.csv",),
+    ("c3", "tensor", "f32", 3): ("profiles/r03_ncu_full_tensor_f32_c3_3products.csv",),
+    ("c2", "tensor", "f32", 2): ("profiles/r02_ncu_full_tensor_f32_c2.csv",),
+    ("c3", "tensor", "f32", 2): ("profiles/r02_ncu_full_tensor_f32_c3.csv",),
+    ("c2", "factored", "f32"): ("profiles/r02_ncu_full_factored_ws_f32.csv",),
+    ("c2", "factored", "f64"): ("profiles/r02_ncu_full_factored_ws_f64.csv",),
 }
 
 
-def ncu_traffic(workload: str, kernel: str, dtype: str):
-    """(bytes per launch, file) from the newest committed ncu summary of this workload / kernel, or (None, None)."""
-    for rel in NCU_SUMMARIES.get((workload, kernel, dtype), ()):
+def ncu_traffic(workload: str, kernel: str, dtype: str, products: int = 0):
+    """(bytes per launch, file) from the newest committed ncu summary of this workload / kernel (tensor kernel: of this
+    product count; a capture of another precision mode is another kernel), or (None, None)."""
+    key = (workload, kernel, dtype) if kernel != "tensor" else (workload, kernel, dtype, int(products))
+    for rel in NCU_SUMMARIES.get(key, ()):
         path = os.path.join(ROOT, rel)
         if not os.path.exists(path):
             continue
@@ -119,18 +129,34 @@ def measured_tensor_peak():
         return TENSOR_PEAK_FALLBACK, "of fallback (B200_PROFILING.md 1.59 PFLOP/s bf16 burst; fp16:bf16 = 1)"
 
 
+def tensor_instantiation(shape: int, products: int) -> str:
+    """The lsp_tensor_kernel instantiation launch_main picks (csrc/lsp_api.cu) for a standard call, from lsp_last_call_info:
+    <T, PM (0 = three products, 2 = two, 1 = fast_math), epilogue warps, generator groups, GM = 0[, PAIR, max NL]>."""
+    pm = {1: 1, 2: 2, 3: 0}.get(int(products), 0)
+    if shape == 3:
+        return "lsp_tensor_kernel<float,%d,4,4,0,true,112>" % pm
+    return "lsp_tensor_kernel<float,%d,%s,0>" % (pm, "4,4" if shape == 2 else "8,3")
+
+
+def arithmetic_dtype(kernel: str, dtype: str, products: int) -> str:
+    """Machine-readable arithmetic of the contraction (the line's `dtype`): what the multiply-accumulates really are."""
+    if kernel == "tensor":
+        return {1: "f16/f32acc", 2: "f16x2-split/f32acc", 3: "f16x3-split/f32acc"}.get(int(products), "f16-split/f32acc")
+    return dtype
+
+
 def roofline(kernel: str, dtype: str, fast: bool, pairs: float, k_ms: float, pipe_ops: float, workload: str = "",
-             products: int = 0):
+             products: int = 0, shape: int = 0):
     """Roofline object of the dominant kernel: achieved = algorithmic flop per launch
     (8 flop per (t,f) pair x pairs) / mean launch duration measured with CUDA events on the launching stream."""
     achieved = pairs * FLOP_PER_PAIR / (k_ms * 1e-3) / 1e12
-    traffic, traffic_from = (None, None) if fast else ncu_traffic(workload, kernel, dtype)
+    traffic, traffic_from = (None, None) if fast else ncu_traffic(workload, kernel, dtype, products)
     if kernel == "tensor":
         peak, prov = measured_tensor_peak()
         prod = products if products else TENSOR_PRODUCTS[bool(fast)]
         return {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_from": traffic_from,
-                "kernel": "lsp_tensor_kernel<float,%d>" % int(bool(fast)), "flop_per_pair": FLOP_PER_PAIR,
+                "kernel": tensor_instantiation(shape, prod), "flop_per_pair": FLOP_PER_PAIR,
                 "peak_is": prov,
                 "executed_flop_per_pair": FLOP_PER_PAIR * prod,
                 "executed_tflops": achieved * prod, "frac_executed": achieved * prod / peak,
@@ -170,7 +196,7 @@ def parse_args():
     ap.add_argument("--fast-math", action="store_true", help="FP32: MUFU.SIN/COS instead of accurate sincospif")
     ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "factored", "tensor"])
     ap.add_argument("--tensor-products", type=int, default=0, choices=[0, 2, 3],
-                    help="tensor path, accurate mode: FP16 products per MAC (lsp_config.tensor_products; 0 = library default = 2)")
+                    help="tensor path, accurate mode: FP16 products per MAC (lsp_config.tensor_products; 0 = library default = 3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-secondary", action="store_true", help="primary leg only (no fp64 / fp32_fma_pipe / c3 / c4 objects)")
     ap.add_argument("--variants", action="store_true", help="add the comparison legs: fast_math, direct kernels, generalised mode")
@@ -459,14 +485,13 @@ ARITHMETIC = {
 
 
 def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_clocks: bool, kernel=None, fast=None,
-            with_e2e: bool = True, workload=None, steps=None):
+            with_e2e: bool = True, workload=None, steps=None, tensor_products=None):
     name = args.workload if workload is None else workload
     steps = args.steps if steps is None else steps
     w = workload_for(name, dtype, rank, world)
     kernel = args.kernel if kernel is None else kernel
     fast = bool(args.fast_math if fast is None else fast) and dtype == "f32"
-    leg = Leg(pkg, torch, w, name, dtype, fast, kernel, device, args.tensor_products)
-    products = 1 if fast else (3 if args.tensor_products == 3 else 2)
+    leg = Leg(pkg, torch, w, name, dtype, fast, kernel, device, args.tensor_products if tensor_products is None else tensor_products)
     pairs_step = w.pairs
     pairs_all = pairs_step
     if world > 1:
@@ -485,7 +510,8 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
     pipe_ops = 0.0
     if info["kernel"] == "factored":
         pipe_ops, _ = pipe_peak(1 if dtype == "f32" else 2, device)
-    rf = roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, name, products)
+    products = int(info.get("tensor_products", 0))     # what the library launched (0 = not the tensor kernel), never argv
+    rf = roofline(info["kernel"], dtype, fast, pairs_step, k_ms, pipe_ops, name, products, int(info.get("tensor_shape", 0)))
     es = 4 if dtype == "f32" else 8
     in_bytes = w.n_obs * 2 * es + (w.n_obj + 1) * 8
     out_bytes = w.n_obj * (2 * es + 8) if leg.best_only else w.n_obj * w.n_freq * es
@@ -496,6 +522,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
         rf["hbm_write_gbs"] = out_bytes / (k_ms * 1e-3) / 1e9
     out = {
         "dtype": dtype,
+        "arithmetic_dtype": arithmetic_dtype(info["kernel"], dtype, products), "tensor_products": products,
         "value": pairs_all * steps / (total_ms * 1e-3),
         "ms_per_step": ms_step,
         "kernel": info["kernel"], "n_split": info["n_split"], "fast_math": fast, "tensor_shape": info.get("tensor_shape", 0),
@@ -503,6 +530,7 @@ def run_leg(args, pkg, torch, dist, rank, world, device, dtype, flush, with_cloc
         "gpu_launches": dev_launches,
         "roofline": rf,
         "arithmetic": ARITHMETIC_3 if (info["kernel"] == "tensor" and products == 3) else ARITHMETIC.get((info["kernel"], fast), ""),
+        "io_dtype": dtype,
     }
     if world > 1 and name == "c3":
         obs = [torch.zeros(1, dtype=torch.int64, device="cuda") for _ in range(world)]
@@ -638,7 +666,7 @@ def run_c5(args, pkg, torch, device, flush):
                     kms += plan.last_kernel_ms() * steps / 3.0
                 info = plan.last_call_info()
                 rf = roofline(info["kernel"], dtype, args.fast_math and dtype == "f32", w.pairs, kms / steps, pipe_ops,
-                              products=1 if (args.fast_math and dtype == "f32") else (3 if args.tensor_products == 3 else 2))
+                              products=int(info.get("tensor_products", 0)), shape=int(info.get("tensor_shape", 0)))
                 rows.append({"dtype": dtype, "n_t": nt, "n_freq": nf, "pairs": w.pairs, "kernel": info["kernel"],
                              "n_split": info["n_split"], "ms_per_step": tot / steps, "kernel_ms": kms / steps,
                              "pairs_per_s": w.pairs * steps / (tot * 1e-3), "bound": rf["bound"], "roofline_frac": rf["frac"],
@@ -721,19 +749,48 @@ def run_b200(args, rank: int, world: int, local_rank: int):
     primary, w = run_leg(args, pkg, torch, dist, rank, world, local_rank, args.dtype, flush, True)
     solo = rank == 0 and world == 1
     secondary = not args.no_secondary and args.workload == "c2" and args.kernel == "auto" and not args.fast_math
-    other = fma = c3 = c4 = None
+    other = fma = two = c3 = c4 = fva = c5 = None
     variants = {}
     if secondary:
         other_dtype = "f64" if args.dtype == "f32" else "f32"
         other, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, other_dtype, flush, False)
         # the all-FP32 FFMA2 contraction on the FMA pipe: north_star's "FP32 issue-bound roofline" is answered by this kernel
-        fma, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, kernel="factored", fast=False,
-                         with_e2e=False)
+        fma, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, True, kernel="factored", fast=False,
+                         with_e2e=True)
+        # the two-product opt-in of the tensor path (lsp_config.tensor_products = 2): faster on long objects, not safe on
+        # few-night cadences -- a labelled leg, never the headline
+        if args.tensor_products != 2:
+            two, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, kernel="auto", fast=False,
+                             with_e2e=False, tensor_products=2)
         if solo:
             # BASELINE.json configs[2] and configs[3], short: the driver's record then carries them too
             c3, _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, workload="c3",
                             steps=max(3, min(args.steps, 10)))
             c4 = c4_overlap(args, pkg, torch, local_rank, flush, with_pageable=False)
+            # north_star: "fast-math __sincosf is compared against accurate sincos" (Table 6): the paper-shaped
+            # direct kernel with MUFU sincos vs sincospif, and the tensor path's fast_math mode vs its default
+            few = max(3, min(args.steps, 5))
+            legs = {}
+            for key, kern, fast_ in (("direct_sincosf", "direct", True), ("direct_accurate", "direct", False),
+                                     ("tensor_fast_math", "auto", True)):
+                legs[key], _ = run_leg(args, pkg, torch, dist, rank, world, local_rank, "f32", flush, False, kernel=kern,
+                                       fast=fast_, with_e2e=False, steps=few)
+            fva = {"unit": UNIT, "workload": "c2", "dtype": "f32", "cite": "PAPER.md:L423-433, Table 6 L451-459"}
+            for key, v in legs.items():
+                fva[key] = {"value": v["value"], "kernel_ms": v["kernel_ms_per_step"], "frac": v["roofline"]["frac"],
+                            "bound": v["roofline"]["bound"], "gpu_launches": v["gpu_launches"]}
+            fva["tensor_default"] = {"value": primary["value"], "kernel_ms": primary["kernel_ms_per_step"]}
+            fva["direct_speedup_fast_over_accurate"] = legs["direct_sincosf"]["value"] / legs["direct_accurate"]["value"]
+            fva["tensor_speedup_fast_over_default"] = legs["tensor_fast_math"]["value"] / primary["value"]
+            # BASELINE.json configs[4], compact: per dtype the 12 (N_t x N_f) points' pairs/s and roofline fraction, row-major
+            from workloads import C5_NT, C5_NF
+            rows = run_c5(args, pkg, torch, local_rank, flush)
+            c5 = {"n_t": list(C5_NT), "n_freq": list(C5_NF), "order": "n_t-major", "unit": UNIT}
+            for dt in ("f32", "f64"):
+                rr = [r for r in rows if r["dtype"] == dt]
+                c5[dt] = {"pairs_per_s": [float("%.4g" % r["pairs_per_s"]) for r in rr],
+                          "frac": [float("%.3g" % r["roofline_frac"]) for r in rr],
+                          "bound": sorted({r["bound"] for r in rr}), "kernel": sorted({r["kernel"] for r in rr})}
     if args.variants and args.workload == "c2":
         # fast_math tensor mode and the paper-shaped kernel (thread = frequency, one sincos per pair): __sincosf-class vs
         # accurate sincos, the comparison north_star asks for
@@ -775,10 +832,13 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             return {k: rf[k] for k in rf_keys if k in rf}
 
         def short_leg(v, with_e2e=True):
-            o = {"value": v["value"], "ms_per_step": v["ms_per_step"], "kernel_ms_per_step": v["kernel_ms_per_step"],
-                 "kernel": v["kernel"], "gpu_launches": v["gpu_launches"], "roofline": short_rf(v["roofline"])}
+            o = {"value": v["value"], "dtype": v["arithmetic_dtype"], "ms_per_step": v["ms_per_step"],
+                 "kernel_ms_per_step": v["kernel_ms_per_step"], "kernel": v["kernel"], "gpu_launches": v["gpu_launches"],
+                 "roofline": short_rf(v["roofline"])}
             if with_e2e and "e2e" in v:
                 o["e2e"] = v["e2e"]
+            if "clocks" in v:
+                o["clocks"] = v["clocks"]
             return o
 
         # the contract's keys first, so that a cut tail cannot lose them
@@ -786,8 +846,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
             "metric": METRIC, "value": primary["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": primary["ms_per_step"], "higher_is_better": True,
             "scaling": "strong" if sharded else "weak",
-            "vs_baseline": None, "dtype": primary["dtype"], "data": "synthetic",
+            # dtype = the arithmetic of the multiply-accumulates (an FP16-split tcgen05 contraction is not "f32"); io_dtype = t, y, P
+            "vs_baseline": None, "dtype": primary["arithmetic_dtype"], "data": "synthetic",
             "config": {"workload": describe_workload(args.workload, w), "kernel": primary["kernel"],
+                       "io_dtype": primary["io_dtype"], "tensor_products": primary["tensor_products"],
                        "arithmetic": primary["arithmetic"],
                        "fast_math": bool(args.fast_math and args.dtype == "f32"), "n_split": primary["n_split"],
                        "tensor_shape": primary["tensor_shape"],
@@ -803,9 +865,12 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         if other is not None:
             line["fp64" if other["dtype"] == "f64" else "fp32"] = short_leg(other)
         if fma is not None:
-            line["fp32_fma_pipe"] = {"value": fma["value"], "ms_per_step": fma["ms_per_step"], "frac": fma["roofline"]["frac"],
-                                     "achieved": fma["roofline"]["achieved"], "peak": fma["roofline"]["peak"], "unit": "TFLOP/s",
-                                     "bound": "alu", "kernel": fma["roofline"]["kernel"]}
+            # the all-FP32 answer to north_star's "FP32 issue-bound roofline": a full leg (roofline with traffic, e2e, clocks)
+            line["fp32_fma_pipe"] = short_leg(fma)
+            line["fp32_fma_pipe"]["frac"] = fma["roofline"]["frac"]
+        if two is not None:
+            line["fp32_tensor_2products"] = short_leg(two, with_e2e=False)
+            line["fp32_tensor_2products"]["note"] = "opt-in (lsp_config.tensor_products = 2); over the 1e-3 tolerance on few-night cadences"
         if c3 is not None:
             line["c3"] = {"value": c3["value"], "ms_per_step": c3["ms_per_step"], "kernel_ms_per_step": c3["kernel_ms_per_step"],
                           "frac": c3["roofline"]["frac"], "frac_executed": c3["roofline"].get("frac_executed"),
@@ -813,6 +878,10 @@ def run_b200(args, rank: int, world: int, local_rank: int):
         if c4 is not None:
             line["c4"] = {k: c4[k] for k in ("value", "T_compute_ms", "T_d2h_ms", "T_pipelined_ms", "T_over_max", "d2h_GBps",
                                              "fully_overlapped")}
+        if fva is not None:
+            line["fast_vs_accurate"] = fva
+        if c5 is not None:
+            line["c5"] = c5
         if overlap is not None:
             line["d2h_overlap"] = overlap
         if cpu is not None:

@@ -46,6 +46,32 @@ def test_pipe_peak_helper_builds_outside_the_library():
 def test_roofline_traffic_is_read_from_a_committed_capture():
     sys.path.insert(0, ROOT)
     import bench
-    b, src = bench.ncu_traffic("c2", "tensor", "f32")
+    # the tensor kernel's captures are keyed by its precision mode as well: another product count is another kernel
+    b, src = bench.ncu_traffic("c2", "tensor", "f32", 2)
     assert src is not None and os.path.exists(os.path.join(ROOT, src)) and b > 1e6
-    assert bench.ncu_traffic("c4", "tensor", "f32") == (None, None)
+    for key in bench.NCU_SUMMARIES:
+        got = bench.ncu_traffic(*key)
+        assert got == (None, None) or os.path.exists(os.path.join(ROOT, got[1]))
+    assert bench.ncu_traffic("c2", "tensor", "f32") == (None, None)       # no product count: no capture is claimed
+    assert bench.ncu_traffic("c4", "tensor", "f32", 3) == (None, None)
+
+
+def test_bench_line_names_the_arithmetic_and_the_real_instantiation():
+    """The line's `dtype` is the arithmetic of the multiply-accumulates and roofline.kernel the instantiation the library
+    launched, both derived from lsp_last_call_info (tensor_shape, tensor_products), never from argv."""
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.arithmetic_dtype("tensor", "f32", 3) == "f16x3-split/f32acc"
+    assert bench.arithmetic_dtype("tensor", "f32", 2) == "f16x2-split/f32acc"
+    assert bench.arithmetic_dtype("tensor", "f32", 1) == "f16/f32acc"
+    assert bench.arithmetic_dtype("factored", "f32", 0) == "f32" and bench.arithmetic_dtype("factored", "f64", 0) == "f64"
+    assert bench.tensor_instantiation(3, 3) == "lsp_tensor_kernel<float,0,4,4,0,true,112>"
+    assert bench.tensor_instantiation(3, 2) == "lsp_tensor_kernel<float,2,4,4,0,true,112>"
+    assert bench.tensor_instantiation(1, 3) == "lsp_tensor_kernel<float,0,8,3,0>"
+    assert bench.tensor_instantiation(2, 1) == "lsp_tensor_kernel<float,1,4,4,0>"
+    rf = bench.roofline("tensor", "f32", False, 1e10, 0.15, 0.0, "c2", products=3, shape=3)
+    assert rf["kernel"] == "lsp_tensor_kernel<float,0,4,4,0,true,112>" and rf["executed_flop_per_pair"] == 24.0
+    assert abs(rf["frac_executed"] - 3 * rf["frac"]) < 1e-12 and rf["bound"] == "tensor"
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    for key in ('"fp32_fma_pipe"', '"fp32_tensor_2products"', '"fast_vs_accurate"', '"c5"', '"io_dtype"', '"clocks"', '"e2e"'):
+        assert key in src, key
