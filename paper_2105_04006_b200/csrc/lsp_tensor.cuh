@@ -521,7 +521,7 @@ __host__ __device__ constexpr int tc_a_depth(int pm, int ew, int ng, bool pair, 
 // hundred threads per tile) are bound by the latency of their few loads in flight.
 constexpr int kTcFixThreads = 256;
 #ifndef LSP_TC_FIX_PARTS
-#define LSP_TC_FIX_PARTS 8
+#define LSP_TC_FIX_PARTS 16
 #endif
 constexpr int kTcFixParts = LSP_TC_FIX_PARTS;
 template <typename T>
@@ -559,7 +559,20 @@ lsp_tensor_fix_kernel(GridParams gp, TensorParams tp, const int64_t* __restrict_
 #pragma unroll
         for (int e = 0; e < 4; ++e) acc[e] = make_float4(0.f, 0.f, 0.f, 0.f);
         int sp = 0;
-        for (; sp + 2 <= gp.n_split; sp += 2) {                    // fixed order: split 0, 1, 2, ...; 8 loads in flight
+        for (; sp + 4 <= gp.n_split; sp += 4) {                    // fixed order: split 0, 1, 2, ...; 16 loads in flight (many-split
+            float4 v[4][4];                                        // launches are latency-bound here: few CTAs, long dependent chains)
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) v[q][e] = src[(int64_t)(sp + q) * sstride + e * 128];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    acc[e].x += v[q][e].x;  acc[e].y += v[q][e].y;  acc[e].z += v[q][e].z;  acc[e].w += v[q][e].w;
+                }
+        }
+        for (; sp + 2 <= gp.n_split; sp += 2) {                    // 8 loads in flight
             float4 v0[4], v1[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
