@@ -1277,7 +1277,7 @@ float lsp_last_kernel_ms(lsp_plan* p)
 
 const char* lsp_version(void)
 {
-    return "lsp-b200 0.5 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05 (A operands in TMEM, CTA pairs); modes: standard, generalised)";
+    return "lsp-b200 0.6 (sm_100a; kernels: direct, factored-ffma2, factored-dfma, tensor-tcgen05 (A operands in TMEM, CTA pairs; three FP16 products by default); modes: standard, generalised; allocation-free best period: lsp_best_period_static)";
 }
 
 }  // extern "C"
